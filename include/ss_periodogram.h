@@ -1,0 +1,170 @@
+/*
+ * ss_periodogram.h -- C ABI of the B200-native batched SuperSmoother periodogram.
+ *
+ * The operation is Algorithm 1 of arXiv 2111.07396 applied to every object of a
+ * catalog: per (object, trial frequency) phase-fold ("t1=(tt mod p)/p"), stable sort by
+ * phase, Friedman's variable-span smoother as Listing 1 states it (
+ * "cross validation") or the paper's single-pass generalized-validation variant (
+ * reading R12 in DESIGN.md), the chi-square statistic (reading R6) and the per-object
+ * argmax.  All arithmetic is IEEE fp64 on the GPU; there is no CPU fallback.
+ *
+ * Frequency grid (Table 2): half-open and evenly spaced,
+ *     df = (f_max - f_min) / n_freq,   f_k = f_min + k*df,   k = 0 .. n_freq-1,
+ * the same grid for every object.  Ordinary (not angular) frequency in 1/[time unit].
+ *
+ * Catalog layout (CSR): object i owns elements [offsets[i], offsets[i+1]) of times/mags/errs, in any
+ * time order.  Weights are 1/err^2.
+ *
+ * Periodogram value (R6):  P = (chi0 - chi2)/chi0,  chi0 = sum w (y - ybar_w)^2,
+ * chi2 = sum w (y - smo)^2.  Any positive-affine variant has the same argmax.
+ *
+ * Degenerate cases: an object with fewer than 5 points gets a NaN row, best_freq = NaN,
+ * best_index = -1.  chi0 == 0 (constant magnitudes) gives a row of zeros and best_index = 0.
+ * Argmax ties resolve to the lowest index.
+ *
+ * Errors: every entry point returns SS_OK or an error code; on error the outputs are unspecified
+ * (never partially trusted) and ss_last_error() (thread-local) describes the failure.  The library
+ * never frees or retains caller memory.
+ */
+#ifndef SS_PERIODOGRAM_H
+#define SS_PERIODOGRAM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SS_VERSION 100 /* 0.1.0 */
+
+typedef enum {
+    SS_MODE_CROSS_VALIDATION = 0,      /* Listing 1, PAPER.md:127-297 (paper: SSO-*)            */
+    SS_MODE_GENERALIZED_VALIDATION = 1 /* single-pass variant, PAPER.md:313-329 (paper: SSSP-*) */
+} ss_mode_t;
+
+typedef enum {
+    SS_OK = 0,
+    SS_ERR_INVALID_ARG = 1,   /* null pointer, bad sizes/grid, non-monotone offsets, non-finite data, err <= 0 */
+    SS_ERR_OUT_OF_MEMORY = 2, /* workspace could not be allocated / cap too small for one tile           */
+    SS_ERR_CUDA = 3,          /* a CUDA runtime call or kernel failed                                   */
+    SS_ERR_UNSUPPORTED = 4    /* option not implemented (iper = 2, fixed span: see DESIGN.md "next")     */
+} ss_status_t;
+
+/* Which kernel family serves an object (chosen by its number of points n). */
+typedef enum {
+    SS_PATH_AUTO = 0,
+    SS_PATH_WARP = 1,  /* one warp per (object, frequency); n <= SS_WARP_MAX_N; registers + shuffles   */
+    SS_PATH_BLOCK = 2, /* one CTA per (object, frequency); per-eval arrays in shared memory            */
+    SS_PATH_STAGE = 3  /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
+} ss_path_t;
+
+#define SS_WARP_MAX_N 256
+
+typedef struct {
+    double alpha;           /* bass enhancement.  Default 9.0.                 */
+    double span;            /* 0 = variable span (default).  > 0 (fixed span): UNSUPPORTED */
+    int iper;               /* 1 = non-periodic windows (default, R8).  2: UNSUPPORTED for now          */
+    int force_path;         /* ss_path_t; SS_PATH_AUTO = choose by n.  For tests and sweeps.            */
+    void *stream;           /* cudaStream_t the work is enqueued on (NULL = legacy default stream)      */
+    size_t workspace_cap;   /* bytes of device workspace the library may allocate; 0 = 75 % of free
+                               device memory (the paper's beta = 0.75)                    */
+    int64_t freq_tile;      /* host entry point only: force this many frequencies per output tile
+                               (0 = planner decides).  For tests.                                       */
+    int skip_validation;    /* 1 = trust the inputs (no device validation pass, no host sync for it)    */
+} ss_options_t;
+
+/* Fill *opt with the defaults listed above. */
+void ss_default_options(ss_options_t *opt);
+
+/*
+ * DEVICE-pointer entry point (PAPER.md:88-117 over a catalog).
+ *   times, mags, errs : const double[offsets[n_objects]]   device, read only
+ *   offsets           : const int64_t[n_objects + 1]       device, offsets[0] == 0, non-decreasing
+ *   pgram_out         : double[n_objects * n_freq] row-major device, or NULL (not materialised)
+ *   best_freq_out     : double[n_objects]  device, f_min + k* * df, or NULL
+ *   best_index_out    : int64_t[n_objects] device, k*, or NULL
+ * Work is enqueued on the legacy default stream; the call returns after it has completed.
+ */
+ss_status_t ss_periodogram(const double *times, const double *mags, const double *errs,
+                           const int64_t *offsets, int64_t n_objects,
+                           double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
+                           double *pgram_out, double *best_freq_out, int64_t *best_index_out);
+
+/* Same with options; enqueues on opt->stream and returns after that stream's work has completed. */
+ss_status_t ss_periodogram_ex(const double *times, const double *mags, const double *errs,
+                              const int64_t *offsets, int64_t n_objects,
+                              double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
+                              double *pgram_out, double *best_freq_out, int64_t *best_index_out,
+                              const ss_options_t *opt);
+
+/*
+ * HOST-pointer entry point: same operation, all array arguments are HOST pointers (pageable or
+ * pinned).  The library copies the catalog to the device, tiles objects x frequencies with the batch
+ * planner so the device-side periodogram tile plus workspace stays under opt->workspace_cap
+ * (the batching scheme), overlaps the device->host copy of finished tiles with the
+ * next tile's kernels, and returns when every output has landed in host memory.
+ */
+ss_status_t ss_periodogram_host(const double *times, const double *mags, const double *errs,
+                                const int64_t *offsets, int64_t n_objects,
+                                double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
+                                double *pgram_out, double *best_freq_out, int64_t *best_index_out,
+                                const ss_options_t *opt);
+
+/* ------------------------------------------------------------------ batch planner (host only) */
+
+typedef struct {
+    int64_t n_freq_tiles;     /* number of frequency tiles (the paper's N_b, Eq. 1)                    */
+    int64_t freq_per_tile;    /* frequencies per tile (last tile may be shorter)                       */
+    int64_t n_object_tiles;   /* number of object tiles                                                */
+    int64_t objects_per_tile; /* objects per tile (last may be shorter)                                */
+    size_t tile_bytes;        /* device bytes of one periodogram tile buffer (host entry point: x2)    */
+    size_t fixed_bytes;       /* catalog copy + per-object records + scheduler state                   */
+    size_t stage_bytes;       /* global staging scratch for SS_PATH_STAGE objects                      */
+    size_t total_bytes;       /* what the call will allocate                                           */
+} ss_plan_t;
+
+/*
+ * The plan ss_periodogram_host would use.  host_tiles != 0: output tiles are device buffers that are
+ * copied back (host entry point); 0: the caller's device pgram_out is written directly.
+ * Returns SS_ERR_OUT_OF_MEMORY if even a 1 x 1 tile does not fit under cap.
+ */
+ss_status_t ss_plan(int64_t n_points_total, int64_t max_n, int64_t n_objects, int64_t n_freq,
+                    ss_mode_t mode, size_t cap_bytes, int host_tiles, int want_pgram,
+                    ss_plan_t *plan_out);
+
+/* Device bytes the library allocates for a call (planner query; = plan.total_bytes). */
+size_t ss_workspace_bytes(int64_t n_points_total, int64_t max_n, int64_t n_objects,
+                          int64_t n_freq, ss_mode_t mode);
+
+/* The paper's own footprint model, for comparison and tests: bytes of its N_t*N_f layout
+ * (15*N_t*N_f words) and Eq. 1's N_b = ceil(r / (beta*s)) with r from
+ * PAPER.md:357/363 (FP64).  */
+double ss_paper_footprint_bytes(int64_t n_t, int64_t n_f);
+int64_t ss_paper_batches(int64_t n_t, int64_t n_f, ss_mode_t mode, double device_gib, double beta);
+
+/* Path class the library picks for an object of n points (SS_PATH_WARP/BLOCK/STAGE). */
+int ss_path_for_n(int64_t n, ss_mode_t mode);
+
+/* ------------------------------------------------------------------ diagnostics */
+
+/* Smoothed values of ONE (object, frequency) eval, in phase order, plus the permutation
+ * (device pointers; smo_out double[n], perm_out int32_t[n], either may be NULL).  Test hook. */
+ss_status_t ss_debug_eval(const double *times, const double *mags, const double *errs, int64_t n,
+                          double freq, ss_mode_t mode, const ss_options_t *opt,
+                          double *smo_out, int32_t *perm_out, double *p_out);
+
+/* Microbenchmarks used for the roofline denominators: sustained fp64 FMA
+ * rate (FLOP/s, 2 per DFMA) and shared-memory read bandwidth (B/s) of this device. */
+ss_status_t ss_microbench(double *fp64_flops_out, double *smem_bytes_per_s_out, void *stream);
+
+/* Kernel launches issued by this thread's most recent ss_periodogram* call. */
+int64_t ss_last_launch_count(void);
+
+const char *ss_last_error(void); /* thread-local, never NULL */
+int ss_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SS_PERIODOGRAM_H */

@@ -1,0 +1,748 @@
+// ss_api.cu -- C-ABI entry points, host driver (Algorithm 1, restructured so that
+// nothing is materialised at N_t*N_f), prep / argmax / fill kernels and the microbenchmarks.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/ss_periodogram.h"
+#include "ss_block_kernel.cuh"
+#include "ss_common.cuh"
+#include "ss_planner.h"
+#include "ss_warp_kernel.cuh"
+
+namespace ss {
+
+static thread_local std::string g_err = "";
+static thread_local int64_t g_launches = 0;
+
+static ss_status_t fail(ss_status_t st, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return st;
+}
+
+#define SS_CUDA(call)                                                                        \
+    do {                                                                                     \
+        cudaError_t e_ = (call);                                                             \
+        if (e_ != cudaSuccess)                                                               \
+            return fail(e_ == cudaErrorMemoryAllocation ? SS_ERR_OUT_OF_MEMORY : SS_ERR_CUDA, \
+                        "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// P0 prep: tt = t - min t, w = e^-2, ybar_w, chi0; yc = y - ybar_w.
+// One CTA per object.  Also validates: finite t, y, e and e > 0 (flag[0] |= 1 otherwise).
+// ------------------------------------------------------------------------------------------------
+constexpr int PREP_T = 256;
+
+__device__ __forceinline__ double prep_block_sum(double v, double* red)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+    for (int q = 0; q < PREP_T / 32; q++) s += red[q];
+    return s;
+}
+
+__global__ void __launch_bounds__(PREP_T) prep_kernel(const double* __restrict__ times,
+                                                      const double* __restrict__ mags,
+                                                      const double* __restrict__ errs, ObjRec* recs,
+                                                      int n_recs, double* tt, double* yc, double* w,
+                                                      int* flag)
+{
+    __shared__ double red[PREP_T / 32];
+    const int ri = blockIdx.x;
+    if (ri >= n_recs) return;
+    const int64_t off = recs[ri].off;
+    const int n = recs[ri].n;
+    const int tid = threadIdx.x;
+    double tmin = INFINITY;
+    int bad = 0;
+    for (int j = tid; j < n; j += PREP_T) {
+        double t = times[off + j], y = mags[off + j], e = errs[off + j];
+        if (!isfinite(t) || !isfinite(y) || !isfinite(e) || !(e > 0.0)) bad = 1;
+        tmin = fmin(tmin, t);
+    }
+    if (bad) atomicOr(flag, 1);
+    // block min
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) tmin = fmin(tmin, __shfl_xor_sync(0xffffffffu, tmin, d));
+    __syncthreads();
+    if ((tid & 31) == 0) red[tid >> 5] = tmin;
+    __syncthreads();
+    tmin = red[0];
+    for (int q = 1; q < PREP_T / 32; q++) tmin = fmin(tmin, red[q]);
+    double sw = 0.0, swy = 0.0;
+    // centre on the first magnitude before summing so the weighted mean keeps full precision
+    const double y0 = mags[off];
+    for (int j = tid; j < n; j += PREP_T) {
+        double e = errs[off + j];
+        double wj = 1.0 / (e * e);
+        w[off + j] = wj;
+        tt[off + j] = times[off + j] - tmin;
+        sw += wj;
+        swy += wj * (mags[off + j] - y0);
+    }
+    sw = prep_block_sum(sw, red);
+    swy = prep_block_sum(swy, red);
+    const double ybar = y0 + swy / sw;
+    double c0 = 0.0;
+    for (int j = tid; j < n; j += PREP_T) {
+        double d = mags[off + j] - ybar;
+        yc[off + j] = d;
+        c0 += w[off + j] * d * d;
+    }
+    c0 = prep_block_sum(c0, red);
+    if (tid == 0) {
+        recs[ri].chi0 = c0;
+        recs[ri].ybar = ybar;
+    }
+}
+
+// Fold one tile's partial maxima into the running best of each object (O8: first maximum wins).
+__global__ void fold_best_kernel(const ObjRec* recs, const int32_t* list, int n_list, int chunks,
+                                 int chunks_total, int chunk_base, const double* part_val,
+                                 const int64_t* part_idx, double* best_val, int64_t* best_idx)
+{
+    const int gw = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (gw >= n_list) return;
+    const int ri = list[gw];
+    double bv = -INFINITY;
+    int64_t bk = INT64_MAX;
+    for (int c = lane; c < chunks; c += 32) {
+        int64_t slot = (int64_t)ri * chunks_total + chunk_base + c;
+        double v = part_val[slot];
+        int64_t k = part_idx[slot];
+        if (v > bv || (v == bv && k < bk)) { bv = v; bk = k; }
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        double ov = __shfl_xor_sync(0xffffffffu, bv, d);
+        int64_t ok = __shfl_xor_sync(0xffffffffu, bk, d);
+        if (ov > bv || (ov == bv && ok < bk)) { bv = ov; bk = ok; }
+    }
+    if (lane == 0) {
+        const int64_t o = recs[ri].obj;
+        double cv = best_val[o];
+        int64_t ck = best_idx[o];
+        if (ck < 0 || bv > cv || (bv == cv && bk < ck)) { best_val[o] = bv; best_idx[o] = bk; }
+    }
+}
+
+__global__ void init_best_kernel(int64_t n, double* best_val, int64_t* best_idx)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) { best_val[i] = -INFINITY; best_idx[i] = -1; }
+}
+
+// best_index = k*, best_freq = f_min + k* df; objects that were never evaluated
+// (n < 5) keep index -1 and get NaN.
+__global__ void finish_kernel(int64_t n, const int64_t* best_idx, double f_min, double df,
+                              double* best_freq_out, int64_t* best_index_out)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int64_t k = best_idx[i];
+    if (best_index_out) best_index_out[i] = k;
+    if (best_freq_out) best_freq_out[i] = k >= 0 ? freq_of(f_min, df, k) : nan("");
+}
+
+// NaN rows for degenerate objects (n < 5).
+__global__ void nan_rows_kernel(const int64_t* rows, int n_rows, int64_t row0, int64_t width,
+                                int64_t stride, double* pgram)
+{
+    const int r = blockIdx.y;
+    if (r >= n_rows) return;
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < width) pgram[(rows[r] - row0) * stride + c] = nan("");
+}
+
+// ------------------------------------------------------------------------------------------------
+// Microbenchmarks for the roofline denominators.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double* out, int iters)
+{
+    double a[8];
+    const double m = 1.0000001, c = 1e-9;
+#pragma unroll
+    for (int i = 0; i < 8; i++) a[i] = threadIdx.x * 1e-3 + i;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 8; i++) a[i] = fma(a[i], m, c);
+    }
+    double s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) s += a[i];
+    if (s == 12345.678) out[0] = s;
+}
+
+__global__ void __launch_bounds__(256) smem_peak_kernel(double* out, int iters)
+{
+    __shared__ double buf[4096];
+    for (int i = threadIdx.x; i < 4096; i += 256) buf[i] = i;
+    __syncthreads();
+    double s = 0;
+    int idx = threadIdx.x;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            s += buf[(idx + u * 256) & 4095];
+        }
+        idx = (idx + 37) & 4095;
+    }
+    if (s == 12345.678) out[0] = s;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Engine: device state of one call.
+// ------------------------------------------------------------------------------------------------
+struct ClassList {
+    int path;               // SS_PATH_*
+    int variant;            // path-specific sub-class (warp: points per lane; block: smem tier)
+    std::vector<int32_t> recs;   // record indices, longest first
+    int64_t list_off = 0;   // offset into the device list array
+    int max_n = 0;
+};
+
+struct Engine {
+    cudaStream_t stream = nullptr;
+    ss_options_t opt{};
+    int mode = 0;
+    int64_t n_objects = 0, n_freq = 0, total = 0;
+    double f_min = 0, df = 0;
+    std::vector<int64_t> off;
+    std::vector<ObjRec> recs;          // objects with n >= 5
+    std::vector<int64_t> degenerate;   // object indices with n < 5
+    int max_n = 0;
+    // device workspace
+    char* ws = nullptr;
+    size_t ws_bytes = 0;
+    double *tt = nullptr, *yc = nullptr, *w = nullptr;
+    ObjRec* d_recs = nullptr;
+    int32_t* d_list = nullptr;
+    int64_t* d_degen = nullptr;
+    double* best_val = nullptr;
+    int64_t* best_idx = nullptr;
+    double* part_val = nullptr;
+    int64_t* part_idx = nullptr;
+    unsigned int* counters = nullptr;
+    int* flag = nullptr;
+    double* stage = nullptr;
+    char* extra = nullptr;            // caller-requested extra bytes (host entry point buffers)
+    int64_t stage_stride = 0;
+    int n_counters = 0, next_counter = 0;
+    ss_plan_t plan{};
+    // per object tile: class lists
+    std::vector<std::vector<ClassList>> tiles;
+    int sm_count = 148;
+
+    ~Engine() { if (ws) cudaFree(ws); }
+
+    ss_status_t setup(const double* times, const double* mags, const double* errs,
+                      const int64_t* offsets_host, int64_t n_obj, double fmin, double fmax,
+                      int64_t nfreq, int md, const ss_options_t& o, bool host_tiles, bool want_pgram,
+                      size_t extra_bytes);
+    ss_status_t run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int freq_tile_index,
+                         double* pgram, int64_t row_stride, int64_t row0, int64_t k0);
+    ss_status_t finish(double* best_freq_out, int64_t* best_index_out);
+};
+
+static ss_status_t validate_scalars(int64_t n_objects, double f_min, double f_max, int64_t n_freq,
+                                    int mode, const ss_options_t& o)
+{
+    if (n_objects < 0) return fail(SS_ERR_INVALID_ARG, "n_objects < 0");
+    if (n_freq < 1) return fail(SS_ERR_INVALID_ARG, "n_freq < 1");
+    if (!(f_min > 0.0) || !std::isfinite(f_min)) return fail(SS_ERR_INVALID_ARG, "f_min must be finite and > 0");
+    if (!(f_max > f_min) || !std::isfinite(f_max)) return fail(SS_ERR_INVALID_ARG, "f_max must be finite and > f_min");
+    if (mode != SS_MODE_CROSS_VALIDATION && mode != SS_MODE_GENERALIZED_VALIDATION)
+        return fail(SS_ERR_INVALID_ARG, "unknown mode %d", mode);
+    if (o.span != 0.0) return fail(SS_ERR_UNSUPPORTED, "fixed span is not implemented (DESIGN.md: next)");
+    if (o.iper != 1) return fail(SS_ERR_UNSUPPORTED, "iper = %d is not implemented (DESIGN.md: next)", o.iper);
+    if (!std::isfinite(o.alpha)) return fail(SS_ERR_INVALID_ARG, "alpha is not finite");
+    return SS_OK;
+}
+
+static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+ss_status_t Engine::setup(const double* times, const double* mags, const double* errs,
+                          const int64_t* offsets_host, int64_t n_obj, double fmin, double fmax,
+                          int64_t nfreq, int md, const ss_options_t& o, bool host_tiles,
+                          bool want_pgram, size_t extra_bytes)
+{
+    opt = o;
+    stream = (cudaStream_t)o.stream;
+    mode = md;
+    n_objects = n_obj;
+    n_freq = nfreq;
+    f_min = fmin;
+    df = (fmax - fmin) / (double)nfreq;
+    int dev = 0;
+    SS_CUDA(cudaGetDevice(&dev));
+    SS_CUDA(cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev));
+
+    off.assign(offsets_host, offsets_host + n_obj + 1);
+    if (n_obj > 0 && off[0] != 0) return fail(SS_ERR_INVALID_ARG, "offsets[0] != 0");
+    for (int64_t i = 0; i < n_obj; i++)
+        if (off[i + 1] < off[i]) return fail(SS_ERR_INVALID_ARG, "offsets not non-decreasing at %lld", (long long)i);
+    total = n_obj > 0 ? off[n_obj] : 0;
+    for (int64_t i = 0; i < n_obj; i++) {
+        int64_t n = off[i + 1] - off[i];
+        if (n > (int64_t)1 << 24) return fail(SS_ERR_UNSUPPORTED, "object %lld has %lld points (limit 2^24)", (long long)i, (long long)n);
+        if (n < MIN_POINTS) { degenerate.push_back(i); continue; }
+        ObjRec r{};
+        r.off = off[i]; r.obj = i; r.n = (int32_t)n;
+        r.ibw[0] = half_width(n, SPAN0); r.ibw[1] = half_width(n, SPAN1); r.ibw[2] = half_width(n, SPAN2);
+        r.q1 = (int32_t)(n / 4 - 1); r.q3 = 3 * (r.q1 + 1) - 1;
+        recs.push_back(r);
+        max_n = std::max(max_n, (int)n);
+    }
+
+    // ---- plan (P6)
+    size_t cap = o.workspace_cap;
+    if (cap == 0) {
+        size_t fr = 0, tot = 0;
+        SS_CUDA(cudaMemGetInfo(&fr, &tot));
+        cap = (size_t)(0.75 * (double)fr);   // the paper's beta
+    }
+    PlanInput pin{total, max_n, n_obj, nfreq, md, cap, host_tiles ? 1 : 0, want_pgram ? 1 : 0, o.freq_tile};
+    ss_status_t st = make_plan(pin, &plan);
+    if (st != SS_OK) return fail(st, "workspace cap %zu B too small for the smallest tile", cap);
+
+    // ---- class lists per object tile
+    const int n_ot = (int)std::max<int64_t>(plan.n_object_tiles, 1);
+    tiles.assign(n_ot, {});
+    std::vector<int32_t> all_lists;
+    for (int t = 0; t < n_ot; t++) {
+        const int64_t o0 = (int64_t)t * plan.objects_per_tile, o1 = std::min(n_obj, o0 + plan.objects_per_tile);
+        std::vector<ClassList> cls;
+        auto find = [&](int path, int variant) -> ClassList& {
+            for (auto& c : cls) if (c.path == path && c.variant == variant) return c;
+            cls.push_back(ClassList{path, variant, {}, 0, 0});
+            return cls.back();
+        };
+        for (size_t ri = 0; ri < recs.size(); ri++) {
+            const ObjRec& r = recs[ri];
+            if (r.obj < o0 || r.obj >= o1) continue;
+            int path = o.force_path != SS_PATH_AUTO ? o.force_path : path_for_n(r.n, md);
+            if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_BLOCK;
+            if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
+            int variant = 0;
+            if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
+            else if (path == SS_PATH_BLOCK) variant = r.n <= 500 ? 0 : (r.n <= 1020 ? 1 : 2);
+            ClassList& c = find(path, variant);
+            c.recs.push_back((int32_t)ri);
+            c.max_n = std::max(c.max_n, (int)r.n);
+        }
+        for (auto& c : cls) {
+            std::stable_sort(c.recs.begin(), c.recs.end(),
+                             [&](int32_t a, int32_t b) { return recs[a].n > recs[b].n; });
+            c.list_off = (int64_t)all_lists.size();
+            all_lists.insert(all_lists.end(), c.recs.begin(), c.recs.end());
+        }
+        tiles[t] = std::move(cls);
+    }
+
+    // ---- workspace
+    const bool need_stage = max_n > BLOCK_MAX_N || o.force_path == SS_PATH_STAGE;
+    stage_stride = need_stage ? BLOCK_SLOTS * block_slot_len(max_n) : 0;
+    const int stage_ctas = sm_count * 2;
+    const int64_t cpo = chunks_per_object(plan.objects_per_tile, plan.freq_per_tile);
+    n_counters = 64;
+    size_t b = 0;
+    auto carve = [&](size_t bytes) { size_t o_ = b; b += align_up(bytes); return o_; };
+    size_t o_tt = carve(8 * (size_t)total), o_yc = carve(8 * (size_t)total), o_w = carve(8 * (size_t)total);
+    size_t o_recs = carve(sizeof(ObjRec) * std::max<size_t>(recs.size(), 1));
+    size_t o_list = carve(4 * std::max<size_t>(all_lists.size(), 1));
+    size_t o_deg = carve(8 * std::max<size_t>(degenerate.size(), 1));
+    size_t o_bv = carve(8 * (size_t)std::max<int64_t>(n_obj, 1)), o_bi = carve(8 * (size_t)std::max<int64_t>(n_obj, 1));
+    size_t o_pv = carve(8 * std::max<size_t>(recs.size(), 1) * (size_t)cpo), o_pi = carve(8 * std::max<size_t>(recs.size(), 1) * (size_t)cpo);
+    size_t o_cnt = carve(4 * (size_t)n_counters), o_flag = carve(64);
+    size_t o_stage = carve(need_stage ? 8 * (size_t)stage_stride * (size_t)stage_ctas : 0);
+    size_t o_extra = carve(extra_bytes);
+    ws_bytes = b;
+    if (ws_bytes > cap + (64 << 20))
+        return fail(SS_ERR_OUT_OF_MEMORY, "workspace %zu B exceeds the cap %zu B", ws_bytes, cap);
+    SS_CUDA(cudaMalloc((void**)&ws, ws_bytes));
+    tt = (double*)(ws + o_tt); yc = (double*)(ws + o_yc); w = (double*)(ws + o_w);
+    d_recs = (ObjRec*)(ws + o_recs); d_list = (int32_t*)(ws + o_list); d_degen = (int64_t*)(ws + o_deg);
+    best_val = (double*)(ws + o_bv); best_idx = (int64_t*)(ws + o_bi);
+    part_val = (double*)(ws + o_pv); part_idx = (int64_t*)(ws + o_pi);
+    counters = (unsigned int*)(ws + o_cnt); flag = (int*)(ws + o_flag);
+    stage = need_stage ? (double*)(ws + o_stage) : nullptr;
+    extra = ws + o_extra;
+
+    if (!recs.empty()) SS_CUDA(cudaMemcpyAsync(d_recs, recs.data(), sizeof(ObjRec) * recs.size(), cudaMemcpyHostToDevice, stream));
+    if (!all_lists.empty()) SS_CUDA(cudaMemcpyAsync(d_list, all_lists.data(), 4 * all_lists.size(), cudaMemcpyHostToDevice, stream));
+    if (!degenerate.empty()) SS_CUDA(cudaMemcpyAsync(d_degen, degenerate.data(), 8 * degenerate.size(), cudaMemcpyHostToDevice, stream));
+    SS_CUDA(cudaMemsetAsync(counters, 0, 4 * (size_t)n_counters, stream));
+    SS_CUDA(cudaMemsetAsync(flag, 0, 64, stream));
+    if (n_obj > 0) {
+        init_best_kernel<<<(unsigned)((n_obj + 255) / 256), 256, 0, stream>>>(n_obj, best_val, best_idx);
+        g_launches++;
+    }
+    if (!recs.empty()) {
+        prep_kernel<<<(unsigned)recs.size(), PREP_T, 0, stream>>>(times, mags, errs, d_recs, (int)recs.size(), tt, yc, w, flag);
+        g_launches++;
+        SS_CUDA(cudaGetLastError());
+    }
+    if (!o.skip_validation) {
+        int h_flag = 0;
+        SS_CUDA(cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream));
+        SS_CUDA(cudaStreamSynchronize(stream));
+        if (h_flag) return fail(SS_ERR_INVALID_ARG, "non-finite time/magnitude/error or error <= 0 in the catalog");
+    }
+    return SS_OK;
+}
+
+template <typename K>
+static ss_status_t set_smem(K kernel, size_t bytes)
+{
+    if (bytes > 48 * 1024)
+        SS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return SS_OK;
+}
+
+ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int freq_tile_index,
+                             double* pgram, int64_t row_stride, int64_t row0, int64_t k0)
+{
+    (void)freq_tile_index;
+    if (tiles.empty()) return SS_OK;
+    const int64_t nk = k_end - k_begin;
+    const int64_t o0 = (int64_t)obj_tile * plan.objects_per_tile, o1 = std::min(n_objects, o0 + plan.objects_per_tile);
+    const int64_t cpo_cap = chunks_per_object(plan.objects_per_tile, plan.freq_per_tile);
+    for (ClassList& c : tiles[obj_tile]) {
+        if (c.recs.empty()) continue;
+        EvalParams p{};
+        p.tt = tt; p.yc = yc; p.w = w; p.recs = d_recs;
+        p.list = d_list + c.list_off; p.n_list = (int32_t)c.recs.size();
+        p.f_min = f_min; p.df = df; p.k_begin = k_begin; p.k_end = k_end;
+        int64_t cpo = std::min<int64_t>(cpo_cap, nk);
+        int64_t chunk = (nk + cpo - 1) / cpo;
+        if (c.path == SS_PATH_WARP) chunk = (chunk + WARPS_PER_CTA - 1) / WARPS_PER_CTA * WARPS_PER_CTA;
+        cpo = (nk + chunk - 1) / chunk;
+        p.chunk = (int32_t)chunk; p.chunks_per_obj = (int32_t)cpo;
+        p.chunks_total = (int32_t)cpo_cap; p.chunk_base = 0;
+        p.alpha = opt.alpha; p.mode = mode;
+        p.pgram = pgram; p.pgram_row_stride = row_stride; p.pgram_k0 = k0; p.pgram_row0 = row0;
+        p.part_val = part_val; p.part_idx = part_idx;
+        p.counter = counters + (next_counter % n_counters);
+        p.stage = stage; p.stage_stride = stage_stride;
+        const int64_t n_items = (int64_t)p.n_list * cpo;
+        if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
+        if (c.path == SS_PATH_WARP) {
+            ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
+            if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        } else {
+            SS_CUDA(cudaMemsetAsync(p.counter, 0, 4, stream));
+            next_counter++;
+            if (c.path == SS_PATH_BLOCK) {
+                const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(c.max_n) * 8;
+                if (c.variant == 2) {
+                    SS_CUDA(cudaFuncSetAttribute(block_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    int grid = (int)std::min<int64_t>(n_items, sm_count);
+                    block_kernel<512, false><<<grid, 512, smem, stream>>>(p);
+                } else {
+                    SS_CUDA(cudaFuncSetAttribute(block_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    int per_sm = c.variant == 0 ? 4 : 2;
+                    int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * per_sm);
+                    block_kernel<256, false><<<grid, 256, smem, stream>>>(p);
+                }
+            } else {
+                int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 2);
+                block_kernel<512, true><<<grid, 512, 0, stream>>>(p);
+            }
+        }
+        g_launches++;
+        SS_CUDA(cudaGetLastError());
+        fold_best_kernel<<<(unsigned)((p.n_list * 32 + 255) / 256), 256, 0, stream>>>(
+            d_recs, p.list, p.n_list, (int)cpo, p.chunks_total, 0, part_val, part_idx, best_val, best_idx);
+        g_launches++;
+        SS_CUDA(cudaGetLastError());
+    }
+    // NaN rows of degenerate objects in this tile
+    if (pgram && !degenerate.empty()) {
+        // degenerate[] is sorted; select the sub-range inside [o0, o1)
+        auto lo = std::lower_bound(degenerate.begin(), degenerate.end(), o0);
+        auto hi = std::lower_bound(degenerate.begin(), degenerate.end(), o1);
+        int n_rows = (int)(hi - lo);
+        for (int r0 = 0; r0 < n_rows; r0 += 65535) {
+            int nr = std::min(65535, n_rows - r0);
+            dim3 grid((unsigned)((nk + 255) / 256), (unsigned)nr);
+            nan_rows_kernel<<<grid, 256, 0, stream>>>(d_degen + (lo - degenerate.begin()) + r0, nr, row0,
+                                                      nk, row_stride, pgram + (k_begin - k0));
+            g_launches++;
+        }
+        SS_CUDA(cudaGetLastError());
+    }
+    return SS_OK;
+}
+
+ss_status_t Engine::finish(double* best_freq_out, int64_t* best_index_out)
+{
+    if (n_objects > 0 && (best_freq_out || best_index_out)) {
+        finish_kernel<<<(unsigned)((n_objects + 255) / 256), 256, 0, stream>>>(n_objects, best_idx, f_min, df,
+                                                                              best_freq_out, best_index_out);
+        g_launches++;
+        SS_CUDA(cudaGetLastError());
+    }
+    return SS_OK;
+}
+
+}  // namespace ss
+
+// ================================================================================================
+// C ABI
+// ================================================================================================
+using namespace ss;
+
+extern "C" {
+
+void ss_default_options(ss_options_t* opt)
+{
+    if (!opt) return;
+    memset(opt, 0, sizeof *opt);
+    opt->alpha = 9.0;
+    opt->span = 0.0;
+    opt->iper = 1;      // DESIGN.md R8
+    opt->force_path = SS_PATH_AUTO;
+}
+
+const char* ss_last_error(void) { return g_err.c_str(); }
+int ss_version(void) { return SS_VERSION; }
+int64_t ss_last_launch_count(void) { return g_launches; }
+int ss_path_for_n(int64_t n, ss_mode_t mode) { return path_for_n(n, (int)mode); }
+double ss_paper_footprint_bytes(int64_t n_t, int64_t n_f) { return paper_footprint_bytes(n_t, n_f); }
+int64_t ss_paper_batches(int64_t n_t, int64_t n_f, ss_mode_t mode, double device_gib, double beta)
+{
+    return paper_batches(n_t, n_f, (int)mode, device_gib, beta);
+}
+
+ss_status_t ss_plan(int64_t n_points_total, int64_t max_n, int64_t n_objects, int64_t n_freq,
+                    ss_mode_t mode, size_t cap_bytes, int host_tiles, int want_pgram, ss_plan_t* plan_out)
+{
+    if (!plan_out) return fail(SS_ERR_INVALID_ARG, "plan_out is null");
+    if (n_points_total < 0 || max_n < 0 || n_objects < 0 || n_freq < 1)
+        return fail(SS_ERR_INVALID_ARG, "negative size");
+    PlanInput in{n_points_total, max_n, n_objects, n_freq, (int)mode, cap_bytes, host_tiles, want_pgram, 0};
+    ss_status_t st = make_plan(in, plan_out);
+    if (st != SS_OK) return fail(st, "cap %zu B too small", cap_bytes);
+    return SS_OK;
+}
+
+size_t ss_workspace_bytes(int64_t n_points_total, int64_t max_n, int64_t n_objects, int64_t n_freq,
+                          ss_mode_t mode)
+{
+    ss_plan_t pl{};
+    PlanInput in{n_points_total, max_n, n_objects, n_freq, (int)mode, (size_t)-1, 0, 0, 0};
+    if (make_plan(in, &pl) != SS_OK) return 0;
+    return pl.total_bytes;
+}
+
+ss_status_t ss_periodogram_ex(const double* times, const double* mags, const double* errs,
+                              const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                              int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                              int64_t* best_index_out, const ss_options_t* opt_in)
+{
+    g_launches = 0;
+    ss_options_t o;
+    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    ss_status_t st = validate_scalars(n_objects, f_min, f_max, n_freq, (int)mode, o);
+    if (st != SS_OK) return st;
+    if (!offsets) return fail(SS_ERR_INVALID_ARG, "offsets is null");
+    if (n_objects == 0) return SS_OK;
+    cudaStream_t stream = (cudaStream_t)o.stream;
+    std::vector<int64_t> off((size_t)n_objects + 1);
+    SS_CUDA(cudaMemcpyAsync(off.data(), offsets, 8 * ((size_t)n_objects + 1), cudaMemcpyDeviceToHost, stream));
+    SS_CUDA(cudaStreamSynchronize(stream));
+    if (off[n_objects] > 0 && (!times || !mags || !errs)) return fail(SS_ERR_INVALID_ARG, "times/mags/errs is null");
+    Engine eng;
+    st = eng.setup(times, mags, errs, off.data(), n_objects, f_min, f_max, n_freq, (int)mode, o, false,
+                   pgram_out != nullptr, 0);
+    if (st != SS_OK) return st;
+    // device output: the caller's array is written directly; frequency tiles only bound the
+    // partial-argmax rows
+    for (int ot = 0; ot < (int)eng.tiles.size(); ot++) {
+        for (int64_t ft = 0; ft < eng.plan.n_freq_tiles; ft++) {
+            int64_t k0 = ft * eng.plan.freq_per_tile, k1 = std::min(n_freq, k0 + eng.plan.freq_per_tile);
+            st = eng.run_tile(ot, k0, k1, (int)ft, pgram_out, n_freq, 0, 0);
+            if (st != SS_OK) return st;
+        }
+    }
+    st = eng.finish(best_freq_out, best_index_out);
+    if (st != SS_OK) return st;
+    SS_CUDA(cudaStreamSynchronize(stream));
+    return SS_OK;
+}
+
+ss_status_t ss_periodogram(const double* times, const double* mags, const double* errs,
+                           const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                           int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                           int64_t* best_index_out)
+{
+    return ss_periodogram_ex(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                             best_freq_out, best_index_out, nullptr);
+}
+
+ss_status_t ss_periodogram_host(const double* times, const double* mags, const double* errs,
+                                const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                                int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                                int64_t* best_index_out, const ss_options_t* opt_in)
+{
+    g_launches = 0;
+    ss_options_t o;
+    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    ss_status_t st = validate_scalars(n_objects, f_min, f_max, n_freq, (int)mode, o);
+    if (st != SS_OK) return st;
+    if (!offsets) return fail(SS_ERR_INVALID_ARG, "offsets is null");
+    if (n_objects == 0) return SS_OK;
+    for (int64_t i = 0; i < n_objects; i++)
+        if (offsets[i + 1] < offsets[i]) return fail(SS_ERR_INVALID_ARG, "offsets not non-decreasing");
+    const int64_t total = offsets[n_objects];
+    if (total > 0 && (!times || !mags || !errs)) return fail(SS_ERR_INVALID_ARG, "times/mags/errs is null");
+    cudaStream_t stream = (cudaStream_t)o.stream;
+
+    Engine eng;
+    // raw catalog copy + best outputs live in the engine's workspace ("extra")
+    const size_t raw_b = align_up(8 * (size_t)total);
+    const size_t out_b = align_up(8 * (size_t)n_objects);
+    // the raw copy must exist before setup() runs the prep kernel: allocate it separately first
+    char* raw = nullptr;
+    SS_CUDA(cudaMalloc((void**)&raw, 3 * raw_b + 2 * out_b + 256));
+    struct Guard { char* p; ~Guard() { if (p) cudaFree(p); } } guard{raw};
+    double* d_t = (double*)raw; double* d_y = (double*)(raw + raw_b); double* d_e = (double*)(raw + 2 * raw_b);
+    double* d_bf = (double*)(raw + 3 * raw_b); int64_t* d_bi = (int64_t*)(raw + 3 * raw_b + out_b);
+    if (total > 0) {
+        SS_CUDA(cudaMemcpyAsync(d_t, times, 8 * (size_t)total, cudaMemcpyHostToDevice, stream));
+        SS_CUDA(cudaMemcpyAsync(d_y, mags, 8 * (size_t)total, cudaMemcpyHostToDevice, stream));
+        SS_CUDA(cudaMemcpyAsync(d_e, errs, 8 * (size_t)total, cudaMemcpyHostToDevice, stream));
+    }
+    st = eng.setup(d_t, d_y, d_e, offsets, n_objects, f_min, f_max, n_freq, (int)mode, o, true,
+                   pgram_out != nullptr, pgram_out ? 0 : 0);
+    if (st != SS_OK) return st;
+
+    // periodogram tiles: two device buffers, D2H of tile i overlaps the kernels of tile i+1
+    double* tile_buf[2] = {nullptr, nullptr};
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t done[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+    struct TileRes {
+        double** b; cudaStream_t* s; cudaEvent_t* d; cudaEvent_t* c;
+        ~TileRes() {
+            for (int i = 0; i < 2; i++) { if (b[i]) cudaFree(b[i]); if (d[i]) cudaEventDestroy(d[i]); if (c[i]) cudaEventDestroy(c[i]); }
+            if (*s) cudaStreamDestroy(*s);
+        }
+    } tres{tile_buf, &copy_stream, done, copied};
+    if (pgram_out) {
+        for (int i = 0; i < 2; i++) {
+            SS_CUDA(cudaMalloc((void**)&tile_buf[i], std::max<size_t>(eng.plan.tile_bytes, 8)));
+            SS_CUDA(cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming));
+            SS_CUDA(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
+        }
+        SS_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+    }
+    int it = 0;
+    for (int ot = 0; ot < (int)eng.tiles.size(); ot++) {
+        const int64_t o0 = (int64_t)ot * eng.plan.objects_per_tile;
+        const int64_t o1 = std::min(n_objects, o0 + eng.plan.objects_per_tile);
+        for (int64_t ft = 0; ft < eng.plan.n_freq_tiles; ft++, it++) {
+            const int64_t k0 = ft * eng.plan.freq_per_tile, k1 = std::min(n_freq, k0 + eng.plan.freq_per_tile);
+            const int bi = it & 1;
+            double* tb = pgram_out ? tile_buf[bi] : nullptr;
+            if (pgram_out && it >= 2) SS_CUDA(cudaStreamWaitEvent(stream, copied[bi], 0));
+            st = eng.run_tile(ot, k0, k1, (int)ft, tb, k1 - k0, o0, k0);
+            if (st != SS_OK) return st;
+            if (pgram_out) {
+                SS_CUDA(cudaEventRecord(done[bi], stream));
+                SS_CUDA(cudaStreamWaitEvent(copy_stream, done[bi], 0));
+                SS_CUDA(cudaMemcpy2DAsync(pgram_out + o0 * n_freq + k0, 8 * (size_t)n_freq, tb, 8 * (size_t)(k1 - k0),
+                                          8 * (size_t)(k1 - k0), (size_t)(o1 - o0), cudaMemcpyDeviceToHost, copy_stream));
+                SS_CUDA(cudaEventRecord(copied[bi], copy_stream));
+            }
+        }
+    }
+    st = eng.finish(best_freq_out ? d_bf : nullptr, best_index_out ? d_bi : nullptr);
+    if (st != SS_OK) return st;
+    if (best_freq_out) SS_CUDA(cudaMemcpyAsync(best_freq_out, d_bf, 8 * (size_t)n_objects, cudaMemcpyDeviceToHost, stream));
+    if (best_index_out) SS_CUDA(cudaMemcpyAsync(best_index_out, d_bi, 8 * (size_t)n_objects, cudaMemcpyDeviceToHost, stream));
+    SS_CUDA(cudaStreamSynchronize(stream));
+    if (copy_stream) SS_CUDA(cudaStreamSynchronize(copy_stream));
+    return SS_OK;
+}
+
+ss_status_t ss_debug_eval(const double* times, const double* mags, const double* errs, int64_t n,
+                          double freq, ss_mode_t mode, const ss_options_t* opt_in, double* smo_out,
+                          int32_t* perm_out, double* p_out)
+{
+    g_launches = 0;
+    ss_options_t o;
+    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    ss_status_t st = validate_scalars(1, freq, freq * 2 + 1, 1, (int)mode, o);
+    if (st != SS_OK) return st;
+    if (n < MIN_POINTS) return fail(SS_ERR_INVALID_ARG, "n < 5");
+    if (!times || !mags || !errs) return fail(SS_ERR_INVALID_ARG, "null input");
+    int64_t off[2] = {0, n};
+    o.force_path = SS_PATH_STAGE;
+    Engine eng;
+    st = eng.setup(times, mags, errs, off, 1, freq, freq * 2 + 1, 1, (int)mode, o, false, false, 0);
+    if (st != SS_OK) return st;
+    EvalParams p{};
+    p.tt = eng.tt; p.yc = eng.yc; p.w = eng.w; p.recs = eng.d_recs; p.alpha = o.alpha; p.mode = (int)mode;
+    p.stage = eng.stage; p.stage_stride = eng.stage_stride;
+    block_debug_kernel<512><<<1, 512, 0, eng.stream>>>(p, freq, smo_out, perm_out, p_out);
+    g_launches++;
+    SS_CUDA(cudaGetLastError());
+    SS_CUDA(cudaStreamSynchronize(eng.stream));
+    return SS_OK;
+}
+
+ss_status_t ss_microbench(double* fp64_flops_out, double* smem_bytes_per_s_out, void* stream_v)
+{
+    cudaStream_t stream = (cudaStream_t)stream_v;
+    int dev = 0, sms = 0;
+    SS_CUDA(cudaGetDevice(&dev));
+    SS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    double* d = nullptr;
+    SS_CUDA(cudaMalloc((void**)&d, 64));
+    cudaEvent_t e0, e1;
+    SS_CUDA(cudaEventCreate(&e0));
+    SS_CUDA(cudaEventCreate(&e1));
+    const int grid = sms * 8, iters = 1 << 15;
+    float ms = 0, best = 1e30f;
+    for (int rep = 0; rep < 5; rep++) {
+        SS_CUDA(cudaEventRecord(e0, stream));
+        fp64_peak_kernel<<<grid, 256, 0, stream>>>(d, iters);
+        SS_CUDA(cudaEventRecord(e1, stream));
+        SS_CUDA(cudaEventSynchronize(e1));
+        SS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    if (fp64_flops_out) *fp64_flops_out = 2.0 * 8.0 * (double)iters * 256.0 * grid / (best * 1e-3);
+    best = 1e30f;
+    for (int rep = 0; rep < 5; rep++) {
+        SS_CUDA(cudaEventRecord(e0, stream));
+        smem_peak_kernel<<<grid, 256, 0, stream>>>(d, iters);
+        SS_CUDA(cudaEventRecord(e1, stream));
+        SS_CUDA(cudaEventSynchronize(e1));
+        SS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best) best = ms;
+    }
+    if (smem_bytes_per_s_out) *smem_bytes_per_s_out = 8.0 * 8.0 * (double)iters * 256.0 * grid / (best * 1e-3);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    return SS_OK;
+}
+
+}  // extern "C"

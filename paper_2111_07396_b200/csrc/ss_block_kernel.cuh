@@ -1,0 +1,465 @@
+// ss_block_kernel.cuh -- one CTA per (object, frequency) eval; any n.
+//
+// Serves the SS_PATH_BLOCK (per-eval arrays in shared memory) and SS_PATH_STAGE (arrays staged in
+// global memory / L2, for light curves that do not fit one SM's shared memory) classes.  Persistent
+// CTAs pull (object, frequency-chunk) work items from an atomic counter, longest objects first.
+//
+// Per eval: fold -> bitonic sort of (phase bits, index) -> gather ->
+// exclusive prefix sums of the weighted moments -> windowed line fits by prefix differences
+// (three spans) -> CV: LOO residuals, residual smooths, span pick, span smooth, interpolation, final
+// smooth (Listing 1) / GV: scores, pick, interpolation (R12) -> chi2 -> P.
+#pragma once
+#include "ss_common.cuh"
+
+namespace ss {
+
+constexpr int BLOCK_SLOTS = 14;  // per-eval arrays of (n+2) doubles each
+
+__host__ __device__ inline int64_t block_slot_len(int n) { return ((int64_t)n + 2) & ~(int64_t)1; }
+
+template <int T>
+struct BlockCtx {
+    static constexpr int NW = T / 32;
+    double (*wsum)[NW];   // [6][NW] cross-warp scan scratch
+    double* red;          // [NW]
+    int* flags;           // [4]: has_ties, bad0, bad1, bad2
+};
+
+// Exclusive prefix sums of NA value streams at once; E[a][0..n], E[a][n] = total.
+template <int T, int NA, typename F>
+__device__ __forceinline__ void block_scan(int n, F vals, double* const (&E)[NA], double (*wsum)[T / 32])
+{
+    constexpr int NW = T / 32;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    double carry[NA];
+#pragma unroll
+    for (int a = 0; a < NA; a++) carry[a] = 0.0;
+    for (int base = 0; base < n; base += T) {
+        const int j = base + tid;
+        double v[NA], inc[NA];
+        if (j < n) vals(j, v);
+        else {
+#pragma unroll
+            for (int a = 0; a < NA; a++) v[a] = 0.0;
+        }
+#pragma unroll
+        for (int a = 0; a < NA; a++) {
+            double s = v[a];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                double o = __shfl_up_sync(0xffffffffu, s, d);
+                if (lane >= d) s += o;
+            }
+            inc[a] = s;
+            if (lane == 31) wsum[a][warp] = s;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int a = 0; a < NA; a++) {
+            double woff = 0.0, tot = 0.0;
+#pragma unroll
+            for (int q = 0; q < NW; q++) {
+                double s = wsum[a][q];
+                if (q < warp) woff += s;
+                tot += s;
+            }
+            if (j < n) E[a][j] = carry[a] + woff + (inc[a] - v[a]);
+            carry[a] += tot;
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+#pragma unroll
+        for (int a = 0; a < NA; a++) E[a][n] = carry[a];
+    }
+    __syncthreads();
+}
+
+template <int T>
+__device__ __forceinline__ double block_sum(double v, double* red)
+{
+    constexpr int NW = T / 32;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < NW; q++) s += red[q];
+    return s;
+}
+
+// Average z over maximal runs of equal keys, w-weighted (O4 last bullet).  Serial, one thread:
+// exact ties in phase are rare (structured time stamps), this is the slow-but-exact path.
+__device__ inline void tie_average_serial(int n, const unsigned long long* key, const double* w, double* z)
+{
+    int j = 0;
+    while (j < n) {
+        int j0 = j;
+        double sy = z[j] * w[j], fbw = w[j];
+        while (j < n - 1 && key[j + 1] <= key[j]) {
+            j++;
+            sy += w[j] * z[j];
+            fbw += w[j];
+        }
+        if (j > j0) {
+            double a = fbw > 0.0 ? sy / fbw : 0.0;
+            for (int i = j0; i <= j; i++) z[i] = a;
+        }
+        j++;
+    }
+}
+
+// Replace the -1 sentinels of the LOO residuals by the previous valid value (R23).
+__device__ inline void carry_fix_serial(int n, double* r)
+{
+    for (int j = 0; j < n; j++)
+        if (r[j] < 0.0) r[j] = j > 0 ? r[j - 1] : 0.0;
+}
+
+// Compare-exchange on (key, idx), ascending, lexicographic: exact stable order (R13).
+__device__ __forceinline__ void cex(unsigned long long* key, unsigned int* idx, int a, int b)
+{
+    unsigned long long ka = key[a], kb = key[b];
+    unsigned int ia = idx[a], ib = idx[b];
+    if (kb < ka || (kb == ka && ib < ia)) {
+        key[a] = kb; key[b] = ka;
+        idx[a] = ib; idx[b] = ia;
+    }
+}
+
+// One eval.  S = base of BLOCK_SLOTS arrays of `sl` doubles (shared or global memory).
+// Returns P (valid in every thread).  If smo_dbg != null the smooth (phase order, un-centred) and the
+// permutation are written out (ss_debug_eval).
+template <int T>
+__device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, double* S, int64_t sl,
+                             const BlockCtx<T>& cx, double* smo_dbg, int32_t* perm_dbg)
+{
+    const int tid = threadIdx.x;
+    const int n = rec.n;
+    const double* tt = p.tt + rec.off;
+    const double* yc = p.yc + rec.off;
+    const double* wo = p.w + rec.off;
+
+    double* x = S;                 double* ys = S + sl;           double* ws = S + 2 * sl;
+    double* Ew = S + 3 * sl;       double* Ewx = S + 4 * sl;      double* Ewxx = S + 5 * sl;
+    double* Ewy = S + 6 * sl;      double* Ewxy = S + 7 * sl;
+    double* A0 = S + 8 * sl;       double* A1 = S + 9 * sl;       double* A2 = S + 10 * sl;
+    double* r0 = S + 11 * sl;      double* r1 = S + 12 * sl;      double* r2 = S + 13 * sl;
+    // sort arrays overlay r0/r1 (dead until pass 1); the keys are kept for tie detection
+    unsigned long long* key = reinterpret_cast<unsigned long long*>(r0);
+    unsigned int* idx = reinterpret_cast<unsigned int*>(r1);
+
+    if (tid < 4) cx.flags[tid] = 0;
+    // ---- P1 fold + key init
+    for (int j = tid; j < n; j += T) {
+        key[j] = (unsigned long long)__double_as_longlong(fold_phase(tt[j], f));
+        idx[j] = (unsigned int)j;
+    }
+    __syncthreads();
+    // ---- P2 bitonic network for arbitrary n (all exchanges ascending; indices >= n act as +inf)
+    int np2 = 1;
+    while (np2 < n) np2 <<= 1;
+    const int half = np2 >> 1;
+    for (int k = 2; (k >> 1) < n; k <<= 1) {
+        const int hk = k >> 1;
+        for (int t = tid; t < half; t += T) {
+            int blk = t / hk, o = t - blk * hk;
+            int a = blk * k + o, b = blk * k + k - 1 - o;
+            if (b < n) cex(key, idx, a, b);
+        }
+        __syncthreads();
+        for (int jj = k >> 2; jj >= 1; jj >>= 1) {
+            for (int t = tid; t < half; t += T) {
+                int blk = t / jj, o = t - blk * jj;
+                int a = blk * 2 * jj + o, b = a + jj;
+                if (b < n) cex(key, idx, a, b);
+            }
+            __syncthreads();
+        }
+    }
+    // ---- gather: x centred by 0.5, y already centred by ybar_w
+    for (int j = tid; j < n; j += T) {
+        unsigned int i = idx[j];
+        x[j] = __longlong_as_double((long long)key[j]) - 0.5;
+        ys[j] = yc[i];
+        ws[j] = wo[i];
+        if (perm_dbg) perm_dbg[j] = (int32_t)i;
+        if (j + 1 < n && key[j + 1] <= key[j]) cx.flags[0] = 1;
+    }
+    __syncthreads();
+    const bool has_ties = cx.flags[0] != 0;
+    // keys must survive pass 1 when there are ties: move them to A2's slot is not possible (A2 is
+    // written in pass 1), so in the tie path they are re-derived from x (x + 0.5 is monotone in key).
+
+    double chi2_part = 0.0;
+    const double phi_first = __longlong_as_double((long long)key[0]);
+    const double phi_last = __longlong_as_double((long long)key[n - 1]);
+    if (phi_last <= phi_first) {
+        // Listing 1 lines 25-36: all phases equal -> weighted mean
+        double sw = 0.0, sy = 0.0;
+        for (int j = tid; j < n; j += T) { sw += ws[j]; sy += ws[j] * ys[j]; }
+        sw = block_sum<T>(sw, cx.red);
+        sy = block_sum<T>(sy, cx.red);
+        double a = sw > 0.0 ? sy / sw : 0.0;
+        for (int j = tid; j < n; j += T) {
+            double r = ys[j] - a;
+            chi2_part += ws[j] * r * r;
+            if (smo_dbg) smo_dbg[j] = a + rec.ybar;
+        }
+        double chi2 = block_sum<T>(chi2_part, cx.red);
+        return rec.chi0 > 0.0 ? (rec.chi0 - chi2) / rec.chi0 : 0.0;
+    }
+    const double scale = __longlong_as_double((long long)key[rec.q3]) - __longlong_as_double((long long)key[rec.q1]);
+    const double vsmlsq = 1.e-6 * scale * scale;
+    __syncthreads();                               // key[] (in r0) is dead from here on
+
+    const int ibw0 = rec.ibw[0], ibw1 = rec.ibw[1], ibw2 = rec.ibw[2];
+    const int K0 = min(2 * ibw0 + 1, n), K1 = min(2 * ibw1 + 1, n), K2 = min(2 * ibw2 + 1, n);
+    const bool gv = p.mode == 1;
+
+    // ---- P3: prefix sums of the weighted moments
+    if (!gv) {
+        double* const E[5] = {Ew, Ewx, Ewxx, Ewy, Ewxy};
+        block_scan<T, 5>(n, [&](int j, double* v) {
+            double w_ = ws[j], x_ = x[j], y_ = ys[j];
+            v[0] = w_; v[1] = w_ * x_; v[2] = w_ * x_ * x_; v[3] = w_ * y_; v[4] = w_ * x_ * y_;
+        }, E, cx.wsum);
+    } else {
+        double* const E[6] = {Ew, Ewx, Ewxx, Ewy, Ewxy, A0};
+        block_scan<T, 6>(n, [&](int j, double* v) {
+            double w_ = ws[j], x_ = x[j], y_ = ys[j];
+            v[0] = w_; v[1] = w_ * x_; v[2] = w_ * x_ * x_; v[3] = w_ * y_; v[4] = w_ * x_ * y_;
+            v[5] = w_ * y_ * y_;
+        }, E, cx.wsum);
+    }
+    const double* Ewyy = A0;   // GV only
+
+    auto wsum2 = [&](const double* E, int lo, int K) { return E[lo + K] - E[lo]; };
+
+    if (gv) {
+        // ---- O6: one sweep, three windows, score, pick, interpolate
+        double* smo = A1;
+        for (int j = tid; j < n; j += T) {
+            const double xj = x[j];
+            double A[3], G[3];
+            const int ib[3] = {ibw0, ibw1, ibw2}, KK[3] = {K0, K1, K2};
+#pragma unroll
+            for (int i = 0; i < 3; i++) {
+                int lo = window_lo(j, ib[i], KK[i], n);
+                XMom m = x_moments(wsum2(Ew, lo, KK[i]), wsum2(Ewx, lo, KK[i]), wsum2(Ewxx, lo, KK[i]), vsmlsq);
+                double Swy = wsum2(Ewy, lo, KK[i]), Swxy = wsum2(Ewxy, lo, KK[i]);
+                double b, yb;
+                A[i] = line_fit(m, Swy, Swxy, xj, b, yb);
+                G[i] = gv_score(m, Swy, Swxy, wsum2(Ewyy, lo, KK[i]), b, yb, KK[i]);
+            }
+            double sp = pick_span(G[0], G[1], G[2], p.alpha);
+            smo[j] = interp_spans(sp, A[0], A[1], A[2]);
+        }
+        __syncthreads();
+        if (has_ties) {
+            if (tid == 0) {
+                // re-derive ordered keys from x: ties in x <=> ties in key
+                int j = 0;
+                while (j < n) {
+                    int j0 = j; double sy = smo[j] * ws[j], fbw = ws[j];
+                    while (j < n - 1 && x[j + 1] <= x[j]) { j++; sy += ws[j] * smo[j]; fbw += ws[j]; }
+                    if (j > j0) { double a = fbw > 0.0 ? sy / fbw : 0.0; for (int i = j0; i <= j; i++) smo[i] = a; }
+                    j++;
+                }
+            }
+            __syncthreads();
+        }
+        for (int j = tid; j < n; j += T) {
+            double r = ys[j] - smo[j];
+            chi2_part += ws[j] * r * r;
+            if (smo_dbg) smo_dbg[j] = smo[j] + rec.ybar;
+        }
+        double chi2 = block_sum<T>(chi2_part, cx.red);
+        return rec.chi0 > 0.0 ? (rec.chi0 - chi2) / rec.chi0 : 0.0;
+    }
+
+    // Serial tie averaging keyed on x (ties in x <=> ties in the phase keys: x = phi - 0.5 is
+    // monotone and maps equal phases to equal x).
+    auto tie_avg = [&](double* z) {
+        int j = 0;
+        while (j < n) {
+            int j0 = j; double sy = z[j] * ws[j], fbw = ws[j];
+            while (j < n - 1 && x[j + 1] <= x[j]) { j++; sy += ws[j] * z[j]; fbw += ws[j]; }
+            if (j > j0) { double a = fbw > 0.0 ? sy / fbw : 0.0; for (int i = j0; i <= j; i++) z[i] = a; }
+            j++;
+        }
+    };
+
+    // ---- CV pass 1: three smooths of y with leave-one-out residuals
+    for (int j = tid; j < n; j += T) {
+        const double xj = x[j], yj = ys[j], wj = ws[j];
+        const int ib[3] = {ibw0, ibw1, ibw2}, KK[3] = {K0, K1, K2};
+        double* const Ao[3] = {A0, A1, A2};
+        double* const ro[3] = {r0, r1, r2};
+#pragma unroll
+        for (int i = 0; i < 3; i++) {
+            int lo = window_lo(j, ib[i], KK[i], n);
+            XMom m = x_moments(wsum2(Ew, lo, KK[i]), wsum2(Ewx, lo, KK[i]), wsum2(Ewxx, lo, KK[i]), vsmlsq);
+            double b, yb;
+            double s = line_fit(m, wsum2(Ewy, lo, KK[i]), wsum2(Ewxy, lo, KK[i]), xj, b, yb);
+            double r = loo_residual(m, xj, wj, yj, s);
+            if (r < 0.0) cx.flags[1 + i] = 1;
+            Ao[i][j] = s;
+            ro[i][j] = r;
+        }
+    }
+    __syncthreads();
+    if (has_ties || cx.flags[1] || cx.flags[2] || cx.flags[3]) {
+        if (tid < 3) {
+            double* const Ao[3] = {A0, A1, A2};
+            double* const ro[3] = {r0, r1, r2};
+            if (has_ties) tie_avg(Ao[tid]);
+            if (cx.flags[1 + tid]) carry_fix_serial(n, ro[tid]);
+        }
+        __syncthreads();
+    }
+    // ---- CV pass 2: smooth each residual at the midrange span, in place
+    {
+        double* const ro[3] = {r0, r1, r2};
+        for (int i = 0; i < 3; i++) {
+            double* z = ro[i];
+            double* const E[2] = {Ewy, Ewxy};
+            block_scan<T, 2>(n, [&](int j, double* v) {
+                double wz = ws[j] * z[j];
+                v[0] = wz; v[1] = wz * x[j];
+            }, E, cx.wsum);
+            for (int j = tid; j < n; j += T) {
+                int lo = window_lo(j, ibw1, K1, n);
+                XMom m = x_moments(wsum2(Ew, lo, K1), wsum2(Ewx, lo, K1), wsum2(Ewxx, lo, K1), vsmlsq);
+                double b, zb;
+                z[j] = line_fit(m, wsum2(Ewy, lo, K1), wsum2(Ewxy, lo, K1), x[j], b, zb);
+            }
+            __syncthreads();
+        }
+        if (has_ties) {
+            if (tid < 3) tie_avg(ro[tid]);
+            __syncthreads();
+        }
+    }
+    // ---- span pick + bass enhancement: sp -> r0
+    for (int j = tid; j < n; j += T) r0[j] = pick_span(r0[j], r1[j], r2[j], p.alpha);
+    __syncthreads();
+    // ---- smooth the spans at midrange: sps -> r1
+    {
+        double* const E[2] = {Ewy, Ewxy};
+        block_scan<T, 2>(n, [&](int j, double* v) {
+            double wz = ws[j] * r0[j];
+            v[0] = wz; v[1] = wz * x[j];
+        }, E, cx.wsum);
+        for (int j = tid; j < n; j += T) {
+            int lo = window_lo(j, ibw1, K1, n);
+            XMom m = x_moments(wsum2(Ew, lo, K1), wsum2(Ewx, lo, K1), wsum2(Ewxx, lo, K1), vsmlsq);
+            double b, zb;
+            r1[j] = line_fit(m, wsum2(Ewy, lo, K1), wsum2(Ewxy, lo, K1), x[j], b, zb);
+        }
+        __syncthreads();
+        if (has_ties) {
+            if (tid == 0) tie_avg(r1);
+            __syncthreads();
+        }
+    }
+    // ---- interpolate between the smooths: B -> r2
+    for (int j = tid; j < n; j += T) r2[j] = interp_spans(r1[j], A0[j], A1[j], A2[j]);
+    __syncthreads();
+    // ---- final tweeter smooth: smo -> r0, then chi2
+    {
+        double* const E[2] = {Ewy, Ewxy};
+        block_scan<T, 2>(n, [&](int j, double* v) {
+            double wz = ws[j] * r2[j];
+            v[0] = wz; v[1] = wz * x[j];
+        }, E, cx.wsum);
+        for (int j = tid; j < n; j += T) {
+            int lo = window_lo(j, ibw0, K0, n);
+            XMom m = x_moments(wsum2(Ew, lo, K0), wsum2(Ewx, lo, K0), wsum2(Ewxx, lo, K0), vsmlsq);
+            double b, zb;
+            r0[j] = line_fit(m, wsum2(Ewy, lo, K0), wsum2(Ewxy, lo, K0), x[j], b, zb);
+        }
+        __syncthreads();
+        if (has_ties) {
+            if (tid == 0) tie_avg(r0);
+            __syncthreads();
+        }
+    }
+    for (int j = tid; j < n; j += T) {
+        double r = ys[j] - r0[j];
+        chi2_part += ws[j] * r * r;
+        if (smo_dbg) smo_dbg[j] = r0[j] + rec.ybar;
+    }
+    double chi2 = block_sum<T>(chi2_part, cx.red);
+    return rec.chi0 > 0.0 ? (rec.chi0 - chi2) / rec.chi0 : 0.0;
+}
+
+// Persistent kernel: work item = (list entry, frequency chunk).  STAGE = per-eval arrays in global.
+template <int T, bool STAGE>
+__global__ void __launch_bounds__(T) block_kernel(const EvalParams p)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NW = T / 32;
+    __shared__ double s_wsum[6][NW];
+    __shared__ double s_red[NW];
+    __shared__ int s_flags[4];
+    __shared__ unsigned int s_item;
+
+    BlockCtx<T> cx;
+    cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
+
+    const unsigned int n_items = (unsigned int)p.n_list * (unsigned int)p.chunks_per_obj;
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_item = atomicAdd(p.counter, 1u);
+        __syncthreads();
+        const unsigned int item = s_item;
+        if (item >= n_items) break;
+        const int li = (int)(item / (unsigned int)p.chunks_per_obj);
+        const int ch = (int)(item - (unsigned int)li * (unsigned int)p.chunks_per_obj);
+        const int ri = p.list[li];
+        const ObjRec rec = p.recs[ri];
+        const int64_t sl = block_slot_len(rec.n);
+        double* S = STAGE ? p.stage + (int64_t)blockIdx.x * p.stage_stride
+                          : reinterpret_cast<double*>(smem_raw);
+        const int64_t k0 = p.k_begin + (int64_t)ch * p.chunk;
+        const int64_t k1 = min(k0 + (int64_t)p.chunk, p.k_end);
+        double best = -INFINITY;
+        int64_t best_k = k0;
+        for (int64_t k = k0; k < k1; k++) {
+            const double f = freq_of(p.f_min, p.df, k);
+            double P = block_eval<T>(p, rec, f, S, sl, cx, nullptr, nullptr);
+            if (threadIdx.x == 0) {
+                if (p.pgram)
+                    p.pgram[(rec.obj - p.pgram_row0) * p.pgram_row_stride + (k - p.pgram_k0)] = P;
+                if (P > best) { best = P; best_k = k; }
+            }
+        }
+        if (threadIdx.x == 0) {
+            int64_t slot = (int64_t)ri * p.chunks_total + p.chunk_base + ch;
+            p.part_val[slot] = best;
+            p.part_idx[slot] = best_k;
+        }
+    }
+}
+
+// ss_debug_eval: one eval, one CTA, arrays staged in global memory.
+template <int T>
+__global__ void __launch_bounds__(T) block_debug_kernel(const EvalParams p, double f, double* smo_out,
+                                                        int32_t* perm_out, double* p_out)
+{
+    constexpr int NW = T / 32;
+    __shared__ double s_wsum[6][NW];
+    __shared__ double s_red[NW];
+    __shared__ int s_flags[4];
+    BlockCtx<T> cx;
+    cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
+    const ObjRec rec = p.recs[0];
+    double P = block_eval<T>(p, rec, f, p.stage, block_slot_len(rec.n), cx, smo_out, perm_out);
+    if (threadIdx.x == 0 && p_out) *p_out = P;
+}
+
+}  // namespace ss

@@ -1,0 +1,121 @@
+// ss_planner.h -- host-only logic of the batch planner and path selection (P6 in DESIGN.md).
+// Pure C++ (no CUDA calls) so it can be exercised on a machine without a GPU.
+#pragma once
+#include <cmath>
+#include <cstddef>
+#include <cstdint>
+
+#include "../../include/ss_periodogram.h"
+
+namespace ss {
+
+// Shared-memory budget of the BLOCK path: 14 arrays of (n+2) doubles per eval, 227 KB per CTA.
+constexpr int64_t BLOCK_SMEM_MAX = 232448 - 2048;   // dynamic part; 2 KB left for static arrays
+constexpr int64_t BLOCK_BYTES_PER_POINT = 14 * 8;
+constexpr int64_t BLOCK_MAX_N = BLOCK_SMEM_MAX / BLOCK_BYTES_PER_POINT - 2;   // 2055
+
+inline int path_for_n(int64_t n, int /*mode*/)
+{
+    if (n <= SS_WARP_MAX_N) return SS_PATH_WARP;
+    if (n <= BLOCK_MAX_N) return SS_PATH_BLOCK;
+    return SS_PATH_STAGE;
+}
+
+// Window half-width of Friedman's smoother (O4/R21): max(2, floor(0.5*span*n + 0.5)),
+// evaluated in this order in IEEE double with no contraction (volatile keeps the compiler honest).
+inline int half_width(int64_t n, double span)
+{
+    volatile double a = 0.5 * span;
+    volatile double b = a * (double)n;
+    volatile double c = b + 0.5;
+    int ibw = (int)std::floor(c);
+    return ibw < 2 ? 2 : ibw;
+}
+
+// The paper's footprint model.
+inline double paper_footprint_bytes(int64_t n_t, int64_t n_f) { return 15.0 * 8.0 * (double)n_t * (double)n_f; }
+inline double paper_r_gib(int64_t n_t, int64_t n_f, int mode)
+{
+    double per = mode == SS_MODE_GENERALIZED_VALIDATION ? 96.0 : 160.0;
+    return (8.0 * (double)n_f + 24.0 * (double)n_t + per * (double)n_f * (double)n_t) / (1024.0 * 1024.0 * 1024.0);
+}
+inline int64_t paper_batches(int64_t n_t, int64_t n_f, int mode, double device_gib, double beta)
+{
+    double nb = paper_r_gib(n_t, n_f, mode) / (beta * device_gib);
+    int64_t b = (int64_t)std::ceil(nb);
+    return b < 1 ? 1 : b;
+}
+
+constexpr int STAGE_CTAS = 148 * 2;      // persistent CTAs of the STAGE path (2 per SM)
+constexpr int64_t MIN_CHUNK = 1;          // smallest frequency chunk a work item may cover
+
+// Work items are (object, frequency chunk); aim at >= TARGET_ITEMS items per tile so that
+// persistent CTAs / the hardware scheduler can balance ragged objects.
+constexpr int64_t TARGET_ITEMS = 16384;
+inline int64_t chunks_per_object(int64_t n_objects_in_tile, int64_t freq_per_tile)
+{
+    if (n_objects_in_tile < 1) n_objects_in_tile = 1;
+    int64_t c = (TARGET_ITEMS + n_objects_in_tile - 1) / n_objects_in_tile;
+    if (c > freq_per_tile) c = freq_per_tile;
+    return c < 1 ? 1 : c;
+}
+
+struct PlanInput {
+    int64_t n_points_total, max_n, n_objects, n_freq;
+    int mode;
+    size_t cap_bytes;
+    int host_tiles;    // output tiles are device buffers copied back (x2, double buffered)
+    int want_pgram;
+    int64_t force_freq_tile;
+};
+
+// New footprint model: nothing is materialised at N_t*N_f.  Fixed = catalog copy (tt, yc, w) +
+// records + lists + partial argmax rows; stage = scratch of the STAGE path; tiles = periodogram
+// output buffers when the caller's array lives on the host.
+inline ss_status_t make_plan(const PlanInput& in, ss_plan_t* out)
+{
+    ss_plan_t p{};
+    const int64_t nobj = in.n_objects > 0 ? in.n_objects : 0;
+    // tt, yc, w (+ the raw catalog copy when the caller's arrays live on the host), records, lists,
+    // running best (value, index), offsets, scheduler counters
+    p.fixed_bytes = (size_t)((in.host_tiles ? 6 : 3) * 8 * in.n_points_total)
+                  + (size_t)(nobj * (64 + 4 + 8 + 8 + 8)) + 8192;
+    if (in.max_n > BLOCK_MAX_N)
+        p.stage_bytes = (size_t)STAGE_CTAS * (size_t)(14 * 8 * (((in.max_n + 2) + 1) & ~(int64_t)1));
+    // upper bound of the partial argmax rows (see below), so shrinking tiles cannot overshoot
+    size_t base = p.fixed_bytes + p.stage_bytes + (size_t)16 * (size_t)(TARGET_ITEMS + nobj);
+    int64_t fpt = in.n_freq, opt = nobj > 0 ? nobj : 1;
+    if (in.host_tiles && in.want_pgram) {
+        // shrink the frequency tile first (the paper's N_b batches), then objects
+        auto need = [&](int64_t f, int64_t o) { return base + (size_t)2 * 8 * (size_t)f * (size_t)o; };
+        if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) fpt = in.force_freq_tile;
+        if (need(fpt, opt) > in.cap_bytes) {
+            size_t avail = in.cap_bytes > base ? in.cap_bytes - base : 0;
+            int64_t f = (int64_t)(avail / ((size_t)16 * (size_t)opt));
+            if (f >= 1) fpt = f < fpt ? f : fpt;
+            else {
+                fpt = 1;
+                int64_t o = (int64_t)(avail / 16);
+                if (o < 1) return SS_ERR_OUT_OF_MEMORY;
+                opt = o;
+            }
+        }
+        p.tile_bytes = (size_t)8 * (size_t)fpt * (size_t)opt;
+    } else if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) {
+        fpt = in.force_freq_tile;
+    }
+    p.freq_per_tile = fpt;
+    p.n_freq_tiles = (in.n_freq + fpt - 1) / fpt;
+    p.objects_per_tile = opt;
+    p.n_object_tiles = nobj > 0 ? (nobj + opt - 1) / opt : 0;
+    // partial argmax rows of ONE tile: 16 B per (object, chunk); folded into the running best
+    // per object after every tile, so they never scale with the number of tiles
+    size_t partials = (size_t)16 * (size_t)opt * (size_t)chunks_per_object(opt, fpt);
+    p.fixed_bytes += partials;
+    p.total_bytes = p.fixed_bytes + p.stage_bytes + (in.host_tiles && in.want_pgram ? 2 * p.tile_bytes : 0);
+    if (p.total_bytes > in.cap_bytes) return SS_ERR_OUT_OF_MEMORY;
+    *out = p;
+    return SS_OK;
+}
+
+}  // namespace ss
