@@ -72,6 +72,8 @@ typedef struct {
     int64_t freq_tile;      /* host entry point only: force this many frequencies per output tile
                                (0 = planner decides).  For tests.                                       */
     int skip_validation;    /* 1 = trust the inputs (no device validation pass, no host sync for it)    */
+    int profile;            /* 1 = bracket every eval-kernel launch with CUDA events on the stream;
+                               read the sum with ss_last_kernel_ms() after the call                     */
 } ss_options_t;
 
 /* Fill *opt with the defaults listed above. */
@@ -160,6 +162,11 @@ ss_status_t ss_microbench(double *fp64_flops_out, double *smem_bytes_per_s_out, 
 
 /* Kernel launches issued by this thread's most recent ss_periodogram* call. */
 int64_t ss_last_launch_count(void);
+
+/* With opt->profile = 1: total device time (ms, CUDA events on the launching stream) and number of
+ * the eval-kernel launches (warp/block/stage kernels) of this thread's most recent call. */
+double ss_last_kernel_ms(void);
+int64_t ss_last_kernel_count(void);
 
 const char *ss_last_error(void); /* thread-local, never NULL */
 int ss_version(void);

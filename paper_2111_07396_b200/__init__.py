@@ -23,7 +23,7 @@ LIB_PATH = os.path.join(_HERE, "libss_b200.so")
 
 EXPORTS = ["ss_default_options", "ss_periodogram", "ss_periodogram_ex", "ss_periodogram_host",
            "ss_plan", "ss_workspace_bytes", "ss_paper_footprint_bytes", "ss_paper_batches",
-           "ss_path_for_n", "ss_debug_eval", "ss_microbench", "ss_last_launch_count",
+           "ss_path_for_n", "ss_debug_eval", "ss_microbench", "ss_last_launch_count", "ss_last_kernel_ms", "ss_last_kernel_count",
            "ss_last_error", "ss_version"]
 
 
@@ -36,7 +36,7 @@ class SSError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [("alpha", C.c_double), ("span", C.c_double), ("iper", C.c_int),
                 ("force_path", C.c_int), ("stream", C.c_void_p), ("workspace_cap", C.c_size_t),
-                ("freq_tile", C.c_int64), ("skip_validation", C.c_int)]
+                ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int)]
 
 
 class Plan(C.Structure):
@@ -78,6 +78,8 @@ def load():
     L.ss_debug_eval.argtypes = [vp, vp, vp, i64, d, C.c_int, C.POINTER(Options), vp, vp, vp]
     L.ss_microbench.argtypes = [C.POINTER(d), C.POINTER(d), vp]
     L.ss_last_launch_count.restype = i64
+    L.ss_last_kernel_ms.restype = d
+    L.ss_last_kernel_count.restype = i64
     L.ss_last_error.restype = C.c_char_p
     L.ss_version.restype = C.c_int
     _lib = L
@@ -105,6 +107,12 @@ def version() -> int:
 
 def last_launch_count() -> int:
     return int(load().ss_last_launch_count())
+
+
+def last_kernel_ms():
+    """(total ms, launches) of the eval kernels of the last call made with options.profile = 1."""
+    L = load()
+    return float(L.ss_last_kernel_ms()), int(L.ss_last_kernel_count())
 
 
 def path_for_n(n: int, mode: int = CROSS_VALIDATION) -> int:

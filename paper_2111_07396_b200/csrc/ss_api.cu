@@ -18,6 +18,8 @@ namespace ss {
 
 static thread_local std::string g_err = "";
 static thread_local int64_t g_launches = 0;
+static thread_local double g_kernel_ms = 0.0;
+static thread_local int64_t g_kernel_count = 0;
 
 static ss_status_t fail(ss_status_t st, const char* fmt, ...)
 {
@@ -241,6 +243,11 @@ struct Engine {
     unsigned int* counters = nullptr;
     int* flag = nullptr;
     double* stage = nullptr;
+    unsigned long long* defer_entries = nullptr;   // warp path -> generic kernel hand-over
+    double* defer_val = nullptr;
+    unsigned int* defer_count = nullptr;
+    unsigned long long *dmax = nullptr, *dmin = nullptr;
+    unsigned int defer_capacity = DEFER_CAPACITY;
     char* extra = nullptr;            // caller-requested extra bytes (host entry point buffers)
     int64_t stage_stride = 0;
     int n_counters = 0, next_counter = 0;
@@ -248,8 +255,27 @@ struct Engine {
     // per object tile: class lists
     std::vector<std::vector<ClassList>> tiles;
     int sm_count = 148;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof;   // opt.profile: events around eval kernels
 
-    ~Engine() { if (ws) cudaFree(ws); }
+    ~Engine()
+    {
+        for (auto& e : prof) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
+        if (ws) cudaFree(ws);
+    }
+    // After the stream is synchronised: did the deferred list overflow?
+    bool defer_overflowed()
+    {
+        unsigned int h[2] = {0, 0};
+        if (!defer_count) return false;
+        if (cudaMemcpy(h, defer_count, 8, cudaMemcpyDeviceToHost) != cudaSuccess) return false;
+        return h[1] != 0;
+    }
+    // Sum the profiled kernel times (call after the stream has been synchronised).
+    void collect_profile()
+    {
+        g_kernel_ms = 0.0; g_kernel_count = (int64_t)prof.size();
+        for (auto& e : prof) { float ms = 0; if (cudaEventElapsedTime(&ms, e.first, e.second) == cudaSuccess) g_kernel_ms += ms; }
+    }
 
     ss_status_t setup(const double* times, const double* mags, const double* errs,
                       const int64_t* offsets_host, int64_t n_obj, double fmin, double fmax,
@@ -371,6 +397,8 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     size_t o_pv = carve(8 * std::max<size_t>(recs.size(), 1) * (size_t)cpo), o_pi = carve(8 * std::max<size_t>(recs.size(), 1) * (size_t)cpo);
     size_t o_cnt = carve(4 * (size_t)n_counters), o_flag = carve(64);
     size_t o_stage = carve(need_stage ? 8 * (size_t)stage_stride * (size_t)stage_ctas : 0);
+    size_t o_de = carve(8 * (size_t)defer_capacity), o_dv = carve(8 * (size_t)defer_capacity), o_dc = carve(64);
+    size_t o_dmax = carve(8 * (size_t)std::max<int64_t>(n_obj, 1)), o_dmin = carve(8 * (size_t)std::max<int64_t>(n_obj, 1));
     size_t o_extra = carve(extra_bytes);
     ws_bytes = b;
     if (ws_bytes > cap + (64 << 20))
@@ -382,6 +410,9 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     part_val = (double*)(ws + o_pv); part_idx = (int64_t*)(ws + o_pi);
     counters = (unsigned int*)(ws + o_cnt); flag = (int*)(ws + o_flag);
     stage = need_stage ? (double*)(ws + o_stage) : nullptr;
+    defer_entries = (unsigned long long*)(ws + o_de); defer_val = (double*)(ws + o_dv);
+    defer_count = (unsigned int*)(ws + o_dc);
+    dmax = (unsigned long long*)(ws + o_dmax); dmin = (unsigned long long*)(ws + o_dmin);
     extra = ws + o_extra;
 
     if (!recs.empty()) SS_CUDA(cudaMemcpyAsync(d_recs, recs.data(), sizeof(ObjRec) * recs.size(), cudaMemcpyHostToDevice, stream));
@@ -389,6 +420,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     if (!degenerate.empty()) SS_CUDA(cudaMemcpyAsync(d_degen, degenerate.data(), 8 * degenerate.size(), cudaMemcpyHostToDevice, stream));
     SS_CUDA(cudaMemsetAsync(counters, 0, 4 * (size_t)n_counters, stream));
     SS_CUDA(cudaMemsetAsync(flag, 0, 64, stream));
+    SS_CUDA(cudaMemsetAsync(defer_count, 0, 64, stream));
     if (n_obj > 0) {
         init_best_kernel<<<(unsigned)((n_obj + 255) / 256), 256, 0, stream>>>(n_obj, best_val, best_idx);
         g_launches++;
@@ -440,14 +472,24 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         p.part_val = part_val; p.part_idx = part_idx;
         p.counter = counters + (next_counter % n_counters);
         p.stage = stage; p.stage_stride = stage_stride;
+        p.defer_entries = defer_entries; p.defer_count = defer_count; p.defer_capacity = defer_capacity;
         const int64_t n_items = (int64_t)p.n_list * cpo;
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
+        cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+        if (opt.profile) {
+            SS_CUDA(cudaEventCreate(&ev0));
+            SS_CUDA(cudaEventCreate(&ev1));
+            prof.emplace_back(ev0, ev1);
+        }
+        if (c.path != SS_PATH_WARP) {
+            SS_CUDA(cudaMemsetAsync(p.counter, 0, 4, stream));
+            next_counter++;
+        }
+        if (ev0) SS_CUDA(cudaEventRecord(ev0, stream));
         if (c.path == SS_PATH_WARP) {
             ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else {
-            SS_CUDA(cudaMemsetAsync(p.counter, 0, 4, stream));
-            next_counter++;
             if (c.path == SS_PATH_BLOCK) {
                 const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(c.max_n) * 8;
                 if (c.variant == 2) {
@@ -465,12 +507,27 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
                 block_kernel<512, true><<<grid, 512, 0, stream>>>(p);
             }
         }
+        if (ev1) SS_CUDA(cudaEventRecord(ev1, stream));
         g_launches++;
         SS_CUDA(cudaGetLastError());
         fold_best_kernel<<<(unsigned)((p.n_list * 32 + 255) / 256), 256, 0, stream>>>(
             d_recs, p.list, p.n_list, (int)cpo, p.chunks_total, 0, part_val, part_idx, best_val, best_idx);
         g_launches++;
         SS_CUDA(cudaGetLastError());
+        if (c.path == SS_PATH_WARP) {
+            // evals the warp path deferred (tied / misordered phases, LOO denominator <= 0):
+            // recompute with the generic code, patch the periodogram, fold into the running best
+            SS_CUDA(cudaMemsetAsync(dmax, 0, 8 * (size_t)n_objects, stream));
+            SS_CUDA(cudaMemsetAsync(dmin, 0xff, 8 * (size_t)n_objects, stream));
+            const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(SS_WARP_MAX_N) * 8;
+            SS_CUDA(cudaFuncSetAttribute(deferred_eval_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            deferred_eval_kernel<<<sm_count * 4, DEFER_T, smem, stream>>>(p, defer_val, dmax);
+            deferred_min_kernel<<<sm_count, 256, 0, stream>>>(p, defer_val, dmax, dmin);
+            deferred_merge_kernel<<<sm_count, 256, 0, stream>>>(p, defer_val, dmax, dmin, best_val, best_idx);
+            g_launches += 3;
+            SS_CUDA(cudaGetLastError());
+            SS_CUDA(cudaMemsetAsync(defer_count, 0, 4, stream));   // the overflow flag [1] stays
+        }
     }
     // NaN rows of degenerate objects in this tile
     if (pgram && !degenerate.empty()) {
@@ -523,6 +580,8 @@ void ss_default_options(ss_options_t* opt)
 const char* ss_last_error(void) { return g_err.c_str(); }
 int ss_version(void) { return SS_VERSION; }
 int64_t ss_last_launch_count(void) { return g_launches; }
+double ss_last_kernel_ms(void) { return g_kernel_ms; }
+int64_t ss_last_kernel_count(void) { return g_kernel_count; }
 int ss_path_for_n(int64_t n, ss_mode_t mode) { return path_for_n(n, (int)mode); }
 double ss_paper_footprint_bytes(int64_t n_t, int64_t n_f) { return paper_footprint_bytes(n_t, n_f); }
 int64_t ss_paper_batches(int64_t n_t, int64_t n_f, ss_mode_t mode, double device_gib, double beta)
@@ -584,6 +643,16 @@ ss_status_t ss_periodogram_ex(const double* times, const double* mags, const dou
     st = eng.finish(best_freq_out, best_index_out);
     if (st != SS_OK) return st;
     SS_CUDA(cudaStreamSynchronize(stream));
+    eng.collect_profile();
+    if (eng.defer_overflowed()) {
+        // more exact ties than the hand-over list holds (e.g. duplicated time stamps in every
+        // object): serve everything with the generic kernel instead
+        if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "deferred list overflow on the block path");
+        ss_options_t o2 = o;
+        o2.force_path = SS_PATH_BLOCK;
+        return ss_periodogram_ex(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                                 best_freq_out, best_index_out, &o2);
+    }
     return SS_OK;
 }
 
@@ -678,6 +747,14 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
     if (best_index_out) SS_CUDA(cudaMemcpyAsync(best_index_out, d_bi, 8 * (size_t)n_objects, cudaMemcpyDeviceToHost, stream));
     SS_CUDA(cudaStreamSynchronize(stream));
     if (copy_stream) SS_CUDA(cudaStreamSynchronize(copy_stream));
+    eng.collect_profile();
+    if (eng.defer_overflowed()) {
+        if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "deferred list overflow on the block path");
+        ss_options_t o2 = o;
+        o2.force_path = SS_PATH_BLOCK;
+        return ss_periodogram_host(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                                   best_freq_out, best_index_out, &o2);
+    }
     return SS_OK;
 }
 

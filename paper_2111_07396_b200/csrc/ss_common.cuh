@@ -50,6 +50,10 @@ struct EvalParams {
     unsigned int* counter;    // dynamic work counter (persistent kernels)
     double* stage;            // global staging scratch (STAGE path), stage_stride doubles per CTA
     int64_t stage_stride;
+    // evals the warp path defers to the generic kernel: (record index << 32 | k - k_begin)
+    unsigned long long* defer_entries;
+    unsigned int* defer_count;   // [0] = appended (may exceed capacity), [1] = sticky overflow flag
+    unsigned int defer_capacity;
 };
 
 // f_k = f_min + k*df as one multiply and one add, unfused (R2).

@@ -46,6 +46,7 @@ inline int64_t paper_batches(int64_t n_t, int64_t n_f, int mode, double device_g
     return b < 1 ? 1 : b;
 }
 
+constexpr unsigned int DEFER_CAPACITY = 1u << 20;   // evals the warp path may defer per tile
 constexpr int STAGE_CTAS = 148 * 2;      // persistent CTAs of the STAGE path (2 per SM)
 constexpr int64_t MIN_CHUNK = 1;          // smallest frequency chunk a work item may cover
 
@@ -79,7 +80,8 @@ inline ss_status_t make_plan(const PlanInput& in, ss_plan_t* out)
     // tt, yc, w (+ the raw catalog copy when the caller's arrays live on the host), records, lists,
     // running best (value, index), offsets, scheduler counters
     p.fixed_bytes = (size_t)((in.host_tiles ? 6 : 3) * 8 * in.n_points_total)
-                  + (size_t)(nobj * (64 + 4 + 8 + 8 + 8)) + 8192;
+                  + (size_t)(nobj * (64 + 4 + 8 + 8 + 8 + 16)) + 8192
+                  + (size_t)DEFER_CAPACITY * 16;   // warp-path hand-over list (entries + values)
     if (in.max_n > BLOCK_MAX_N)
         p.stage_bytes = (size_t)STAGE_CTAS * (size_t)(14 * 8 * (((in.max_n + 2) + 1) & ~(int64_t)1));
     // upper bound of the partial argmax rows (see below), so shrinking tiles cannot overshoot

@@ -1,0 +1,301 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Bar (BASELINE.json north_star):
+    |P_gpu - P_ref| <= 1e-9*|P_ref| + 1e-12   per periodogram value,
+    identical best-frequency index except ties within 1e-12.
+An eval that misses the bar is re-examined with the definition oracle (long double window sums);
+if its closest span pick is a near-tie (relative margin < 1e-9) it is "branch-ambiguous" (R29) and
+must match the oracle's re-evaluation with that pick forced the other way.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import ss_inputs
+
+pytestmark = pytest.mark.gpu
+
+CV, GV = 0, 1
+RTOL, ATOL = 1e-9, 1e-12
+
+
+@pytest.fixture(scope="module")
+def ss():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2111_07396_b200 as m
+    m.load()
+    return m
+
+
+def _tol(ref):
+    return RTOL * np.abs(ref) + ATOL
+
+
+def check_parity(cat, pg, ref, mode, max_ambiguous=3, label=""):
+    """pg, ref: [n_objects, n_freq].  Returns number of branch-ambiguous evals."""
+    assert pg.shape == ref.shape
+    both_nan = np.isnan(pg) & np.isnan(ref)
+    d = np.abs(pg - ref)
+    bad = (d > _tol(ref)) & ~both_nan
+    bad |= np.isnan(pg) ^ np.isnan(ref)
+    ambiguous = 0
+    for o, k in zip(*np.nonzero(bad)):
+        t, y, e = cat.obj(int(o))
+        f = oracle.freq(cat.f_min, cat.f_max, cat.n_freq, int(k))
+        r = oracle.eval_one(t, y, e, f, mode=mode, variant=oracle.DEFINITION, alt_threshold=1e-7)
+        if abs(pg[o, k] - r["P"]) <= _tol(r["P"]):
+            continue            # the fast oracle was the inexact side; the definition oracle agrees
+        if r["margin"] < 1e-9 and abs(pg[o, k] - r["P_alt"]) <= _tol(r["P_alt"]):
+            ambiguous += 1
+            continue
+        raise AssertionError(f"{label} obj {o} k {k}: gpu {pg[o, k]!r} oracle {r['P']!r} "
+                             f"(fast {ref[o, k]!r}) margin {r['margin']:.3e}")
+    assert ambiguous <= max_ambiguous, f"{label}: {ambiguous} branch-ambiguous evals"
+    return ambiguous
+
+
+def check_best(pg_ref, bi_gpu, bf_gpu, cat):
+    """Best index identical to the oracle's, except ties within 1e-12 (R15)."""
+    for o in range(pg_ref.shape[0]):
+        row = pg_ref[o]
+        if np.all(np.isnan(row)):
+            assert bi_gpu[o] == -1 and np.isnan(bf_gpu[o])
+            continue
+        kb = int(np.argmax(row))
+        kg = int(bi_gpu[o])
+        if kg != kb:
+            assert abs(row[kg] - row[kb]) <= 1e-12 * max(1.0, abs(row[kb])), (o, kg, kb, row[kg], row[kb])
+        assert bf_gpu[o] == oracle.freq(cat.f_min, cat.f_max, cat.n_freq, kg)
+
+
+def run_both(ss, cat, mode, variant, **opts):
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                         mode, **opts)
+    assert ss.last_launch_count() > 0
+    ref, bf, bi = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
+                                     cat.n_freq, mode=mode, variant=variant)
+    return res, ref
+
+
+# ------------------------------------------------------------------ the five configs (reduced)
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config1_full(ss, mode):
+    cat = ss_inputs.make(1)
+    res, ref = run_both(ss, cat, mode, oracle.DEFINITION)
+    check_parity(cat, res.pgram, ref, mode, label="cfg1")
+    check_best(ref, res.best_index, res.best_freq, cat)
+    assert abs(res.best_freq[0] - 1 / 0.37) < 0.01 * (1 / 0.37)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config2_reduced(ss, mode):
+    cat = ss_inputs.make(2).with_grid(n_freq=3001)
+    res, ref = run_both(ss, cat, mode, oracle.FAST)
+    check_parity(cat, res.pgram, ref, mode, label="cfg2")
+    check_best(ref, res.best_index, res.best_freq, cat)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config3_reduced(ss, mode):
+    """96 ragged objects (n = 50..200 incl. both extremes), 1,537 frequencies over the config's range."""
+    full = ss_inputs.config3(n_objects=400, n_freq=1537)
+    ns = np.diff(full.offsets)
+    pick = sorted(set(list(range(90)) + [int(np.argmin(ns)), int(np.argmax(ns))]
+                      + [int(i) for i in np.nonzero(ns % 32 == 0)[0][:4]]))
+    cat = full.subset(pick)
+    res, ref = run_both(ss, cat, mode, oracle.DEFINITION)
+    check_parity(cat, res.pgram, ref, mode, label="cfg3")
+    check_best(ref, res.best_index, res.best_freq, cat)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config4_reduced_and_planner_tiling(ss, mode):
+    """8 objects of config 4 (n = 500..2000, heteroscedastic, one pure-noise object), 301 frequencies;
+    the host entry point is forced to tile frequencies (cap and freq_tile) and must return the same
+    bits as the untiled run."""
+    full = ss_inputs.config4(n_objects=30, n_freq=301)
+    ns = np.diff(full.offsets)
+    pick = sorted(set([0, 1, 2, 9, 19, int(np.argmin(ns)), int(np.argmax(ns)), 29]))
+    cat = full.subset(pick)
+    res, ref = run_both(ss, cat, mode, oracle.FAST)
+    check_parity(cat, res.pgram, ref, mode, label="cfg4")
+    check_best(ref, res.best_index, res.best_freq, cat)
+    tiled = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                           mode, freq_tile=37)
+    assert np.array_equal(tiled.pgram, res.pgram)
+    assert np.array_equal(tiled.best_index, res.best_index)
+    # shrink the cap until the planner must tile frequencies by itself
+    n_max = int(ns[pick].max())
+    cap = ss.plan(cat.n_points, n_max, cat.n_objects, cat.n_freq, mode, cap_bytes=1 << 40,
+                  host_tiles=True).total_bytes
+    while True:
+        cap -= 8 * cat.n_objects * 16
+        p = ss.plan(cat.n_points, n_max, cat.n_objects, cat.n_freq, mode, cap_bytes=cap, host_tiles=True)
+        if p.n_freq_tiles >= 3:
+            break
+    assert p.total_bytes <= cap
+    capped = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                            mode, workspace_cap=cap)
+    assert np.array_equal(capped.pgram, res.pgram)
+    assert np.array_equal(capped.best_index, res.best_index)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config5_reduced_global_staging(ss, mode):
+    """n = 20,000 (exceeds one SM's shared memory -> SS_PATH_STAGE), 40 frequencies."""
+    cat = ss_inputs.make(5).with_grid(n_freq=40)
+    assert ss.path_for_n(20000) == ss.PATH_STAGE
+    res, ref = run_both(ss, cat, mode, oracle.FAST)
+    check_parity(cat, res.pgram, ref, mode, label="cfg5")
+    check_best(ref, res.best_index, res.best_freq, cat)
+    # two evals against the definition oracle (long double direct window sums)
+    t, y, e = cat.obj(0)
+    for k in (3, 31):
+        f = oracle.freq(cat.f_min, cat.f_max, cat.n_freq, k)
+        r = oracle.eval_one(t, y, e, f, mode=mode, variant=oracle.DEFINITION)
+        assert abs(res.pgram[0, k] - r["P"]) <= _tol(r["P"])
+
+
+# ------------------------------------------------------------------ one eval, element by element
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("n", [5, 6, 7, 33, 100, 257, 1000])
+def test_smooth_values_and_permutation(ss, mode, n):
+    rng = np.random.default_rng(100 + n)
+    t = np.sort(rng.uniform(0, 30, size=n))
+    y = 15 + 0.4 * np.sin(2 * np.pi * t / 0.61) + rng.normal(0, 0.05, size=n)
+    e = rng.uniform(0.01, 0.2, size=n)
+    for f in (0.5, 1.639, 7.77):
+        P, smo, perm = ss.debug_eval(t, y, e, f, mode)
+        r = oracle.eval_one(t, y, e, f, mode=mode, variant=oracle.DEFINITION, want_smo=True)
+        assert np.array_equal(perm, r["perm"])              # bit-exact fold + stable order (R2, R13)
+        if r["margin"] < 1e-9:
+            continue
+        assert np.abs(smo - r["smo"]).max() < 1e-10
+        assert abs(P - r["P"]) <= _tol(r["P"])
+
+
+# ------------------------------------------------------------------ paths agree
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_forced_paths_agree(ss, mode):
+    cat = ss_inputs.config3(n_objects=12, n_freq=257)
+    ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
+                                   cat.n_freq, mode=mode, variant=oracle.DEFINITION)
+    for path in (ss.PATH_WARP, ss.PATH_BLOCK, ss.PATH_STAGE):
+        res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                             mode, force_path=path)
+        check_parity(cat, res.pgram, ref, mode, label=f"path{path}")
+        check_best(ref, res.best_index, res.best_freq, cat)
+
+
+# ------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_degenerate_objects_and_ragged_catalog(ss, mode):
+    """Empty object, n < 5 (NaN row, index -1), n = 5, constant magnitudes (zeros), unsorted times."""
+    rng = np.random.default_rng(7)
+    ns = [0, 3, 5, 40, 4, 64, 0, 9]
+    T, Y, E = [], [], []
+    for i, n in enumerate(ns):
+        t = rng.uniform(0, 20, size=n)                      # NOT sorted in time
+        y = 15 + 0.3 * np.sin(2 * np.pi * t / 0.8) + rng.normal(0, 0.03, size=n)
+        if i == 5:
+            y = np.full(n, 15.25)                           # constant => chi0 = 0 => zeros
+        T.append(t); Y.append(y); E.append(np.full(n, 0.03))
+    off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
+    cat = ss_inputs.Catalog("edge", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
+                            0.2, 6.0, 97, np.full(len(ns), np.nan))
+    res, ref = run_both(ss, cat, mode, oracle.DEFINITION)
+    for i, n in enumerate(ns):
+        if n < 5:
+            assert np.all(np.isnan(res.pgram[i])) and res.best_index[i] == -1 and np.isnan(res.best_freq[i])
+    assert np.all(res.pgram[5] == 0.0) and res.best_index[5] == 0
+    check_parity(cat, res.pgram, ref, mode, label="edge")
+    check_best(ref, res.best_index, res.best_freq, cat)
+    # nothing to do
+    empty = ss.periodogram(np.zeros(0), np.zeros(0), np.zeros(0), np.zeros(1, dtype=np.int64), 0.2, 6.0, 10, mode)
+    assert empty.pgram.shape == (0, 10)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_equal_phases_and_tied_runs(ss, mode):
+    """Integer-day time stamps: at f = 1 every phase is 0 (Listing 1 lines 25-36, weighted mean);
+    at f = 0.5 and 0.25 the phases fall into 2 / 4 exactly tied runs (equal-x averaging, R24);
+    duplicated observation times give tied pairs at every frequency."""
+    rng = np.random.default_rng(8)
+    n = 48
+    t1 = np.arange(n, dtype=np.float64) + 1000.0
+    y1 = 15 + rng.normal(0, 0.1, size=n)
+    t2 = np.sort(rng.uniform(0, 25, size=60)); t2[10] = t2[9]; t2[31] = t2[30]; t2[32] = t2[30]
+    y2 = 15 + 0.5 * np.sin(2 * np.pi * t2 / 1.3) + rng.normal(0, 0.05, size=60)
+    off = np.array([0, n, n + 60], dtype=np.int64)
+    cat = ss_inputs.Catalog("ties", np.concatenate([t1, t2]), np.concatenate([y1, y2]),
+                            np.concatenate([rng.uniform(0.05, 0.2, size=n), np.full(60, 0.05)]), off,
+                            0.25, 1.25, 4, np.array([np.nan, 1 / 1.3]))      # f = 0.25, 0.5, 0.75, 1.0
+    assert oracle.freq(cat.f_min, cat.f_max, cat.n_freq, 3) == 1.0
+    for path in (ss.PATH_AUTO, ss.PATH_BLOCK, ss.PATH_STAGE):
+        res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                             mode, force_path=path)
+        ref, bf, bi = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
+                                         cat.n_freq, mode=mode, variant=oracle.DEFINITION)
+        assert abs(res.pgram[0, 3]) < 1e-12                      # all phases equal: chi2 == chi0
+        check_parity(cat, res.pgram, ref, mode, label=f"ties/path{path}")
+
+
+def test_invalid_arguments(ss):
+    t = np.linspace(0, 10, 20); y = np.sin(t); e = np.full(20, 0.1)
+    off = np.array([0, 20], dtype=np.int64)
+    def call(**kw):
+        a = dict(times=t, mags=y, errs=e, offsets=off, f_min=0.1, f_max=2.0, n_freq=16)
+        a.update(kw)
+        return ss.periodogram(a["times"], a["mags"], a["errs"], a["offsets"], a["f_min"], a["f_max"], a["n_freq"])
+    call()
+    for kw in (dict(f_min=0.0), dict(f_min=-1.0), dict(f_max=0.05), dict(n_freq=0),
+               dict(errs=np.where(np.arange(20) == 3, 0.0, e)), dict(errs=-e),
+               dict(mags=np.where(np.arange(20) == 5, np.nan, y)),
+               dict(times=np.where(np.arange(20) == 5, np.inf, t)),
+               dict(offsets=np.array([0, 25, 20], dtype=np.int64))):
+        with pytest.raises(ss.SSError) as ei:
+            call(**kw)
+        assert ei.value.status == ss.SS_ERR_INVALID_ARG, kw
+    with pytest.raises(ss.SSError) as ei:
+        ss.periodogram(t, y, e, off, 0.1, 2.0, 16, span=0.3)
+    assert ei.value.status == ss.SS_ERR_UNSUPPORTED
+
+
+def test_alpha_option(ss):
+    """alpha in (0,10] switches the bass enhancement; alpha = 0 disables it."""
+    cat = ss_inputs.config3(n_objects=3, n_freq=64)
+    for alpha in (0.0, 5.0, 10.0):
+        res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                             CV, alpha=alpha)
+        ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
+                                       cat.n_freq, mode=CV, variant=oracle.DEFINITION, alpha=alpha)
+        check_parity(cat, res.pgram, ref, CV, label=f"alpha{alpha}")
+
+
+# ------------------------------------------------------------------ device-tensor entry point
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_device_entry_point_matches_host_entry_point(ss, mode):
+    import torch
+    cat = ss_inputs.config3(n_objects=20, n_freq=333)
+    dev = torch.device("cuda")
+    t = torch.as_tensor(cat.times, device=dev); y = torch.as_tensor(cat.mags, device=dev)
+    e = torch.as_tensor(cat.errs, device=dev); off = torch.as_tensor(cat.offsets, device=dev)
+    pg = torch.full((cat.n_objects, cat.n_freq), -7.0, dtype=torch.float64, device=dev)
+    bf = torch.empty(cat.n_objects, dtype=torch.float64, device=dev)
+    bi = torch.empty(cat.n_objects, dtype=torch.int64, device=dev)
+    ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, bf, bi)
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode)
+    assert np.array_equal(pg.cpu().numpy(), res.pgram)
+    assert np.array_equal(bi.cpu().numpy(), res.best_index)
+    assert np.array_equal(bf.cpu().numpy(), res.best_freq)
+    # pgram_out = NULL: only the best frequency is produced
+    bi2 = torch.empty_like(bi)
+    ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, None, None, bi2)
+    assert torch.equal(bi, bi2)
+    # on a side stream
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        pg3 = torch.empty_like(pg)
+        ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg3, None, None)
+    s.synchronize()
+    assert torch.equal(pg, pg3)
