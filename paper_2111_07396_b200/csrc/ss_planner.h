@@ -84,36 +84,43 @@ inline ss_status_t make_plan(const PlanInput& in, ss_plan_t* out)
                   + (size_t)DEFER_CAPACITY * 16;   // warp-path hand-over list (entries + values)
     if (in.max_n > BLOCK_MAX_N)
         p.stage_bytes = (size_t)STAGE_CTAS * (size_t)(14 * 8 * (((in.max_n + 2) + 1) & ~(int64_t)1));
-    // upper bound of the partial argmax rows (see below), so shrinking tiles cannot overshoot
-    size_t base = p.fixed_bytes + p.stage_bytes + (size_t)16 * (size_t)(TARGET_ITEMS + nobj);
+    // partial argmax rows of ONE tile: 16 B per (object, chunk); folded into the running best per
+    // object after every tile, so they never scale with the number of tiles
+    auto partials = [&](int64_t f, int64_t o) { return (size_t)16 * (size_t)o * (size_t)chunks_per_object(o, f); };
+    const size_t base = p.fixed_bytes + p.stage_bytes;
     int64_t fpt = in.n_freq, opt = nobj > 0 ? nobj : 1;
+    if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) fpt = in.force_freq_tile;
     if (in.host_tiles && in.want_pgram) {
-        // shrink the frequency tile first (the paper's N_b batches), then objects
-        auto need = [&](int64_t f, int64_t o) { return base + (size_t)2 * 8 * (size_t)f * (size_t)o; };
-        if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) fpt = in.force_freq_tile;
+        // exact need of an (f x o) tile: double-buffered output tile + partial rows
+        auto need = [&](int64_t f, int64_t o) { return base + partials(f, o) + (size_t)2 * 8 * (size_t)f * (size_t)o; };
+        // shrink the frequency tile first (the paper's N_b batches), then objects;
+        // need() is non-decreasing in f and in o, so bisect
         if (need(fpt, opt) > in.cap_bytes) {
-            size_t avail = in.cap_bytes > base ? in.cap_bytes - base : 0;
-            int64_t f = (int64_t)(avail / ((size_t)16 * (size_t)opt));
-            if (f >= 1) fpt = f < fpt ? f : fpt;
-            else {
+            if (need(1, opt) <= in.cap_bytes) {
+                int64_t lo = 1, hi = fpt;          // need(lo) fits, need(hi) does not
+                while (hi - lo > 1) {
+                    int64_t mid = lo + (hi - lo) / 2;
+                    if (need(mid, opt) <= in.cap_bytes) lo = mid; else hi = mid;
+                }
+                fpt = lo;
+            } else {
                 fpt = 1;
-                int64_t o = (int64_t)(avail / 16);
-                if (o < 1) return SS_ERR_OUT_OF_MEMORY;
-                opt = o;
+                if (need(1, 1) > in.cap_bytes) return SS_ERR_OUT_OF_MEMORY;
+                int64_t lo = 1, hi = opt;
+                while (hi - lo > 1) {
+                    int64_t mid = lo + (hi - lo) / 2;
+                    if (need(1, mid) <= in.cap_bytes) lo = mid; else hi = mid;
+                }
+                opt = lo;
             }
         }
         p.tile_bytes = (size_t)8 * (size_t)fpt * (size_t)opt;
-    } else if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) {
-        fpt = in.force_freq_tile;
     }
     p.freq_per_tile = fpt;
     p.n_freq_tiles = (in.n_freq + fpt - 1) / fpt;
     p.objects_per_tile = opt;
     p.n_object_tiles = nobj > 0 ? (nobj + opt - 1) / opt : 0;
-    // partial argmax rows of ONE tile: 16 B per (object, chunk); folded into the running best
-    // per object after every tile, so they never scale with the number of tiles
-    size_t partials = (size_t)16 * (size_t)opt * (size_t)chunks_per_object(opt, fpt);
-    p.fixed_bytes += partials;
+    p.fixed_bytes += partials(fpt, opt);
     p.total_bytes = p.fixed_bytes + p.stage_bytes + (in.host_tiles && in.want_pgram ? 2 * p.tile_bytes : 0);
     if (p.total_bytes > in.cap_bytes) return SS_ERR_OUT_OF_MEMORY;
     *out = p;
