@@ -134,10 +134,10 @@ __device__ __forceinline__ WinFit tweeter_fit(const double (&ux)[C + 2 * IBW0], 
         if (GV) mzz += wz * z_;
     }
     WinFit f;
-    f.inv_sw = m0 > 0.0 ? 1.0 / m0 : 0.0;
+    f.inv_sw = m0 > 0.0 ? rcp64(m0) : 0.0;
     const double xr = m1 * f.inv_sw;             // xbar relative to c
     const double sxx = m2 - xr * m1;
-    f.inv_sxx = sxx > vsmlsq ? 1.0 / sxx : 0.0;
+    f.inv_sxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
     f.xbar = c + xr;
     f.zbar = mz * f.inv_sw;
     const double sxz = m1z - xr * mz;
@@ -147,7 +147,7 @@ __device__ __forceinline__ WinFit tweeter_fit(const double (&ux)[C + 2 * IBW0], 
         double rss = (mzz - f.zbar * mz) - f.b * sxz;
         rss = rss > 0.0 ? rss : 0.0;
         const double p = f.inv_sxx != 0.0 ? 2.0 : 1.0;
-        f.g = m0 > 0.0 ? sqrt(rss * f.inv_sw) / (1.0 - p / (double)(2 * IBW0 + 1)) : 0.0;
+        f.g = m0 > 0.0 ? sqrt(rss * f.inv_sw) * rcp64(1.0 - p / (double)(2 * IBW0 + 1)) : 0.0;
     }
     return f;
 }
@@ -321,7 +321,7 @@ __device__ __forceinline__ double warp_eval_body(const ObjRec& rec, const WarpMe
             {
                 const double dx = xj - tw[s].xbar;
                 const double a = 1.0 - wj * (tw[s].inv_sw + dx * dx * tw[s].inv_sxx);
-                r0[s] = a > 0.0 ? fabs(yj - A0[s]) / a : -1.0;
+                r0[s] = a > 0.0 ? fabs(yj - A0[s]) * rcp64(a) : -1.0;
             }
             XMom m1 = x_moments(wdiff<C>(Ew, s1lo[s], s1hi[s]), wdiff<C>(Ewx, s1lo[s], s1hi[s]),
                                 wdiff<C>(Ewxx, s1lo[s], s1hi[s]), vsmlsq);
@@ -479,7 +479,7 @@ inline size_t warp_smem_bytes()
 }
 
 template <int C, int IBW0, bool GV>
-__global__ void __launch_bounds__(WARPS_PER_CTA * 32) warp_kernel(const EvalParams p)
+__global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_kernel(const EvalParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double s_best[WARPS_PER_CTA];
