@@ -29,9 +29,12 @@ import ss_inputs  # noqa: E402
 METRIC = "object_frequency_evals_per_second"
 UNIT = "evals/s"
 
-# Algorithmic work per point-eval: fp64 operations the method itself needs
-# in the windowed-moment formulation, FMA = 2 FLOP, add/mul/div/sqrt = 1 FLOP.
-FLOP_PER_POINT_EVAL = {"cv": 330.0, "gv": 200.0}
+# Algorithmic work per point-eval: fp64 pipe lane-instructions
+# ("slots") the method itself needs in the windowed-moment formulation -- 133 add/mul/fma + 10 div/sqrt
+# at 8 slots each (CV), 85 + 10 (GV) -- reported as FMA-equivalent FLOP (2 per slot) against a peak that
+# counts an FMA as 2.
+SLOTS_PER_POINT_EVAL = {"cv": 213.0, "gv": 165.0}
+FLOP_PER_POINT_EVAL = {m: 2.0 * s for m, s in SLOTS_PER_POINT_EVAL.items()}
 FP64_LANES_PER_SM = 64          # B200 fp64 pipe: 64 FMA lanes per SM per clock
 N_SM = 148
 
