@@ -485,7 +485,10 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_ker
     __shared__ double s_best[WARPS_PER_CTA];
     __shared__ long long s_bestk[WARPS_PER_CTA];
     constexpr int NE = WarpNE<C, GV>::value;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    // warp index through a lane-0 broadcast: the compiler then knows it (and the eval loop's bounds) to be
+    // warp-uniform, so the shuffles inside the loop need no WARPSYNC / ENDCOLLECTIVE wrappers
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const int item = blockIdx.x;
     const int li = item / p.chunks_per_obj, ch = item - li * p.chunks_per_obj;
     const int ri = p.list[li];
