@@ -23,6 +23,7 @@ namespace ss {
 constexpr bool WARP_IMPLEMENTED = true;
 constexpr int WARPS_PER_CTA = 8;
 constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lanes + the total)
+constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0
 
 template <int C> struct Pow2Ceil { static constexpr int value = C <= 2 ? 2 : (C <= 4 ? 4 : 8); };
 
@@ -44,24 +45,44 @@ __device__ __forceinline__ double shfl_down_d(double v, int d) { return __shfl_d
 template <int C>
 __device__ __forceinline__ int wst(int e) { return (e % C) * WROW + e / C; }
 
-// Warp-wide exclusive prefix of C values per lane (blocked); writes E[j], j = 0..32C, transposed.
-template <int C>
-__device__ __forceinline__ void warp_prefix_store(const double (&v)[C], double* E, int lane)
+// One Kogge-Stone step on a double: inc += (value of lane - d) for lanes >= d.  The shuffle's own
+// "source in range" predicate guards the add, so the step is 2 SHFL + 1 predicated DADD (a C-level
+// `if (lane >= d)` compiles to an unconditional add plus two FSEL).
+__device__ __forceinline__ void scan_step(double& inc, int d)
 {
-    double e[C];
-    double run = 0.0;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        ".reg .b32 lo, hi, olo, ohi;\n\t"
+        ".reg .f64 o;\n\t"
+        "mov.b64 {lo, hi}, %0;\n\t"
+        "shfl.sync.up.b32 olo|p, lo, %1, 0, 0xffffffff;\n\t"
+        "shfl.sync.up.b32 ohi, hi, %1, 0, 0xffffffff;\n\t"
+        "mov.b64 o, {olo, ohi};\n\t"
+        "@p add.f64 %0, %0, o;\n\t"
+        "}"
+        : "+d"(inc)
+        : "r"(d));
+}
+
+// Warp-wide exclusive prefix sums of two arrays at once (C values per lane, blocked), written
+// interleaved as double2 and transposed: E[wst(j)] = (sum_{i<j} a_i, sum_{i<j} b_i), j = 0..32C.
+template <int C>
+__device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const double (&b)[C], double2* E, int lane)
+{
+    double ea[C], eb[C];
+    double ra = a[0], rb = b[0];
+    ea[0] = 0.0; eb[0] = 0.0;
 #pragma unroll
-    for (int s = 0; s < C; s++) { e[s] = run; run += v[s]; }
-    double inc = run;
+    for (int s = 1; s < C; s++) { ea[s] = ra; ra += a[s]; eb[s] = rb; rb += b[s]; }
+    double ia = ra, ib = rb;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        double o = shfl_up_d(inc, d);
-        if (lane >= d) inc += o;
-    }
-    const double excl = inc - run;
+    for (int d = 1; d < 32; d <<= 1) { scan_step(ia, d); scan_step(ib, d); }
+    const double xa = ia - ra, xb = ib - rb;
+    E[lane] = make_double2(xa, xb);
 #pragma unroll
-    for (int s = 0; s < C; s++) E[s * WROW + lane] = excl + e[s];
-    if (lane == 31) E[32] = inc;     // E[32*C] lives at row 0, column 32
+    for (int s = 1; s < C; s++) E[s * WROW + lane] = make_double2(xa + ea[s], xb + eb[s]);
+    if (lane == 31) E[32] = make_double2(ia, ib);     // E[32*C] lives at row 0, column 32
 }
 
 __device__ __forceinline__ void cex32(unsigned& a, unsigned& b)
@@ -112,67 +133,11 @@ __device__ __forceinline__ void warp_sort(unsigned (&key)[S], int lane)
     }
 }
 
-// Fit ingredients of one window, shareable between points that use the same window (clamped ends).
-struct WinFit {
-    double inv_sw, xbar, inv_sxx;   // x-moments (xbar absolute, in centred-x units)
-    double zbar, b;                 // z-moments folded into mean and slope
-    double g;                       // GV score (GV only)
-};
-
-// Direct sums over the 2*IBW0+1 window centred on halo element `ctr` of (ux, uw, uz).
-template <int C, int IBW0, bool GV>
-__device__ __forceinline__ WinFit tweeter_fit(const double (&ux)[C + 2 * IBW0], const double (&uw)[C + 2 * IBW0],
-                                              const double (&uz)[C + 2 * IBW0], int s, double vsmlsq)
-{
-    const double c = ux[IBW0 + s];
-    double m0 = 0.0, m1 = 0.0, m2 = 0.0, mz = 0.0, m1z = 0.0, mzz = 0.0;
-#pragma unroll
-    for (int t = 0; t <= 2 * IBW0; t++) {
-        const double d = ux[s + t] - c, w_ = uw[s + t], z_ = uz[s + t];
-        const double wd = w_ * d, wz = w_ * z_;
-        m0 += w_; m1 += wd; m2 += wd * d; mz += wz; m1z += wd * z_;
-        if (GV) mzz += wz * z_;
-    }
-    WinFit f;
-    f.inv_sw = m0 > 0.0 ? rcp64(m0) : 0.0;
-    const double xr = m1 * f.inv_sw;             // xbar relative to c
-    const double sxx = m2 - xr * m1;
-    f.inv_sxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-    f.xbar = c + xr;
-    f.zbar = mz * f.inv_sw;
-    const double sxz = m1z - xr * mz;
-    f.b = sxz * f.inv_sxx;
-    f.g = 0.0;
-    if (GV) {
-        double rss = (mzz - f.zbar * mz) - f.b * sxz;
-        rss = rss > 0.0 ? rss : 0.0;
-        const double p = f.inv_sxx != 0.0 ? 2.0 : 1.0;
-        f.g = m0 > 0.0 ? sqrt(rss * f.inv_sw) * rcp64(1.0 - p / (double)(2 * IBW0 + 1)) : 0.0;
-    }
-    return f;
-}
-
-// Only the z-dependent part, x-moments given (final smooth of CV).
-template <int C, int IBW0>
-__device__ __forceinline__ void tweeter_refit(const double (&ux)[C + 2 * IBW0], const double (&uw)[C + 2 * IBW0],
-                                              const double (&uz)[C + 2 * IBW0], int s, double inv_sw, double xbar,
-                                              double inv_sxx, double& zbar, double& b)
-{
-    const double c = ux[IBW0 + s];
-    double mz = 0.0, m1z = 0.0;
-#pragma unroll
-    for (int t = 0; t <= 2 * IBW0; t++) {
-        const double wz = uw[s + t] * uz[s + t];
-        mz += wz; m1z += wz * (ux[s + t] - c);
-    }
-    zbar = mz * inv_sw;
-    b = (m1z - (xbar - c) * mz) * inv_sxx;
-}
-
-// Halo of one register array: u[t] = element at j = lane*C - IBW0 + t.
+// Halo of one register array: u[t] = element at j = lane*C - IBW0 + t (fill outside 0..32C-1).
 template <int C, int IBW0>
 __device__ __forceinline__ void make_halo(const double (&v)[C], double (&u)[C + 2 * IBW0], int lane, double fill)
 {
+    static_assert(IBW0 <= C, "halo reaches one lane to either side");
 #pragma unroll
     for (int t = 0; t < IBW0; t++) {
         double l = shfl_up_d(v[C - IBW0 + t], 1);
@@ -184,104 +149,179 @@ __device__ __forceinline__ void make_halo(const double (&v)[C], double (&u)[C + 
     for (int s = 0; s < C; s++) u[IBW0 + s] = v[s];
 }
 
-template <int C>
-__device__ __forceinline__ double pick_slot(const double (&v)[C], int slot)
+// Sums of e over the 2*IBW0+1 halo elements around each of the lane's C points, by sliding:
+// out[0] = e[0] + .. + e[2*IBW0]; out[s] = out[s-1] + e[s + 2*IBW0] - e[s-1].
+template <int C, int IBW0>
+__device__ __forceinline__ void slide_sums(const double (&e)[C + 2 * IBW0], double (&out)[C])
 {
-    double r = v[0];
+    double acc = e[0];
 #pragma unroll
-    for (int s = 1; s < C; s++) r = slot == s ? v[s] : r;
-    return r;
+    for (int t = 1; t <= 2 * IBW0; t++) acc += e[t];
+    out[0] = acc;
+#pragma unroll
+    for (int s = 1; s < C; s++) { acc += e[s + 2 * IBW0] - e[s - 1]; out[s] = acc; }
+}
+
+// Value of register slot `slot` (warp-uniform, run time) of lane `src`, without a select chain:
+// the uniform branch picks the one shuffle that runs.
+template <int C>
+__device__ __forceinline__ double bcast_slot(const double (&a)[C], int slot, int src)
+{
+    double v = 0.0;
+#pragma unroll
+    for (int s = 0; s < C; s++)
+        if (slot == s) v = shfl_d(a[s], src);
+    return v;
+}
+
+// sqrt(v) for v >= 0: MUFU.RSQ64H seed and two coupled Newton steps (Goldschmidt), ~1 ulp; 0 for v <= 0.
+__device__ __forceinline__ double sqrt64(double v)
+{
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(v));
+    double g = v * r, h = 0.5 * r;
+    double e = fma(-h, g, 0.5);
+    g = fma(g, e, g); h = fma(h, e, h);
+    e = fma(-h, g, 0.5);
+    g = fma(g, e, g);
+    return v > 0.0 ? g : 0.0;
 }
 
 // Per-warp view of the shared memory.
 struct WarpMem {
     const double* tt; const double* yc; const double* w;   // the object's arrays (CTA-wide)
-    double* E;               // per-warp: NE prefix arrays of C*WROW doubles
+    double2* E;              // per-warp: 3 pair-prefix arrays of C*WROW double2
     unsigned char* perm;     // per-warp: 256 bytes (rank -> index), only when S != C
 };
 
+// Per-object constants of the eval loop (warp-uniform).
+struct EvalConst {
+    int n, ibw1, ibw2, K1, K2;
+    int lane_r, slot_r;      // owner of the right-end tweeter window, jr = n-1-IBW0
+    int q1l, q1s, q3l, q3s;  // owners of the quartile points
+    double gk1[2], gk2[2];   // 1/(1 - p/K) for p = 1, 2 (GV score, R12)
+    double alpha, bexp;      // bass enhancement
+    int bass;                // 0 = off, 1 = exponent 1 (alpha = 9), 2 = general pow
+    double chi0, inv_chi0;
+};
 
-// Window of span i for point j through the prefix arrays: S = E[lo+K] - E[lo].
-template <int C>
-__device__ __forceinline__ double wdiff(const double* E, int slo, int shi) { return E[shi] - E[slo]; }
+// Listing 1 lines 63-77 with the loop-invariant tests hoisted.
+__device__ __forceinline__ double pick_span_w(double v0, double v1, double v2, const EvalConst& K)
+{
+    double resmin = v0, sp = SPAN0;
+    if (!(v0 < 1.e20)) { resmin = 1.e20; sp = 0.0; }
+    if (v1 < resmin) { resmin = v1; sp = SPAN1; }
+    if (v2 < resmin) { resmin = v2; sp = SPAN2; }
+    if (K.bass != 0 && resmin < v2 && resmin > 0.0) {
+        double tmp = resmin * rcp64(v2);
+        if (tmp < 1.e-7) tmp = 1.e-7;
+        const double pw = K.bass == 1 ? tmp : pow(tmp, K.bexp);
+        sp += (SPAN2 - sp) * pw;
+    }
+    return sp;
+}
 
 // Smoother + statistic on the sorted, gathered eval (x centred by 0.5, y centred by ybar_w).
+// Padded slots (j >= n) carry x = 0, y = 0, w = W_PAD.
 template <int C, int IBW0, bool GV>
-__device__ __forceinline__ double warp_eval_body(const ObjRec& rec, const WarpMem& M, const double (&x)[C],
+__device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpMem& M, const double (&x)[C],
                                                  const double (&y)[C], const double (&w)[C], double vsmlsq,
-                                                 double alpha, int lane, bool& defer)
+                                                 int lane, bool& defer)
 {
     constexpr int ASZ = C * WROW;
-    const int n = rec.n;
-    const int ibw1 = rec.ibw[1], ibw2 = rec.ibw[2];
-    const int K1 = min(2 * ibw1 + 1, n), K2 = min(2 * ibw2 + 1, n);
-    double* Ew = M.E;            double* Ewx = M.E + ASZ;      double* Ewxx = M.E + 2 * ASZ;
-    double* Ewy = M.E + 3 * ASZ; double* Ewxy = M.E + 4 * ASZ; double* Ewyy = M.E + 5 * ASZ;   // Ewyy: GV only
+    constexpr int H = C + 2 * IBW0;
+    constexpr int K0 = 2 * IBW0 + 1;
+    const int n = K.n;
+    double2* E01 = M.E;             // (w, wx)
+    double2* E23 = M.E + ASZ;       // (wxx, wy)
+    double2* E45 = M.E + 2 * ASZ;   // (wxy, wyy)
 
     // ---- prefix sums of the weighted moments (midrange and woofer windows)
     {
-        double v[C];
+        double a[C], b[C], c[C];
 #pragma unroll
-        for (int s = 0; s < C; s++) v[s] = w[s];
-        warp_prefix_store<C>(v, Ew, lane);
+        for (int s = 0; s < C; s++) { a[s] = w[s]; b[s] = w[s] * x[s]; }
+        pair_prefix_store<C>(a, b, E01, lane);
 #pragma unroll
-        for (int s = 0; s < C; s++) v[s] = w[s] * x[s];
-        warp_prefix_store<C>(v, Ewx, lane);
-        double v2[C];
+        for (int s = 0; s < C; s++) { c[s] = b[s] * x[s]; a[s] = w[s] * y[s]; }
+        pair_prefix_store<C>(c, a, E23, lane);
 #pragma unroll
-        for (int s = 0; s < C; s++) v2[s] = v[s] * x[s];
-        warp_prefix_store<C>(v2, Ewxx, lane);
-#pragma unroll
-        for (int s = 0; s < C; s++) v2[s] = v[s] * y[s];
-        warp_prefix_store<C>(v2, Ewxy, lane);
-#pragma unroll
-        for (int s = 0; s < C; s++) v[s] = w[s] * y[s];
-        warp_prefix_store<C>(v, Ewy, lane);
-        if (GV) {
-#pragma unroll
-            for (int s = 0; s < C; s++) v[s] = v[s] * y[s];
-            warp_prefix_store<C>(v, Ewyy, lane);
-        }
+        for (int s = 0; s < C; s++) { b[s] = b[s] * y[s]; c[s] = GV ? a[s] * y[s] : 0.0; }
+        pair_prefix_store<C>(b, c, E45, lane);
     }
     __syncwarp();
 
-    // ---- tweeter: direct window sums from neighbour-lane halos
-    double ux[C + 2 * IBW0], uw[C + 2 * IBW0], uz[C + 2 * IBW0];
-    make_halo<C, IBW0>(x, ux, lane, 0.0);
-    make_halo<C, IBW0>(w, uw, lane, 0.0);
-    make_halo<C, IBW0>(y, uz, lane, 0.0);
-    WinFit tw[C];
+    // ---- tweeter: window sums about the lane's first point from neighbour-lane halos, sliding
+    double t_isw[C], t_xb[C], t_isxx[C], t_zb[C], t_b[C], t_g[C];
+    {
+        double ux[H], uw[H], uy[H];
+        make_halo<C, IBW0>(x, ux, lane, 0.0);
+        make_halo<C, IBW0>(w, uw, lane, 0.0);
+        make_halo<C, IBW0>(y, uy, lane, 0.0);
+        const double c0 = x[0];
+        double m0[C], m1[C], m2[C], mz[C], m1z[C], mzz[C];
+        slide_sums<C, IBW0>(uw, m0);
+        double e1[H], e2[H];
 #pragma unroll
-    for (int s = 0; s < C; s++) tw[s] = tweeter_fit<C, IBW0, GV>(ux, uw, uz, s, vsmlsq);
+        for (int t = 0; t < H; t++) { ux[t] -= c0; e1[t] = uw[t] * ux[t]; }
+        slide_sums<C, IBW0>(e1, m1);
+#pragma unroll
+        for (int t = 0; t < H; t++) e2[t] = e1[t] * ux[t];
+        slide_sums<C, IBW0>(e2, m2);
+#pragma unroll
+        for (int t = 0; t < H; t++) e2[t] = e1[t] * uy[t];
+        slide_sums<C, IBW0>(e2, m1z);
+#pragma unroll
+        for (int t = 0; t < H; t++) e1[t] = uw[t] * uy[t];
+        slide_sums<C, IBW0>(e1, mz);
+        if (GV) {
+#pragma unroll
+            for (int t = 0; t < H; t++) e2[t] = e1[t] * uy[t];
+            slide_sums<C, IBW0>(e2, mzz);
+        }
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            const double isw = rcp64(m0[s]);
+            const double xr = m1[s] * isw;              // xbar relative to c0
+            const double sxx = m2[s] - xr * m1[s];
+            const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+            const double zb = mz[s] * isw;
+            const double sxz = m1z[s] - xr * mz[s];
+            const double b = sxz * isxx;
+            t_isw[s] = isw; t_xb[s] = c0 + xr; t_isxx[s] = isxx; t_zb[s] = zb; t_b[s] = b;
+            if (GV) {
+                double rss = (mzz[s] - zb * mz[s]) - b * sxz;
+                constexpr double G1 = 1.0 / (1.0 - 1.0 / (double)K0), G2 = 1.0 / (1.0 - 2.0 / (double)K0);
+                t_g[s] = sqrt64(rss * isw) * (isxx != 0.0 ? G2 : G1);
+            }
+        }
+    }
     // clamped ends (O4): points j < IBW0 use the window of jl = IBW0, points j > jr = n-1-IBW0 the
     // window of jr.  The owner's fit is broadcast.
     const int jr = n - 1 - IBW0;
-    const int lane_r = jr / C, slot_r = jr % C;
-    WinFit twl, twr;
     {
-        double a[C];
-#define SS_BCAST(field)                                                                   \
+        constexpr int LL = IBW0 / C, LS = IBW0 % C;      // owner of the left-end window (static)
+        const int sr = K.slot_r, lr = K.lane_r;
+#define SS_CLAMP(arr)                                                                     \
         {                                                                                 \
-            _Pragma("unroll") for (int s = 0; s < C; s++) a[s] = tw[s].field;             \
-            twr.field = shfl_d(pick_slot<C>(a, slot_r), lane_r);                          \
-            twl.field = IBW0 < C ? shfl_d(a[IBW0 < C ? IBW0 : 0], 0) : shfl_d(a[0], 1);   \
+            const double vl = shfl_d(arr[LS], LL);                                        \
+            const double vr = bcast_slot<C>(arr, sr, lr);                                 \
+            _Pragma("unroll") for (int s = 0; s < C; s++) {                               \
+                const int j = lane * C + s;                                               \
+                if (s < IBW0 && j < IBW0) arr[s] = vl;                                    \
+                if (j > jr) arr[s] = vr;                                                  \
+            }                                                                             \
         }
-        SS_BCAST(inv_sw) SS_BCAST(xbar) SS_BCAST(inv_sxx) SS_BCAST(zbar) SS_BCAST(b)
-        if (GV) SS_BCAST(g)
-    }
-#pragma unroll
-    for (int s = 0; s < C; s++) {
-        const int j = lane * C + s;
-        if (j < IBW0) tw[s] = twl;
-        if (j > jr) tw[s] = twr;
+        SS_CLAMP(t_isw) SS_CLAMP(t_xb) SS_CLAMP(t_isxx) SS_CLAMP(t_zb) SS_CLAMP(t_b)
+        if (GV) SS_CLAMP(t_g)
     }
 
-    // ---- window indices of the midrange and woofer spans (transposed storage)
+    // ---- window indices of the midrange span (transposed storage)
     int s1lo[C], s1hi[C];
 #pragma unroll
     for (int s = 0; s < C; s++) {
-        const int lo = window_lo(lane * C + s, ibw1, K1, n);
-        s1lo[s] = wst<C>(lo); s1hi[s] = wst<C>(lo + K1);
+        const int lo = window_lo(lane * C + s, K.ibw1, K.K1, n);
+        s1lo[s] = wst<C>(lo); s1hi[s] = wst<C>(lo + K.K1);
     }
 
     double chi2 = 0.0;
@@ -290,21 +330,36 @@ __device__ __forceinline__ double warp_eval_body(const ObjRec& rec, const WarpMe
 #pragma unroll
         for (int s = 0; s < C; s++) {
             const double xj = x[s];
-            const double A0 = tw[s].zbar + tw[s].b * (xj - tw[s].xbar);
-            XMom m1 = x_moments(wdiff<C>(Ew, s1lo[s], s1hi[s]), wdiff<C>(Ewx, s1lo[s], s1hi[s]),
-                                wdiff<C>(Ewxx, s1lo[s], s1hi[s]), vsmlsq);
-            double b1, yb1;
-            const double Sy1 = wdiff<C>(Ewy, s1lo[s], s1hi[s]), Sxy1 = wdiff<C>(Ewxy, s1lo[s], s1hi[s]);
-            const double A1 = line_fit(m1, Sy1, Sxy1, xj, b1, yb1);
-            const double G1 = gv_score(m1, Sy1, Sxy1, wdiff<C>(Ewyy, s1lo[s], s1hi[s]), b1, yb1, K1);
-            const int lo2 = window_lo(lane * C + s, ibw2, K2, n);
-            const int a2 = wst<C>(lo2), b2i = wst<C>(lo2 + K2);
-            XMom m2 = x_moments(wdiff<C>(Ew, a2, b2i), wdiff<C>(Ewx, a2, b2i), wdiff<C>(Ewxx, a2, b2i), vsmlsq);
-            double b2, yb2;
-            const double Sy2 = wdiff<C>(Ewy, a2, b2i), Sxy2 = wdiff<C>(Ewxy, a2, b2i);
-            const double A2 = line_fit(m2, Sy2, Sxy2, xj, b2, yb2);
-            const double G2 = gv_score(m2, Sy2, Sxy2, wdiff<C>(Ewyy, a2, b2i), b2, yb2, K2);
-            const double sp = pick_span(tw[s].g, G1, G2, alpha);
+            const double A0 = t_zb[s] + t_b[s] * (xj - t_xb[s]);
+            double A1, A2, G1, G2;
+            {
+                const double2 l0 = E01[s1lo[s]], h0 = E01[s1hi[s]], l1 = E23[s1lo[s]], h1 = E23[s1hi[s]];
+                const double2 l2 = E45[s1lo[s]], h2 = E45[s1hi[s]];
+                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                const double isw = rcp64(Sw), xb = Swx * isw;
+                const double sxx = Swxx - xb * Swx;
+                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+                const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
+                A1 = yb + b * (xj - xb);
+                const double rss = (Syy - yb * Sy) - b * sxy;
+                G1 = sqrt64(rss * isw) * (isxx != 0.0 ? K.gk1[1] : K.gk1[0]);
+            }
+            {
+                const int lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
+                const int a2 = wst<C>(lo2), b2 = wst<C>(lo2 + K.K2);
+                const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2], l2 = E45[a2], h2 = E45[b2];
+                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                const double isw = rcp64(Sw), xb = Swx * isw;
+                const double sxx = Swxx - xb * Swx;
+                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+                const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
+                A2 = yb + b * (xj - xb);
+                const double rss = (Syy - yb * Sy) - b * sxy;
+                G2 = sqrt64(rss * isw) * (isxx != 0.0 ? K.gk2[1] : K.gk2[0]);
+            }
+            const double sp = pick_span_w(t_g[s], G1, G2, K);
             const double smo = interp_spans(sp, A0, A1, A2);
             const double r = y[s] - smo;
             chi2 += w[s] * r * r;
@@ -312,101 +367,130 @@ __device__ __forceinline__ double warp_eval_body(const ObjRec& rec, const WarpMe
     } else {
         // ---- CV pass 1
         double A0[C], A1[C], A2[C], r0[C], r1[C], r2[C];
-        double m_isw[C], m_xb[C], m_isxx[C];      // midrange x-moments, reused by four more smooths
-        bool bad = false;
+        double m_isw[C], m_xb[C], m_g[C];      // midrange x-moments, reused by four more smooths
+        int amin = 0x7fffffff;                 // smallest high word of the three LOO denominators
 #pragma unroll
         for (int s = 0; s < C; s++) {
             const double xj = x[s], yj = y[s], wj = w[s];
-            A0[s] = tw[s].zbar + tw[s].b * (xj - tw[s].xbar);
             {
-                const double dx = xj - tw[s].xbar;
-                const double a = 1.0 - wj * (tw[s].inv_sw + dx * dx * tw[s].inv_sxx);
-                r0[s] = a > 0.0 ? fabs(yj - A0[s]) * rcp64(a) : -1.0;
+                const double dx = xj - t_xb[s];
+                A0[s] = t_zb[s] + t_b[s] * dx;
+                const double a = 1.0 - wj * (t_isw[s] + dx * dx * t_isxx[s]);
+                r0[s] = fabs(yj - A0[s]) * rcp64(a);
+                amin = min(amin, __double2hiint(a));
             }
-            XMom m1 = x_moments(wdiff<C>(Ew, s1lo[s], s1hi[s]), wdiff<C>(Ewx, s1lo[s], s1hi[s]),
-                                wdiff<C>(Ewxx, s1lo[s], s1hi[s]), vsmlsq);
-            m_isw[s] = m1.inv_sw; m_xb[s] = m1.xbar; m_isxx[s] = m1.inv_sxx;
-            double b_, zb_;
-            A1[s] = line_fit(m1, wdiff<C>(Ewy, s1lo[s], s1hi[s]), wdiff<C>(Ewxy, s1lo[s], s1hi[s]), xj, b_, zb_);
-            r1[s] = loo_residual(m1, xj, wj, yj, A1[s]);
-            const int lo2 = window_lo(lane * C + s, ibw2, K2, n);
-            const int a2 = wst<C>(lo2), b2i = wst<C>(lo2 + K2);
-            XMom m2 = x_moments(wdiff<C>(Ew, a2, b2i), wdiff<C>(Ewx, a2, b2i), wdiff<C>(Ewxx, a2, b2i), vsmlsq);
-            A2[s] = line_fit(m2, wdiff<C>(Ewy, a2, b2i), wdiff<C>(Ewxy, a2, b2i), xj, b_, zb_);
-            r2[s] = loo_residual(m2, xj, wj, yj, A2[s]);
-            if (lane * C + s < n && (r0[s] < 0.0 || r1[s] < 0.0 || r2[s] < 0.0)) bad = true;
+            {
+                const double2 l0 = E01[s1lo[s]], h0 = E01[s1hi[s]], l1 = E23[s1lo[s]], h1 = E23[s1hi[s]];
+                const double lxy = E45[s1lo[s]].x, hxy = E45[s1hi[s]].x;
+                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const double Sxy = hxy - lxy;
+                const double isw = rcp64(Sw), xb = Swx * isw;
+                const double sxx = Swxx - xb * Swx;
+                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+                const double dx = xj - xb;
+                m_isw[s] = isw; m_xb[s] = xb; m_g[s] = isxx * dx;
+                A1[s] = Sy * isw + (Sxy - xb * Sy) * m_g[s];
+                const double a = 1.0 - wj * (isw + dx * m_g[s]);
+                r1[s] = fabs(yj - A1[s]) * rcp64(a);
+                amin = min(amin, __double2hiint(a));
+            }
+            {
+                const int lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
+                const int a2 = wst<C>(lo2), b2 = wst<C>(lo2 + K.K2);
+                const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2];
+                const double lxy = E45[a2].x, hxy = E45[b2].x;
+                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const double Sxy = hxy - lxy;
+                const double isw = rcp64(Sw), xb = Swx * isw;
+                const double sxx = Swxx - xb * Swx;
+                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+                const double dx = xj - xb, g = isxx * dx;
+                A2[s] = Sy * isw + (Sxy - xb * Sy) * g;
+                const double a = 1.0 - wj * (isw + dx * g);
+                r2[s] = fabs(yj - A2[s]) * rcp64(a);
+                amin = min(amin, __double2hiint(a));
+            }
         }
-        if (__any_sync(0xffffffffu, bad)) { defer = true; return 0.0; }
-        __syncwarp();      // every lane is done reading Ewy / Ewxy
+        // a <= 0 (or below the smallest normal): the residual carries (R23) -> generic path.  Padded slots have a ~ 1.
+        if (__any_sync(0xffffffffu, amin < 0x00100000)) { defer = true; return 0.0; }
+        __syncwarp();      // every lane is done reading the primary prefix arrays
 
-        // midrange smooth of a register array z through two prefix arrays
-        auto mid_smooth = [&](const double (&z)[C], double (&out)[C]) {
-            double v[C];
+        // midrange smooth of a register array z through one pair-prefix array
+        auto mid_store = [&](const double (&z)[C], double2* Ez) {
+            double a[C], b[C];
 #pragma unroll
-            for (int s = 0; s < C; s++) v[s] = w[s] * z[s];
-            warp_prefix_store<C>(v, Ewy, lane);
-#pragma unroll
-            for (int s = 0; s < C; s++) v[s] = v[s] * x[s];
-            warp_prefix_store<C>(v, Ewxy, lane);
-            __syncwarp();
+            for (int s = 0; s < C; s++) { a[s] = w[s] * z[s]; b[s] = a[s] * x[s]; }
+            pair_prefix_store<C>(a, b, Ez, lane);
+        };
+        auto mid_load = [&](const double2* Ez, double (&out)[C]) {
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double Sz = wdiff<C>(Ewy, s1lo[s], s1hi[s]), Sxz = wdiff<C>(Ewxy, s1lo[s], s1hi[s]);
-                const double zb = Sz * m_isw[s];
-                out[s] = zb + (Sxz - m_xb[s] * Sz) * m_isxx[s] * (x[s] - m_xb[s]);
+                const double2 l = Ez[s1lo[s]], h = Ez[s1hi[s]];
+                const double Sz = h.x - l.x, Sxz = h.y - l.y;
+                out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
             }
-            __syncwarp();
         };
         double sp[C];
         {
+            mid_store(r0, E01); mid_store(r1, E23); mid_store(r2, E45);
+            __syncwarp();
             double R0[C], R1[C], R2[C];
-            mid_smooth(r0, R0);
-            mid_smooth(r1, R1);
-            mid_smooth(r2, R2);
+            mid_load(E01, R0); mid_load(E23, R1); mid_load(E45, R2);
             // span pick + bass enhancement
 #pragma unroll
-            for (int s = 0; s < C; s++) sp[s] = pick_span(R0[s], R1[s], R2[s], alpha);
+            for (int s = 0; s < C; s++) sp[s] = pick_span_w(R0[s], R1[s], R2[s], K);
         }
-        double sps[C];
-        mid_smooth(sp, sps);
+        __syncwarp();
+        mid_store(sp, E01);
+        __syncwarp();
         double B[C];
+        mid_load(E01, B);
 #pragma unroll
-        for (int s = 0; s < C; s++) B[s] = interp_spans(sps[s], A0[s], A1[s], A2[s]);
-        // ---- final tweeter smooth, direct sums again
-        make_halo<C, IBW0>(B, uz, lane, 0.0);
+        for (int s = 0; s < C; s++) B[s] = interp_spans(B[s], A0[s], A1[s], A2[s]);
+        // ---- final tweeter smooth: direct window sums of (wB, wxB), sliding
         double zb[C], bb[C];
+        {
+            double p1[C], p2[C], u[H];
 #pragma unroll
-        for (int s = 0; s < C; s++)
-            tweeter_refit<C, IBW0>(ux, uw, uz, s, tw[s].inv_sw, tw[s].xbar, tw[s].inv_sxx, zb[s], bb[s]);
-        // NOTE: for clamped points tw[s] already holds the shared window's x-moments, but the z-sums
+            for (int s = 0; s < C; s++) { p1[s] = w[s] * B[s]; p2[s] = p1[s] * x[s]; }
+            make_halo<C, IBW0>(p1, u, lane, 0.0);
+            slide_sums<C, IBW0>(u, zb);
+            make_halo<C, IBW0>(p2, u, lane, 0.0);
+            slide_sums<C, IBW0>(u, bb);
+#pragma unroll
+            for (int s = 0; s < C; s++) {
+                const double mz = zb[s];
+                zb[s] = mz * t_isw[s];
+                bb[s] = (bb[s] - t_xb[s] * mz) * t_isxx[s];
+            }
+        }
+        // NOTE: for clamped points t_*[s] already hold the shared window's x-moments, but the z-sums
         // above were taken over the point's own (wrong) window: take the owner's (zbar, b).
-        const double zr = shfl_d(pick_slot<C>(zb, slot_r), lane_r), br = shfl_d(pick_slot<C>(bb, slot_r), lane_r);
-        const double zl = IBW0 < C ? shfl_d(zb[IBW0 < C ? IBW0 : 0], 0) : shfl_d(zb[0], 1);
-        const double bl = IBW0 < C ? shfl_d(bb[IBW0 < C ? IBW0 : 0], 0) : shfl_d(bb[0], 1);
+        {
+            constexpr int LL = IBW0 / C, LS = IBW0 % C;
+            const int sr = K.slot_r, lr = K.lane_r;
+            SS_CLAMP(zb) SS_CLAMP(bb)
+        }
 #pragma unroll
         for (int s = 0; s < C; s++) {
-            const int j = lane * C + s;
-            double z_ = zb[s], b_ = bb[s];
-            if (j < IBW0) { z_ = zl; b_ = bl; }
-            if (j > jr) { z_ = zr; b_ = br; }
-            const double smo = z_ + b_ * (x[s] - tw[s].xbar);
+            const double smo = zb[s] + bb[s] * (x[s] - t_xb[s]);
             const double r = y[s] - smo;
             chi2 += w[s] * r * r;
         }
     }
+#undef SS_CLAMP
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, d);
-    return rec.chi0 > 0.0 ? (rec.chi0 - chi2) / rec.chi0 : 0.0;
+    return (K.chi0 - chi2) * K.inv_chi0;
 }
 
 // One eval.  Returns P in every lane; `defer` is set (warp-uniform) when the fast path cannot
 // decide the eval exactly.
 template <int C, int IBW0, bool GV>
-__device__ __forceinline__ double warp_eval(const ObjRec& rec, const WarpMem& M, double f, double alpha, int lane,
-                                            bool& defer)
+__device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M, double f, int lane, bool& defer)
 {
     constexpr int S = Pow2Ceil<C>::value;
-    const int n = rec.n;
+    const int n = K.n;
     defer = false;
 
     // ---- P1 fold + 32-bit keys (24 phase bits | 8 index bits); P2 sort
@@ -444,7 +528,7 @@ __device__ __forceinline__ double warp_eval(const ObjRec& rec, const WarpMem& M,
             phi[s] = fold_phase(M.tt[i], f);
             y[s] = M.yc[i];
             w[s] = M.w[i];
-        } else { phi[s] = 4.0; y[s] = 0.0; w[s] = 0.0; }
+        } else { phi[s] = 4.0; y[s] = 0.0; w[s] = W_PAD; }
     }
     bool bad = false;
     double nxt = shfl_down_d(phi[0], 1);
@@ -455,13 +539,13 @@ __device__ __forceinline__ double warp_eval(const ObjRec& rec, const WarpMem& M,
         if (lane * C + s + 1 < n && nx <= phi[s]) bad = true;   // tie or quantisation misorder
     }
     // vsmlsq from the quartile spread
-    const double p1 = shfl_d(pick_slot<C>(phi, rec.q1 % C), rec.q1 / C);
-    const double p3 = shfl_d(pick_slot<C>(phi, rec.q3 % C), rec.q3 / C);
+    const double p1 = bcast_slot<C>(phi, K.q1s, K.q1l);
+    const double p3 = bcast_slot<C>(phi, K.q3s, K.q3l);
     if (__any_sync(0xffffffffu, bad)) { defer = true; return 0.0; }
 #pragma unroll
     for (int s = 0; s < C; s++) x[s] = (lane * C + s < n) ? phi[s] - 0.5 : 0.0;
     const double scale = p3 - p1;
-    return warp_eval_body<C, IBW0, GV>(rec, M, x, y, w, 1.e-6 * scale * scale, alpha, lane, defer);
+    return warp_eval_body<C, IBW0, GV>(K, M, x, y, w, 1.e-6 * scale * scale, lane, defer);
 }
 
 
@@ -469,14 +553,14 @@ __device__ __forceinline__ double warp_eval(const ObjRec& rec, const WarpMem& M,
 // Kernel: one CTA = one work item (object, chunk of frequencies); its WARPS_PER_CTA warps split the
 // chunk into contiguous runs.  P values are staged in registers and written 32 at a time.
 // ------------------------------------------------------------------------------------------------
-template <int C, bool GV> struct WarpNE { static constexpr int value = GV ? 6 : 5; };
-
-template <int C, bool GV>
+template <int C>
 inline size_t warp_smem_bytes()
 {
-    // object arrays (3 x 32C doubles) + per warp: NE prefix arrays + 256 B permutation bytes
-    return (size_t)3 * 32 * C * 8 + (size_t)WARPS_PER_CTA * ((size_t)WarpNE<C, GV>::value * C * WROW * 8 + 256);
+    // object arrays (3 x 32C doubles) + per warp: 3 pair-prefix arrays + 256 B permutation bytes
+    return (size_t)3 * 32 * C * 8 + (size_t)WARPS_PER_CTA * ((size_t)3 * C * WROW * 16 + 256);
 }
+
+__device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 
 template <int C, int IBW0, bool GV>
 __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_kernel(const EvalParams p)
@@ -484,7 +568,6 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_ker
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double s_best[WARPS_PER_CTA];
     __shared__ long long s_bestk[WARPS_PER_CTA];
-    constexpr int NE = WarpNE<C, GV>::value;
     const int tid = threadIdx.x, lane = tid & 31;
     // warp index through a lane-0 broadcast: the compiler then knows it (and the eval loop's bounds) to be
     // warp-uniform, so the shuffles inside the loop need no WARPSYNC / ENDCOLLECTIVE wrappers
@@ -493,16 +576,32 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_ker
     const int li = item / p.chunks_per_obj, ch = item - li * p.chunks_per_obj;
     const int ri = p.list[li];
     const ObjRec rec = p.recs[ri];
-    const int n = rec.n;
+    const int n = uni(rec.n);
+
+    EvalConst K;
+    K.n = n; K.ibw1 = uni(rec.ibw[1]); K.ibw2 = uni(rec.ibw[2]);
+    K.K1 = min(2 * K.ibw1 + 1, n); K.K2 = min(2 * K.ibw2 + 1, n);
+    {
+        const int jr = n - 1 - IBW0;
+        K.lane_r = jr / C; K.slot_r = jr % C;
+        const int q1 = uni(rec.q1), q3 = uni(rec.q3);
+        K.q1l = q1 / C; K.q1s = q1 % C; K.q3l = q3 / C; K.q3s = q3 % C;
+    }
+    K.gk1[0] = 1.0 / (1.0 - 1.0 / (double)K.K1); K.gk1[1] = 1.0 / (1.0 - 2.0 / (double)K.K1);
+    K.gk2[0] = 1.0 / (1.0 - 1.0 / (double)K.K2); K.gk2[1] = 1.0 / (1.0 - 2.0 / (double)K.K2);
+    K.alpha = p.alpha; K.bexp = 10.0 - p.alpha;
+    K.bass = (p.alpha > 0.0 && p.alpha <= 10.0) ? (K.bexp == 1.0 ? 1 : 2) : 0;
+    K.chi0 = rec.chi0; K.inv_chi0 = rec.chi0 > 0.0 ? 1.0 / rec.chi0 : 0.0;
 
     double* o_tt = reinterpret_cast<double*>(smem_raw);
     double* o_y = o_tt + 32 * C;
     double* o_w = o_y + 32 * C;
-    unsigned char* wbase = smem_raw + (size_t)3 * 32 * C * 8 + (size_t)warp * ((size_t)NE * C * WROW * 8 + 256);
+    constexpr size_t WARP_BYTES = (size_t)3 * C * WROW * 16 + 256;
+    unsigned char* wbase = smem_raw + (size_t)3 * 32 * C * 8 + (size_t)warp * WARP_BYTES;
     WarpMem M;
     M.tt = o_tt; M.yc = o_y; M.w = o_w;
-    M.E = reinterpret_cast<double*>(wbase);
-    M.perm = wbase + (size_t)NE * C * WROW * 8;
+    M.E = reinterpret_cast<double2*>(wbase);
+    M.perm = wbase + (size_t)3 * C * WROW * 16;
     for (int j = tid; j < n; j += WARPS_PER_CTA * 32) {
         o_tt[j] = p.tt[rec.off + j];
         o_y[j] = p.yc[rec.off + j];
@@ -523,7 +622,7 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_ker
     for (int64_t k = k0; k < k1; k++) {
         const double f = freq_of(p.f_min, p.df, k);
         bool defer;
-        double P = warp_eval<C, IBW0, GV>(rec, M, f, p.alpha, lane, defer);
+        double P = warp_eval<C, IBW0, GV>(K, M, f, lane, defer);
         if (defer) {
             if (lane == 0) {
                 unsigned pos = atomicAdd(p.defer_count, 1u);
@@ -621,12 +720,12 @@ inline ss_status_t launch_warp_variant(const EvalParams& p, int64_t n_items, cud
 {
     cudaError_t e;
     if (p.mode == 1) {
-        const size_t smem = warp_smem_bytes<C, true>();
+        const size_t smem = warp_smem_bytes<C>();
         e = cudaFuncSetAttribute(warp_kernel<C, IBW0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return SS_ERR_CUDA;
         warp_kernel<C, IBW0, true><<<(unsigned)n_items, WARPS_PER_CTA * 32, smem, stream>>>(p);
     } else {
-        const size_t smem = warp_smem_bytes<C, false>();
+        const size_t smem = warp_smem_bytes<C>();
         e = cudaFuncSetAttribute(warp_kernel<C, IBW0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return SS_ERR_CUDA;
         warp_kernel<C, IBW0, false><<<(unsigned)n_items, WARPS_PER_CTA * 32, smem, stream>>>(p);
