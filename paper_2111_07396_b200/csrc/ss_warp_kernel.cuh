@@ -21,7 +21,14 @@
 namespace ss {
 
 constexpr bool WARP_IMPLEMENTED = true;
-constexpr int WARPS_PER_CTA = 8;
+constexpr int WARPS_PER_CTA = 8;      // frequency chunks are multiples of this (host side)
+
+// Launch shape per points-per-lane: warps per CTA and resident CTAs per SM (register budget =
+// 65536 / (32 * WPC * MINB), rounded down to a multiple of 8).
+template <int C, bool GV> struct WarpCfg {
+    static constexpr int WPC = (C <= 4 || !GV) ? 8 : 4;
+    static constexpr int MINB = C <= 4 ? 2 : (GV ? 3 : 1);
+};
 constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lanes + the total)
 constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0
 
@@ -187,11 +194,46 @@ __device__ __forceinline__ double sqrt64(double v)
     return v > 0.0 ? g : 0.0;
 }
 
+// ---- Tensor memory as a per-thread parking area -------------------------------------------------
+// The warp path is bound by the LSU/shared-memory pipe, and its long-lived per-point values (the
+// three primary smooths, the tweeter x-moments) do not fit the register budget of 16 warps per SM.
+// Blackwell's tensor memory (256 KB per SM, 512 columns x 128 lanes x 32 bit) is idle here, so it
+// serves as a second register file: tcgen05.st/ld with the 32x32b shape give thread i of a warp
+// its own lane (32*(warp%4) + i) and any run of columns, off the LSU pipe.
+__device__ __forceinline__ void tmem_st2(uint32_t taddr, double v)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};"
+                 :: "r"(taddr), "r"(__double2loint(v)), "r"(__double2hiint(v)) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void tmem_park(uint32_t taddr, const double (&v)[N])
+{
+#pragma unroll
+    for (int s = 0; s < N; s++) tmem_st2(taddr + 2 * s, v[s]);
+}
+template <int N>
+__device__ __forceinline__ void tmem_fetch(uint32_t taddr, double (&v)[N])
+{
+    int lo[N], hi[N];
+#pragma unroll
+    for (int s = 0; s < N; s++)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];"
+                     : "=r"(lo[s]), "=r"(hi[s]) : "r"(taddr + 2 * s) : "memory");
+    // the loaded registers are valid only after the wait: tie them to it
+#pragma unroll
+    for (int s = 0; s < N; s++)
+        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(lo[s]), "+r"(hi[s]) :: "memory");
+#pragma unroll
+    for (int s = 0; s < N; s++) v[s] = __hiloint2double(hi[s], lo[s]);
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
 // Per-warp view of the shared memory.
 struct WarpMem {
     const double* tt; const double* yc; const double* w;   // the object's arrays (CTA-wide)
     double2* E;              // per-warp: 3 pair-prefix arrays of C*WROW double2
     unsigned char* perm;     // per-warp: 256 bytes (rank -> index), only when S != C
+    uint32_t tmem;           // per-warp tensor-memory base (lane quarter + first column), CV only
 };
 
 // Per-object constants of the eval loop (warp-uniform).
@@ -414,6 +456,9 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         // a <= 0 (or below the smallest normal): the residual carries (R23) -> generic path.  Padded slots have a ~ 1.
         if (__any_sync(0xffffffffu, amin < 0x00100000)) { defer = true; return 0.0; }
         __syncwarp();      // every lane is done reading the primary prefix arrays
+        // park what is not needed during the four secondary smooths in tensor memory
+        tmem_park<C>(M.tmem, A0); tmem_park<C>(M.tmem + 2 * C, A1); tmem_park<C>(M.tmem + 4 * C, A2);
+        tmem_park<C>(M.tmem + 6 * C, t_isw); tmem_park<C>(M.tmem + 8 * C, t_xb); tmem_park<C>(M.tmem + 10 * C, t_isxx);
 
         // midrange smooth of a register array z through one pair-prefix array
         auto mid_store = [&](const double (&z)[C], double2* Ez) {
@@ -445,8 +490,13 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         __syncwarp();
         double B[C];
         mid_load(E01, B);
+        tmem_wait_st();
+        {
+            double a0[C], a1[C], a2[C];
+            tmem_fetch<C>(M.tmem, a0); tmem_fetch<C>(M.tmem + 2 * C, a1); tmem_fetch<C>(M.tmem + 4 * C, a2);
 #pragma unroll
-        for (int s = 0; s < C; s++) B[s] = interp_spans(B[s], A0[s], A1[s], A2[s]);
+            for (int s = 0; s < C; s++) B[s] = interp_spans(B[s], a0[s], a1[s], a2[s]);
+        }
         // ---- final tweeter smooth: direct window sums of (wB, wxB), sliding
         double zb[C], bb[C];
         {
@@ -457,6 +507,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
             slide_sums<C, IBW0>(u, zb);
             make_halo<C, IBW0>(p2, u, lane, 0.0);
             slide_sums<C, IBW0>(u, bb);
+            tmem_fetch<C>(M.tmem + 6 * C, t_isw); tmem_fetch<C>(M.tmem + 8 * C, t_xb); tmem_fetch<C>(M.tmem + 10 * C, t_isxx);
 #pragma unroll
             for (int s = 0; s < C; s++) {
                 const double mz = zb[s];
@@ -553,21 +604,29 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
 // Kernel: one CTA = one work item (object, chunk of frequencies); its WARPS_PER_CTA warps split the
 // chunk into contiguous runs.  P values are staged in registers and written 32 at a time.
 // ------------------------------------------------------------------------------------------------
-template <int C>
+template <int C, bool GV>
 inline size_t warp_smem_bytes()
 {
     // object arrays (3 x 32C doubles) + per warp: 3 pair-prefix arrays + 256 B permutation bytes
-    return (size_t)3 * 32 * C * 8 + (size_t)WARPS_PER_CTA * ((size_t)3 * C * WROW * 16 + 256);
+    return (size_t)3 * 32 * C * 8 + (size_t)WarpCfg<C, GV>::WPC * ((size_t)3 * C * WROW * 16 + 256);
 }
 
 __device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 
 template <int C, int IBW0, bool GV>
-__global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_kernel(const EvalParams p)
+__global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB) warp_kernel(const EvalParams p)
 {
+    constexpr int WPC = WarpCfg<C, GV>::WPC;
+    static_assert(WARPS_PER_CTA % WPC == 0, "chunks are multiples of WARPS_PER_CTA");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double s_best[WARPS_PER_CTA];
-    __shared__ long long s_bestk[WARPS_PER_CTA];
+    __shared__ double s_best[WPC];
+    __shared__ long long s_bestk[WPC];
+    __shared__ uint32_t s_tmem;
+    // tensor-memory columns: 12C words per warp; warps w and w+4 share a lane quarter
+    constexpr uint32_t TCOLS_WARP = 12 * C;
+    constexpr uint32_t TCOLS_NEED = TCOLS_WARP * ((WPC + 3) / 4);
+    constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
+    static_assert(GV || TCOLS * WarpCfg<C, GV>::MINB <= 512, "tensor memory over-subscribed");
     const int tid = threadIdx.x, lane = tid & 31;
     // warp index through a lane-0 broadcast: the compiler then knows it (and the eval loop's bounds) to be
     // warp-uniform, so the shuffles inside the loop need no WARPSYNC / ENDCOLLECTIVE wrappers
@@ -602,16 +661,29 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_ker
     M.tt = o_tt; M.yc = o_y; M.w = o_w;
     M.E = reinterpret_cast<double2*>(wbase);
     M.perm = wbase + (size_t)3 * C * WROW * 16;
-    for (int j = tid; j < n; j += WARPS_PER_CTA * 32) {
+    M.tmem = 0;
+    if (!GV) {
+        if (warp == 0) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                         :: "r"((uint32_t)__cvta_generic_to_shared(&s_tmem)), "n"(TCOLS) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    }
+    for (int j = tid; j < n; j += WPC * 32) {
         o_tt[j] = p.tt[rec.off + j];
         o_y[j] = p.yc[rec.off + j];
         o_w[j] = p.w[rec.off + j];
     }
     __syncthreads();
+    if (!GV) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        M.tmem = s_tmem + ((uint32_t)(warp & 3) << 21) + (uint32_t)(warp >> 2) * TCOLS_WARP;   // lane 32*(warp%4)
+    }
 
     const int64_t c0 = p.k_begin + (int64_t)ch * p.chunk;
     const int64_t c1 = min(c0 + (int64_t)p.chunk, p.k_end);
-    const int per_warp = p.chunk / WARPS_PER_CTA;          // chunk is a multiple of WARPS_PER_CTA
+    const int per_warp = p.chunk / WPC;                    // chunk is a multiple of WARPS_PER_CTA
     const int64_t k0 = c0 + (int64_t)warp * per_warp;
     const int64_t k1 = min(k0 + (int64_t)per_warp, c1);
     double best = -INFINITY;
@@ -640,9 +712,14 @@ __global__ void __launch_bounds__(WARPS_PER_CTA * 32, (C <= 4 ? 2 : 1)) warp_ker
         }
     }
     if (lane == 0) { s_best[warp] = best; s_bestk[warp] = best_k; }
+    if (!GV) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    if (!GV && warp == 0) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s_tmem), "n"(TCOLS) : "memory");
+    }
     if (tid == 0) {
-        for (int q = 1; q < WARPS_PER_CTA; q++)
+        for (int q = 1; q < WPC; q++)
             if (s_best[q] > best || (s_best[q] == best && s_bestk[q] < best_k)) { best = s_best[q]; best_k = s_bestk[q]; }
         const int64_t slot = (int64_t)ri * p.chunks_total + p.chunk_base + ch;
         p.part_val[slot] = best;
@@ -720,15 +797,15 @@ inline ss_status_t launch_warp_variant(const EvalParams& p, int64_t n_items, cud
 {
     cudaError_t e;
     if (p.mode == 1) {
-        const size_t smem = warp_smem_bytes<C>();
+        const size_t smem = warp_smem_bytes<C, true>();
         e = cudaFuncSetAttribute(warp_kernel<C, IBW0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return SS_ERR_CUDA;
-        warp_kernel<C, IBW0, true><<<(unsigned)n_items, WARPS_PER_CTA * 32, smem, stream>>>(p);
+        warp_kernel<C, IBW0, true><<<(unsigned)n_items, WarpCfg<C, true>::WPC * 32, smem, stream>>>(p);
     } else {
-        const size_t smem = warp_smem_bytes<C>();
+        const size_t smem = warp_smem_bytes<C, false>();
         e = cudaFuncSetAttribute(warp_kernel<C, IBW0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return SS_ERR_CUDA;
-        warp_kernel<C, IBW0, false><<<(unsigned)n_items, WARPS_PER_CTA * 32, smem, stream>>>(p);
+        warp_kernel<C, IBW0, false><<<(unsigned)n_items, WarpCfg<C, false>::WPC * 32, smem, stream>>>(p);
     }
     return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
 }
