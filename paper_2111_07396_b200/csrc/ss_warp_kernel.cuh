@@ -407,21 +407,29 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
             chi2 += w[s] * r * r;
         }
     } else {
-        // ---- CV pass 1
-        double A0[C], A1[C], A2[C], r0[C], r1[C], r2[C];
+        // ---- CV pass 1, one span at a time; each smooth is parked in tensor memory
+        // as soon as it exists (it is needed again only at the interpolation), so are the tweeter
+        // x-moments (needed again by the final smooth) and y (needed again by the statistic)
+        double r0[C], r1[C], r2[C];
         double m_isw[C], m_xb[C], m_g[C];      // midrange x-moments, reused by four more smooths
         int amin = 0x7fffffff;                 // smallest high word of the three LOO denominators
+        {
+            double A0[C];
 #pragma unroll
-        for (int s = 0; s < C; s++) {
-            const double xj = x[s], yj = y[s], wj = w[s];
-            {
-                const double dx = xj - t_xb[s];
+            for (int s = 0; s < C; s++) {
+                const double dx = x[s] - t_xb[s];
                 A0[s] = t_zb[s] + t_b[s] * dx;
-                const double a = 1.0 - wj * (t_isw[s] + dx * dx * t_isxx[s]);
-                r0[s] = fabs(yj - A0[s]) * rcp64(a);
+                const double a = 1.0 - w[s] * (t_isw[s] + dx * dx * t_isxx[s]);
+                r0[s] = fabs(y[s] - A0[s]) * rcp64(a);
                 amin = min(amin, __double2hiint(a));
             }
-            {
+            tmem_park<C>(M.tmem, A0);
+            tmem_park<C>(M.tmem + 6 * C, t_isw); tmem_park<C>(M.tmem + 8 * C, t_xb); tmem_park<C>(M.tmem + 10 * C, t_isxx);
+        }
+        {
+            double A1[C];
+#pragma unroll
+            for (int s = 0; s < C; s++) {
                 const double2 l0 = E01[s1lo[s]], h0 = E01[s1hi[s]], l1 = E23[s1lo[s]], h1 = E23[s1hi[s]];
                 const double lxy = E45[s1lo[s]].x, hxy = E45[s1hi[s]].x;
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
@@ -429,14 +437,19 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
                 const double isw = rcp64(Sw), xb = Swx * isw;
                 const double sxx = Swxx - xb * Swx;
                 const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                const double dx = xj - xb;
+                const double dx = x[s] - xb;
                 m_isw[s] = isw; m_xb[s] = xb; m_g[s] = isxx * dx;
                 A1[s] = Sy * isw + (Sxy - xb * Sy) * m_g[s];
-                const double a = 1.0 - wj * (isw + dx * m_g[s]);
-                r1[s] = fabs(yj - A1[s]) * rcp64(a);
+                const double a = 1.0 - w[s] * (isw + dx * m_g[s]);
+                r1[s] = fabs(y[s] - A1[s]) * rcp64(a);
                 amin = min(amin, __double2hiint(a));
             }
-            {
+            tmem_park<C>(M.tmem + 2 * C, A1);
+        }
+        {
+            double A2[C];
+#pragma unroll
+            for (int s = 0; s < C; s++) {
                 const int lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
                 const int a2 = wst<C>(lo2), b2 = wst<C>(lo2 + K.K2);
                 const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2];
@@ -446,19 +459,18 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
                 const double isw = rcp64(Sw), xb = Swx * isw;
                 const double sxx = Swxx - xb * Swx;
                 const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                const double dx = xj - xb, g = isxx * dx;
+                const double dx = x[s] - xb, g = isxx * dx;
                 A2[s] = Sy * isw + (Sxy - xb * Sy) * g;
-                const double a = 1.0 - wj * (isw + dx * g);
-                r2[s] = fabs(yj - A2[s]) * rcp64(a);
+                const double a = 1.0 - w[s] * (isw + dx * g);
+                r2[s] = fabs(y[s] - A2[s]) * rcp64(a);
                 amin = min(amin, __double2hiint(a));
             }
+            tmem_park<C>(M.tmem + 4 * C, A2);
+            tmem_park<C>(M.tmem + 12 * C, y);
         }
         // a <= 0 (or below the smallest normal): the residual carries (R23) -> generic path.  Padded slots have a ~ 1.
         if (__any_sync(0xffffffffu, amin < 0x00100000)) { defer = true; return 0.0; }
         __syncwarp();      // every lane is done reading the primary prefix arrays
-        // park what is not needed during the four secondary smooths in tensor memory
-        tmem_park<C>(M.tmem, A0); tmem_park<C>(M.tmem + 2 * C, A1); tmem_park<C>(M.tmem + 4 * C, A2);
-        tmem_park<C>(M.tmem + 6 * C, t_isw); tmem_park<C>(M.tmem + 8 * C, t_xb); tmem_park<C>(M.tmem + 10 * C, t_isxx);
 
         // midrange smooth of a register array z through one pair-prefix array
         auto mid_store = [&](const double (&z)[C], double2* Ez) {
@@ -522,10 +534,12 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
             const int sr = K.slot_r, lr = K.lane_r;
             SS_CLAMP(zb) SS_CLAMP(bb)
         }
+        double yy[C];
+        tmem_fetch<C>(M.tmem + 12 * C, yy);
 #pragma unroll
         for (int s = 0; s < C; s++) {
             const double smo = zb[s] + bb[s] * (x[s] - t_xb[s]);
-            const double r = y[s] - smo;
+            const double r = yy[s] - smo;
             chi2 += w[s] * r * r;
         }
     }
@@ -622,8 +636,8 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     __shared__ double s_best[WPC];
     __shared__ long long s_bestk[WPC];
     __shared__ uint32_t s_tmem;
-    // tensor-memory columns: 12C words per warp; warps w and w+4 share a lane quarter
-    constexpr uint32_t TCOLS_WARP = 12 * C;
+    // tensor-memory columns: 14C words per warp; warps w and w+4 share a lane quarter
+    constexpr uint32_t TCOLS_WARP = 14 * C;
     constexpr uint32_t TCOLS_NEED = TCOLS_WARP * ((WPC + 3) / 4);
     constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
     static_assert(GV || TCOLS * WarpCfg<C, GV>::MINB <= 512, "tensor memory over-subscribed");
