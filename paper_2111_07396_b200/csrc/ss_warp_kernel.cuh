@@ -52,30 +52,26 @@ __device__ __forceinline__ double shfl_down_d(double v, int d) { return __shfl_d
 template <int C>
 __device__ __forceinline__ int wst(int e) { return (e % C) * WROW + e / C; }
 
-// One Kogge-Stone step on a double: inc += (value of lane - d) for lanes >= d.  The shuffle's own
-// "source in range" predicate guards the add, so the step is 2 SHFL + 1 predicated DADD (a C-level
-// `if (lane >= d)` compiles to an unconditional add plus two FSEL).
-__device__ __forceinline__ void scan_step(double& inc, int d)
+// Kogge-Stone masks: mk[i] = 1.0 for lanes >= 2^i, else 0.0 (loop-invariant, 5 register pairs).  A step
+// is then 2 SHFL + 1 DFMA; a C-level `if (lane >= d)` or a predicated add compiles to DADD + 2 FSEL.
+struct ScanMask { double m[5]; };
+__device__ __forceinline__ ScanMask make_scan_mask(int lane)
 {
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        ".reg .b32 lo, hi, olo, ohi;\n\t"
-        ".reg .f64 o;\n\t"
-        "mov.b64 {lo, hi}, %0;\n\t"
-        "shfl.sync.up.b32 olo|p, lo, %1, 0, 0xffffffff;\n\t"
-        "shfl.sync.up.b32 ohi, hi, %1, 0, 0xffffffff;\n\t"
-        "mov.b64 o, {olo, ohi};\n\t"
-        "@p add.f64 %0, %0, o;\n\t"
-        "}"
-        : "+d"(inc)
-        : "r"(d));
+    ScanMask k;
+#pragma unroll
+    for (int i = 0; i < 5; i++) k.m[i] = lane >= (1 << i) ? 1.0 : 0.0;
+    return k;
+}
+__device__ __forceinline__ void scan_step(double& inc, int i, const ScanMask& mk)
+{
+    inc = fma(shfl_up_d(inc, 1 << i), mk.m[i], inc);
 }
 
 // Warp-wide exclusive prefix sums of two arrays at once (C values per lane, blocked), written
 // interleaved as double2 and transposed: E[wst(j)] = (sum_{i<j} a_i, sum_{i<j} b_i), j = 0..32C.
 template <int C>
-__device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const double (&b)[C], double2* E, int lane)
+__device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const double (&b)[C], double2* E, int lane,
+                                                  const ScanMask& mk)
 {
     double ea[C], eb[C];
     double ra = a[0], rb = b[0];
@@ -84,12 +80,31 @@ __device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const do
     for (int s = 1; s < C; s++) { ea[s] = ra; ra += a[s]; eb[s] = rb; rb += b[s]; }
     double ia = ra, ib = rb;
 #pragma unroll
-    for (int d = 1; d < 32; d <<= 1) { scan_step(ia, d); scan_step(ib, d); }
+    for (int i = 0; i < 5; i++) { scan_step(ia, i, mk); scan_step(ib, i, mk); }
     const double xa = ia - ra, xb = ib - rb;
     E[lane] = make_double2(xa, xb);
 #pragma unroll
     for (int s = 1; s < C; s++) E[s * WROW + lane] = make_double2(xa + ea[s], xb + eb[s]);
     if (lane == 31) E[32] = make_double2(ia, ib);     // E[32*C] lives at row 0, column 32
+}
+
+// One array: E[wst(j)] = sum_{i<j} a_i as plain doubles (row length WROW doubles).
+template <int C>
+__device__ __forceinline__ void single_prefix_store(const double (&a)[C], double* E, int lane, const ScanMask& mk)
+{
+    double ea[C];
+    double ra = a[0];
+    ea[0] = 0.0;
+#pragma unroll
+    for (int s = 1; s < C; s++) { ea[s] = ra; ra += a[s]; }
+    double ia = ra;
+#pragma unroll
+    for (int i = 0; i < 5; i++) scan_step(ia, i, mk);
+    const double xa = ia - ra;
+    E[lane] = xa;
+#pragma unroll
+    for (int s = 1; s < C; s++) E[s * WROW + lane] = xa + ea[s];
+    if (lane == 31) E[32] = ia;
 }
 
 __device__ __forceinline__ void cex32(unsigned& a, unsigned& b)
@@ -141,16 +156,16 @@ __device__ __forceinline__ void warp_sort(unsigned (&key)[S], int lane)
 }
 
 // Halo of one register array: u[t] = element at j = lane*C - IBW0 + t (fill outside 0..32C-1).
-template <int C, int IBW0>
+template <int C, int IBW0, bool FILL = true>
 __device__ __forceinline__ void make_halo(const double (&v)[C], double (&u)[C + 2 * IBW0], int lane, double fill)
 {
     static_assert(IBW0 <= C, "halo reaches one lane to either side");
 #pragma unroll
     for (int t = 0; t < IBW0; t++) {
         double l = shfl_up_d(v[C - IBW0 + t], 1);
-        u[t] = lane == 0 ? fill : l;
+        u[t] = (FILL && lane == 0) ? fill : l;
         double r = shfl_down_d(v[t], 1);
-        u[IBW0 + C + t] = lane == 31 ? fill : r;
+        u[IBW0 + C + t] = (FILL && lane == 31) ? fill : r;
     }
 #pragma unroll
     for (int s = 0; s < C; s++) u[IBW0 + s] = v[s];
@@ -234,6 +249,7 @@ struct WarpMem {
     double2* E;              // per-warp: 3 pair-prefix arrays of C*WROW double2
     unsigned char* perm;     // per-warp: 256 bytes (rank -> index), only when S != C
     uint32_t tmem;           // per-warp tensor-memory base (lane quarter + first column), CV only
+    ScanMask mk;             // Kogge-Stone masks of this lane
 };
 
 // Per-object constants of the eval loop (warp-uniform).
@@ -283,13 +299,19 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         double a[C], b[C], c[C];
 #pragma unroll
         for (int s = 0; s < C; s++) { a[s] = w[s]; b[s] = w[s] * x[s]; }
-        pair_prefix_store<C>(a, b, E01, lane);
+        pair_prefix_store<C>(a, b, E01, lane, M.mk);
 #pragma unroll
         for (int s = 0; s < C; s++) { c[s] = b[s] * x[s]; a[s] = w[s] * y[s]; }
-        pair_prefix_store<C>(c, a, E23, lane);
+        pair_prefix_store<C>(c, a, E23, lane, M.mk);
 #pragma unroll
-        for (int s = 0; s < C; s++) { b[s] = b[s] * y[s]; c[s] = GV ? a[s] * y[s] : 0.0; }
-        pair_prefix_store<C>(b, c, E45, lane);
+        for (int s = 0; s < C; s++) b[s] = b[s] * y[s];
+        if (GV) {
+#pragma unroll
+            for (int s = 0; s < C; s++) c[s] = a[s] * y[s];
+            pair_prefix_store<C>(b, c, E45, lane, M.mk);
+        } else {
+            single_prefix_store<C>(b, reinterpret_cast<double*>(E45), lane, M.mk);   // CV: wxy only
+        }
     }
     __syncwarp();
 
@@ -297,9 +319,10 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
     double t_isw[C], t_xb[C], t_isxx[C], t_zb[C], t_b[C], t_g[C];
     {
         double ux[H], uw[H], uy[H];
-        make_halo<C, IBW0>(x, ux, lane, 0.0);
+        // only the weights need the zero fill outside 0..32C-1: x and y there are finite and multiply w = 0
+        make_halo<C, IBW0, false>(x, ux, lane, 0.0);
         make_halo<C, IBW0>(w, uw, lane, 0.0);
-        make_halo<C, IBW0>(y, uy, lane, 0.0);
+        make_halo<C, IBW0, false>(y, uy, lane, 0.0);
         const double c0 = x[0];
         double m0[C], m1[C], m2[C], mz[C], m1z[C], mzz[C];
         slide_sums<C, IBW0>(uw, m0);
@@ -412,6 +435,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         // x-moments (needed again by the final smooth) and y (needed again by the statistic)
         double r0[C], r1[C], r2[C];
         double m_isw[C], m_xb[C], m_g[C];      // midrange x-moments, reused by four more smooths
+        const double* E4 = reinterpret_cast<const double*>(E45);
         int amin = 0x7fffffff;                 // smallest high word of the three LOO denominators
         {
             double A0[C];
@@ -431,7 +455,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
 #pragma unroll
             for (int s = 0; s < C; s++) {
                 const double2 l0 = E01[s1lo[s]], h0 = E01[s1hi[s]], l1 = E23[s1lo[s]], h1 = E23[s1hi[s]];
-                const double lxy = E45[s1lo[s]].x, hxy = E45[s1hi[s]].x;
+                const double lxy = E4[s1lo[s]], hxy = E4[s1hi[s]];
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                 const double Sxy = hxy - lxy;
                 const double isw = rcp64(Sw), xb = Swx * isw;
@@ -453,7 +477,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
                 const int lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
                 const int a2 = wst<C>(lo2), b2 = wst<C>(lo2 + K.K2);
                 const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2];
-                const double lxy = E45[a2].x, hxy = E45[b2].x;
+                const double lxy = E4[a2], hxy = E4[b2];
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                 const double Sxy = hxy - lxy;
                 const double isw = rcp64(Sw), xb = Swx * isw;
@@ -477,7 +501,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
             double a[C], b[C];
 #pragma unroll
             for (int s = 0; s < C; s++) { a[s] = w[s] * z[s]; b[s] = a[s] * x[s]; }
-            pair_prefix_store<C>(a, b, Ez, lane);
+            pair_prefix_store<C>(a, b, Ez, lane, M.mk);
         };
         auto mid_load = [&](const double2* Ez, double (&out)[C]) {
 #pragma unroll
@@ -676,6 +700,7 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     M.E = reinterpret_cast<double2*>(wbase);
     M.perm = wbase + (size_t)3 * C * WROW * 16;
     M.tmem = 0;
+    M.mk = make_scan_mask(lane);
     if (!GV) {
         if (warp == 0) {
             asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
