@@ -69,18 +69,16 @@ __device__ __forceinline__ double fold_phase(double tt, double f)
     return __dsub_rn(p, floor(p));
 }
 
-// 1/x to about 1 ulp: MUFU.RCP64H seed (relative error 2^-20, measured 9.9e-7 on B200) and two
-// Newton-Raphson steps on the fp64 pipe (4 DFMA; measured: bit-identical to 1.0/x on 2^20 samples
-// spanning 41 binades).  x must be a normal, finite, non-zero double (the callers guard that).
+// 1/x to about 1 ulp: MUFU.RCP64H seed (relative error 2^-20, measured 9.9e-7 on B200) and one
+// third-order correction on the fp64 pipe (3 DFMA).  x must be a normal, finite, non-zero double (the callers guard that).
 // IEEE division costs ~3x as many fp64 instructions plus a slow-path branch.
 __device__ __forceinline__ double rcp64(double x)
 {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
+    const double e = fma(-x, r, 1.0);     // |e| <= 2^-20
+    const double t = fma(e, e, e);        // e + e^2: r*(1 + e + e^2) leaves a relative error of e^3 = 2^-60
+    return fma(r, t, r);
 }
 
 // x-moments of one window: reused by every smooth over the same window.

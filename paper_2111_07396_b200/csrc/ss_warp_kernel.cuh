@@ -234,10 +234,17 @@ __device__ __forceinline__ void tmem_fetch(uint32_t taddr, double (&v)[N])
     for (int s = 0; s < N; s++)
         asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];"
                      : "=r"(lo[s]), "=r"(hi[s]) : "r"(taddr + 2 * s) : "memory");
-    // the loaded registers are valid only after the wait: tie them to it
-#pragma unroll
-    for (int s = 0; s < N; s++)
-        asm volatile("tcgen05.wait::ld.sync.aligned;" : "+r"(lo[s]), "+r"(hi[s]) :: "memory");
+    // the loaded registers are valid only after the wait: tie them to it (one wait per fetch)
+    static_assert(N >= 2 && N <= 8, "tmem_fetch: 2..8 doubles");
+#define SS_T(i) "+r"(lo[i < N ? i : 0]), "+r"(hi[i < N ? i : 0])
+    if (N == 2) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1) :: "memory");
+    else if (N == 3) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2) :: "memory");
+    else if (N == 4) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3) :: "memory");
+    else if (N == 5) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4) :: "memory");
+    else if (N == 6) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5) :: "memory");
+    else if (N == 7) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6) :: "memory");
+    else asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6), SS_T(7) :: "memory");
+#undef SS_T
 #pragma unroll
     for (int s = 0; s < N; s++) v[s] = __hiloint2double(hi[s], lo[s]);
 }
@@ -266,8 +273,7 @@ struct EvalConst {
 // Listing 1 lines 63-77 with the loop-invariant tests hoisted.
 __device__ __forceinline__ double pick_span_w(double v0, double v1, double v2, const EvalConst& K)
 {
-    double resmin = v0, sp = SPAN0;
-    if (!(v0 < 1.e20)) { resmin = 1.e20; sp = 0.0; }
+    double resmin = v0, sp = SPAN0;      // v0 < 1e20 always (R27): the listing's first test is dropped
     if (v1 < resmin) { resmin = v1; sp = SPAN1; }
     if (v2 < resmin) { resmin = v2; sp = SPAN2; }
     if (K.bass != 0 && resmin < v2 && resmin > 0.0) {
