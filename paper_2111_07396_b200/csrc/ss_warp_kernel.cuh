@@ -248,6 +248,32 @@ __device__ __forceinline__ void tmem_fetch(uint32_t taddr, double (&v)[N])
 #pragma unroll
     for (int s = 0; s < N; s++) v[s] = __hiloint2double(hi[s], lo[s]);
 }
+// 32-bit words (the loop-invariant window indices)
+template <int N>
+__device__ __forceinline__ void tmem_park_words(uint32_t taddr, const int (&v)[N])
+{
+#pragma unroll
+    for (int s = 0; s < N; s++)
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" :: "r"(taddr + s), "r"(v[s]) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void tmem_fetch_words(uint32_t taddr, int (&v)[N])
+{
+    static_assert(N >= 2 && N <= 16 && N % 2 == 0, "tmem_fetch_words: 2..16 words, even");
+#pragma unroll
+    for (int s = 0; s < N; s++)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v[s]) : "r"(taddr + s) : "memory");
+#define SS_T(i) "+r"(v[2 * (i) < N ? 2 * (i) : 0]), "+r"(v[2 * (i) + 1 < N ? 2 * (i) + 1 : 1])
+    if (N == 2) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0) :: "memory");
+    else if (N == 4) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1) :: "memory");
+    else if (N == 6) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2) :: "memory");
+    else if (N == 8) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3) :: "memory");
+    else if (N == 10) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4) :: "memory");
+    else if (N == 12) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5) :: "memory");
+    else if (N == 14) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6) :: "memory");
+    else asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6), SS_T(7) :: "memory");
+#undef SS_T
+}
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // Per-warp view of the shared memory.
@@ -375,7 +401,8 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         const int sr = K.slot_r, lr = K.lane_r;
 #define SS_CLAMP(arr)                                                                     \
         {                                                                                 \
-            const double vl = shfl_d(arr[LS], LL);                                        \
+            /* IBW0 < C: the left owner is a slot of lane 0 itself, no shuffle */         \
+            const double vl = LL == 0 ? arr[LS] : shfl_d(arr[LS], LL);                    \
             const double vr = bcast_slot<C>(arr, sr, lr);                                 \
             _Pragma("unroll") for (int s = 0; s < C; s++) {                               \
                 const int j = lane * C + s;                                               \
@@ -387,25 +414,23 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         if (GV) SS_CLAMP(t_g)
     }
 
-    // ---- window indices of the midrange span (transposed storage)
-    int s1lo[C], s1hi[C];
-#pragma unroll
-    for (int s = 0; s < C; s++) {
-        const int lo = window_lo(lane * C + s, K.ibw1, K.K1, n);
-        s1lo[s] = wst<C>(lo); s1hi[s] = wst<C>(lo + K.K1);
-    }
-
+    // window indices (transposed storage) are loop-invariant: computed once per CTA, parked in tensor
+    // memory at columns [14C, 16C) (midrange lo, hi) and [16C, 18C) (woofer lo, hi)
+    constexpr uint32_t TW1 = GV ? 0 : 14 * C, TW2 = TW1 + 2 * C;   // GV parks nothing else
     double chi2 = 0.0;
     if (GV) {
         // ---- O6: scores, pick, interpolate
+        int w1[2 * C], w2[2 * C];
+        tmem_fetch_words<2 * C>(M.tmem + TW1, w1);
+        tmem_fetch_words<2 * C>(M.tmem + TW2, w2);
 #pragma unroll
         for (int s = 0; s < C; s++) {
             const double xj = x[s];
             const double A0 = t_zb[s] + t_b[s] * (xj - t_xb[s]);
             double A1, A2, G1, G2;
             {
-                const double2 l0 = E01[s1lo[s]], h0 = E01[s1hi[s]], l1 = E23[s1lo[s]], h1 = E23[s1hi[s]];
-                const double2 l2 = E45[s1lo[s]], h2 = E45[s1hi[s]];
+                const double2 l0 = E01[w1[s]], h0 = E01[w1[C + s]], l1 = E23[w1[s]], h1 = E23[w1[C + s]];
+                const double2 l2 = E45[w1[s]], h2 = E45[w1[C + s]];
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                 const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
                 const double isw = rcp64(Sw), xb = Swx * isw;
@@ -417,8 +442,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
                 G1 = sqrt64(rss * isw) * (isxx != 0.0 ? K.gk1[1] : K.gk1[0]);
             }
             {
-                const int lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
-                const int a2 = wst<C>(lo2), b2 = wst<C>(lo2 + K.K2);
+                const int a2 = w2[s], b2 = w2[C + s];
                 const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2], l2 = E45[a2], h2 = E45[b2];
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                 const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
@@ -458,10 +482,12 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         }
         {
             double A1[C];
+            int w1[2 * C];
+            tmem_fetch_words<2 * C>(M.tmem + TW1, w1);
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double2 l0 = E01[s1lo[s]], h0 = E01[s1hi[s]], l1 = E23[s1lo[s]], h1 = E23[s1hi[s]];
-                const double lxy = E4[s1lo[s]], hxy = E4[s1hi[s]];
+                const double2 l0 = E01[w1[s]], h0 = E01[w1[C + s]], l1 = E23[w1[s]], h1 = E23[w1[C + s]];
+                const double lxy = E4[w1[s]], hxy = E4[w1[C + s]];
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                 const double Sxy = hxy - lxy;
                 const double isw = rcp64(Sw), xb = Swx * isw;
@@ -478,10 +504,11 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         }
         {
             double A2[C];
+            int w2[2 * C];
+            tmem_fetch_words<2 * C>(M.tmem + TW2, w2);
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const int lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
-                const int a2 = wst<C>(lo2), b2 = wst<C>(lo2 + K.K2);
+                const int a2 = w2[s], b2 = w2[C + s];
                 const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2];
                 const double lxy = E4[a2], hxy = E4[b2];
                 const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
@@ -510,9 +537,11 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
             pair_prefix_store<C>(a, b, Ez, lane, M.mk);
         };
         auto mid_load = [&](const double2* Ez, double (&out)[C]) {
+            int w1[2 * C];
+            tmem_fetch_words<2 * C>(M.tmem + TW1, w1);
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double2 l = Ez[s1lo[s]], h = Ez[s1hi[s]];
+                const double2 l = Ez[w1[s]], h = Ez[w1[C + s]];
                 const double Sz = h.x - l.x, Sxz = h.y - l.y;
                 out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
             }
@@ -666,11 +695,11 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     __shared__ double s_best[WPC];
     __shared__ long long s_bestk[WPC];
     __shared__ uint32_t s_tmem;
-    // tensor-memory columns: 14C words per warp; warps w and w+4 share a lane quarter
-    constexpr uint32_t TCOLS_WARP = 14 * C;
+    // tensor-memory columns: 18C words per warp (14C of parked doubles, 4C window indices); warps w and w+4 share a lane quarter
+    constexpr uint32_t TCOLS_WARP = GV ? 4 * C : 18 * C;
     constexpr uint32_t TCOLS_NEED = TCOLS_WARP * ((WPC + 3) / 4);
     constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
-    static_assert(GV || TCOLS * WarpCfg<C, GV>::MINB <= 512, "tensor memory over-subscribed");
+    static_assert(TCOLS * WarpCfg<C, GV>::MINB <= 512, "tensor memory over-subscribed");
     const int tid = threadIdx.x, lane = tid & 31;
     // warp index through a lane-0 broadcast: the compiler then knows it (and the eval loop's bounds) to be
     // warp-uniform, so the shuffles inside the loop need no WARPSYNC / ENDCOLLECTIVE wrappers
@@ -707,7 +736,7 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     M.perm = wbase + (size_t)3 * C * WROW * 16;
     M.tmem = 0;
     M.mk = make_scan_mask(lane);
-    if (!GV) {
+    {
         if (warp == 0) {
             asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
                          :: "r"((uint32_t)__cvta_generic_to_shared(&s_tmem)), "n"(TCOLS) : "memory");
@@ -721,9 +750,19 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
         o_w[j] = p.w[rec.off + j];
     }
     __syncthreads();
-    if (!GV) {
+    {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         M.tmem = s_tmem + ((uint32_t)(warp & 3) << 21) + (uint32_t)(warp >> 2) * TCOLS_WARP;   // lane 32*(warp%4)
+        int w1[2 * C], w2[2 * C];
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            const int lo1 = window_lo(lane * C + s, K.ibw1, K.K1, n), lo2 = window_lo(lane * C + s, K.ibw2, K.K2, n);
+            w1[s] = wst<C>(lo1); w1[C + s] = wst<C>(lo1 + K.K1);
+            w2[s] = wst<C>(lo2); w2[C + s] = wst<C>(lo2 + K.K2);
+        }
+        tmem_park_words<2 * C>(M.tmem + (GV ? 0 : 14 * C), w1);
+        tmem_park_words<2 * C>(M.tmem + (GV ? 2 * C : 16 * C), w2);
+        tmem_wait_st();
     }
 
     const int64_t c0 = p.k_begin + (int64_t)ch * p.chunk;
@@ -757,9 +796,9 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
         }
     }
     if (lane == 0) { s_best[warp] = best; s_bestk[warp] = best_k; }
-    if (!GV) asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
-    if (!GV && warp == 0) {
+    if (warp == 0) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s_tmem), "n"(TCOLS) : "memory");
     }
