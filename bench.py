@@ -120,7 +120,23 @@ def dist_env():
 
 
 def make_catalog(args, rank):
+    """Replicas only: rank r times its own catalog of config 3's shape, seed 2 + r."""
     return ss_inputs.config3(seed=2 + rank, n_objects=args.objects, n_freq=args.freqs)
+
+
+def max_over_ranks(x: float, dist=None, device=None) -> float:
+    """The slowest rank's figure (the only collective of the bench: all-reduce MAX of one double)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_throughput(world: int, units_per_rank_step: int, steps: int, elapsed_ms_max: float) -> float:
+    """Whole-job units/s: every rank processed units_per_rank_step per step in the slowest rank's time."""
+    return world * units_per_rank_step * steps / (elapsed_ms_max * 1e-3)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -232,13 +248,9 @@ def run_ours(args):
     ev1.record(stream)
     barrier()
     clocks = sampler.stop() if rank == 0 else None
-    elapsed_ms = ev0.elapsed_time(ev1)
-    if use_dist:
-        tmax = torch.tensor([elapsed_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(tmax.item())
+    elapsed_ms = max_over_ranks(ev0.elapsed_time(ev1), dist if use_dist else None, dev)
     ms_per_step = elapsed_ms / args.steps
-    value = world * evals_per_step * args.steps / (elapsed_ms * 1e-3)
+    value = job_throughput(world, evals_per_step, args.steps, elapsed_ms)
     best_idx_checksum = int(bi.sum().item())
 
     # the other mode, same catalog, same launch configuration (reported, not the headline)
@@ -269,12 +281,8 @@ def run_ours(args):
         for _ in range(n_e2e):
             estep()
         barrier()
-        dt = time.perf_counter() - t0
-        if use_dist:
-            tm = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            dt = float(tm.item())
-        e2e = {"value": world * evals_per_step * n_e2e / dt, "unit": UNIT,
+        dt = max_over_ranks(time.perf_counter() - t0, dist if use_dist else None, dev)
+        e2e = {"value": job_throughput(world, evals_per_step, n_e2e, dt * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": int(3 * 8 * cat.n_points + 8 * (n_obj + 1)),
                "d2h_bytes_per_step": int(8 * n_obj * n_freq + 16 * n_obj),
                "api": "ss_periodogram_host (pinned host buffers, tiled D2H overlapped with kernels)"}

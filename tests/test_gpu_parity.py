@@ -299,3 +299,56 @@ def test_device_entry_point_matches_host_entry_point(ss, mode):
         ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg3, None, None)
     s.synchronize()
     assert torch.equal(pg, pg3)
+
+
+# ------------------------------------------------------------------ full size, bench.py's launch configuration
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config3_full_size_sampled(ss, mode):
+    """Config 3 at BASELINE.json's full size (10,000 objects x 50,000 frequencies, 4 GB of output), launched
+    exactly as bench.py launches it (device pointers, default options).  Checked on sampled outputs the
+    oracle computes one by one: 400 random (object, k) evals plus four whole rows (shortest, longest and
+    two mid-size objects) with their best-frequency index."""
+    import torch
+    cat = ss_inputs.config3()
+    assert cat.n_objects == 10000 and cat.n_freq == 50000
+    dev = torch.device("cuda")
+    t = torch.as_tensor(cat.times, device=dev); y = torch.as_tensor(cat.mags, device=dev)
+    e = torch.as_tensor(cat.errs, device=dev); off = torch.as_tensor(cat.offsets, device=dev)
+    pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev)
+    bf = torch.empty(cat.n_objects, dtype=torch.float64, device=dev)
+    bi = torch.empty(cat.n_objects, dtype=torch.int64, device=dev)
+    ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, bf, bi)
+    torch.cuda.synchronize()
+    assert ss.last_launch_count() > 0
+    # properties that hold at any size
+    assert bool(torch.isfinite(pg).all()) and float(pg.max()) <= 1.0 + 1e-12
+    rowmax, rowarg = pg.max(dim=1)
+    assert torch.equal(rowarg, bi)                      # first maximum of every row (torch.max returns the first)
+    k_t = bi.to(torch.float64)
+    assert torch.equal(bf, cat.f_min + k_t * ((cat.f_max - cat.f_min) / cat.n_freq))
+    # sampled evals
+    rng = np.random.default_rng(12345)
+    objs = rng.integers(0, cat.n_objects, size=400); ks = rng.integers(0, cat.n_freq, size=400)
+    got = pg[torch.as_tensor(objs, device=dev), torch.as_tensor(ks, device=dev)].cpu().numpy()
+    ambiguous = 0
+    for o, k, g in zip(objs, ks, got):
+        tt, yy, ee = cat.obj(int(o))
+        r = oracle.eval_one(tt, yy, ee, oracle.freq(cat.f_min, cat.f_max, cat.n_freq, int(k)), mode=mode,
+                            variant=oracle.DEFINITION, alt_threshold=1e-7)
+        if abs(g - r["P"]) <= _tol(r["P"]):
+            continue
+        assert r["margin"] < 1e-9 and abs(g - r["P_alt"]) <= _tol(r["P_alt"]), (o, k, g, r["P"], r["margin"])
+        ambiguous += 1
+    assert ambiguous <= 2
+    # whole rows
+    ns = np.diff(cat.offsets)
+    rows = [int(np.argmin(ns)), int(np.argmax(ns)), 1234, 7777]
+    sub = cat.subset(rows)
+    ref, _, _ = oracle.periodogram(sub.times, sub.mags, sub.errs, sub.offsets, sub.f_min, sub.f_max, sub.n_freq,
+                                   mode=mode, variant=oracle.FAST)
+    got_rows = pg[torch.as_tensor(rows, device=dev)].cpu().numpy()
+    check_parity(sub, got_rows, ref, mode, max_ambiguous=4, label="cfg3-full")
+    check_best(ref, bi[torch.as_tensor(rows, device=dev)].cpu().numpy(),
+               bf[torch.as_tensor(rows, device=dev)].cpu().numpy(), sub)
+    del pg
+    torch.cuda.empty_cache()
