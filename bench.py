@@ -35,6 +35,9 @@ UNIT = "evals/s"
 # counts an FMA as 2.
 SLOTS_PER_POINT_EVAL = {"cv": 213.0, "gv": 165.0}
 FLOP_PER_POINT_EVAL = {m: 2.0 * s for m, s in SLOTS_PER_POINT_EVAL.items()}
+# Algorithmic on-chip traffic per point-eval: scan arrays written once + window-end
+# reads, 8 B each: 15 + 50 (CV), 6 + 30 (GV) -- the second, co-limiting roofline (shared-memory pipe).
+SMEM_BYTES_PER_POINT_EVAL = {"cv": 520.0, "gv": 288.0}
 FP64_LANES_PER_SM = 64          # B200 fp64 pipe: 64 FMA lanes per SM per clock
 N_SM = 148
 
@@ -306,6 +309,11 @@ def run_ours(args):
                 "flop_per_point_eval": FLOP_PER_POINT_EVAL[args.mode],
                 "point_evals_per_launch": k_units, "kernel_ms_per_launch": k_ms,
                 "kernel_share_of_step": kernel_ms / elapsed_ms,
+                "smem": {"achieved": SMEM_BYTES_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / 1e12,
+                         "peak": smem_meas / 1e12, "unit": "TB/s",
+                         "frac": SMEM_BYTES_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / smem_meas,
+                         "note": "co-limiting roofline: algorithmic shared-memory bytes (SURVEY 8(d)) vs the "
+                                 "shared-memory read microbenchmark measured in this run"},
                 "hbm_gbs_algorithmic": 8.0 * evals_per_step / (ms_per_step * 1e-3) / 1e9}
     cpu = None
     if not args.no_cpu:
