@@ -220,20 +220,46 @@ __device__ __forceinline__ void tmem_st2(uint32_t taddr, double v)
     asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};"
                  :: "r"(taddr), "r"(__double2loint(v)), "r"(__double2hiint(v)) : "memory");
 }
-template <int N>
+#define SS_LOHI(v, i) "r"(__double2loint(v[i])), "r"(__double2hiint(v[i]))
+template <int N, int S0 = 0>
 __device__ __forceinline__ void tmem_park(uint32_t taddr, const double (&v)[N])
 {
-#pragma unroll
-    for (int s = 0; s < N; s++) tmem_st2(taddr + 2 * s, v[s]);
+    // widest power-of-two run first: x8 (4 doubles), x4 (2), x2 (1)
+    if constexpr (N - S0 >= 4) {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+                     :: "r"(taddr + 2 * S0), SS_LOHI(v, S0), SS_LOHI(v, S0 + 1), SS_LOHI(v, S0 + 2), SS_LOHI(v, S0 + 3) : "memory");
+        tmem_park<N, S0 + 4>(taddr, v);
+    } else if constexpr (N - S0 >= 2) {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                     :: "r"(taddr + 2 * S0), SS_LOHI(v, S0), SS_LOHI(v, S0 + 1) : "memory");
+        tmem_park<N, S0 + 2>(taddr, v);
+    } else if constexpr (N - S0 == 1) {
+        tmem_st2(taddr + 2 * S0, v[S0]);
+    }
 }
+#undef SS_LOHI
+#define SS_O(i) "=r"(lo[i]), "=r"(hi[i])
+template <int N, int S0 = 0>
+__device__ __forceinline__ void tmem_issue_ld(uint32_t taddr, int (&lo)[N], int (&hi)[N])
+{
+    if constexpr (N - S0 >= 4) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : SS_O(S0), SS_O(S0 + 1), SS_O(S0 + 2), SS_O(S0 + 3) : "r"(taddr + 2 * S0) : "memory");
+        tmem_issue_ld<N, S0 + 4>(taddr, lo, hi);
+    } else if constexpr (N - S0 >= 2) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : SS_O(S0), SS_O(S0 + 1) : "r"(taddr + 2 * S0) : "memory");
+        tmem_issue_ld<N, S0 + 2>(taddr, lo, hi);
+    } else if constexpr (N - S0 == 1) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : SS_O(S0) : "r"(taddr + 2 * S0) : "memory");
+    }
+}
+#undef SS_O
 template <int N>
 __device__ __forceinline__ void tmem_fetch(uint32_t taddr, double (&v)[N])
 {
     int lo[N], hi[N];
-#pragma unroll
-    for (int s = 0; s < N; s++)
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];"
-                     : "=r"(lo[s]), "=r"(hi[s]) : "r"(taddr + 2 * s) : "memory");
+    tmem_issue_ld<N>(taddr, lo, hi);
     // the loaded registers are valid only after the wait: tie them to it (one wait per fetch)
     static_assert(N >= 2 && N <= 8, "tmem_fetch: 2..8 doubles");
 #define SS_T(i) "+r"(lo[i < N ? i : 0]), "+r"(hi[i < N ? i : 0])
@@ -256,13 +282,29 @@ __device__ __forceinline__ void tmem_park_words(uint32_t taddr, const int (&v)[N
     for (int s = 0; s < N; s++)
         asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" :: "r"(taddr + s), "r"(v[s]) : "memory");
 }
+template <int N, int S0 = 0>
+__device__ __forceinline__ void tmem_issue_ld_words(uint32_t taddr, int (&v)[N])
+{
+    if constexpr (N - S0 >= 8) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : "=r"(v[S0]), "=r"(v[S0 + 1]), "=r"(v[S0 + 2]), "=r"(v[S0 + 3]), "=r"(v[S0 + 4]), "=r"(v[S0 + 5]),
+                       "=r"(v[S0 + 6]), "=r"(v[S0 + 7]) : "r"(taddr + S0) : "memory");
+        tmem_issue_ld_words<N, S0 + 8>(taddr, v);
+    } else if constexpr (N - S0 >= 4) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(v[S0]), "=r"(v[S0 + 1]), "=r"(v[S0 + 2]), "=r"(v[S0 + 3]) : "r"(taddr + S0) : "memory");
+        tmem_issue_ld_words<N, S0 + 4>(taddr, v);
+    } else if constexpr (N - S0 >= 2) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];"
+                     : "=r"(v[S0]), "=r"(v[S0 + 1]) : "r"(taddr + S0) : "memory");
+        tmem_issue_ld_words<N, S0 + 2>(taddr, v);
+    }
+}
 template <int N>
 __device__ __forceinline__ void tmem_fetch_words(uint32_t taddr, int (&v)[N])
 {
     static_assert(N >= 2 && N <= 16 && N % 2 == 0, "tmem_fetch_words: 2..16 words, even");
-#pragma unroll
-    for (int s = 0; s < N; s++)
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x1.b32 {%0}, [%1];" : "=r"(v[s]) : "r"(taddr + s) : "memory");
+    tmem_issue_ld_words<N>(taddr, v);
 #define SS_T(i) "+r"(v[2 * (i) < N ? 2 * (i) : 0]), "+r"(v[2 * (i) + 1 < N ? 2 * (i) + 1 : 1])
     if (N == 2) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0) :: "memory");
     else if (N == 4) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1) :: "memory");
