@@ -56,13 +56,17 @@ __device__ __forceinline__ void block_scan(int n, F vals, double* const (&E)[NA]
         __syncthreads();
 #pragma unroll
         for (int a = 0; a < NA; a++) {
-            double woff = 0.0, tot = 0.0;
+            // every warp scans the NW warp sums itself (lane q holds warp q's sum): no second barrier
+            static_assert(NW <= 32, "one lane per warp sum");
+            const double mine = lane < NW ? wsum[a][lane] : 0.0;
+            double sc = mine;
 #pragma unroll
-            for (int q = 0; q < NW; q++) {
-                double s = wsum[a][q];
-                if (q < warp) woff += s;
-                tot += s;
+            for (int d = 1; d < NW; d <<= 1) {
+                double o = __shfl_up_sync(0xffffffffu, sc, d);
+                if (lane >= d) sc += o;
             }
+            const double woff = __shfl_sync(0xffffffffu, sc - mine, warp);
+            const double tot = __shfl_sync(0xffffffffu, sc, NW - 1);
             if (j < n) E[a][j] = carry[a] + woff + (inc[a] - v[a]);
             carry[a] += tot;
         }
@@ -163,18 +167,19 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
     int np2 = 1;
     while (np2 < n) np2 <<= 1;
     const int half = np2 >> 1;
-    for (int k = 2; (k >> 1) < n; k <<= 1) {
-        const int hk = k >> 1;
+    for (int lk = 1; (1 << (lk - 1)) < n; lk++) {
+        const int k = 1 << lk, hk = k >> 1;           // strides are powers of two: shifts, no division
         for (int t = tid; t < half; t += T) {
-            int blk = t / hk, o = t - blk * hk;
-            int a = blk * k + o, b = blk * k + k - 1 - o;
+            int blk = t >> (lk - 1), o = t & (hk - 1);
+            int a = (blk << lk) + o, b = (blk << lk) + k - 1 - o;
             if (b < n) cex(key, idx, a, b);
         }
         __syncthreads();
-        for (int jj = k >> 2; jj >= 1; jj >>= 1) {
+        for (int lj = lk - 2; lj >= 0; lj--) {
+            const int jj = 1 << lj;
             for (int t = tid; t < half; t += T) {
-                int blk = t / jj, o = t - blk * jj;
-                int a = blk * 2 * jj + o, b = a + jj;
+                int blk = t >> lj, o = t & (jj - 1);
+                int a = (blk << (lj + 1)) + o, b = a + jj;
                 if (b < n) cex(key, idx, a, b);
             }
             __syncthreads();
