@@ -134,6 +134,137 @@ __device__ __forceinline__ void cex(unsigned long long* key, unsigned int* idx, 
     }
 }
 
+// ---- fast sort: packed (phase bits | index) 64-bit keys in registers --------------------------------
+// S keys per thread, blocked (position = tid*S + s).  Warp-local phases run on registers and shuffles,
+// only the log2(NW)*(log2(NW)+1)/2 cross-warp steps go through shared memory.  The low IDX_BITS mantissa
+// bits of the phase give way to the index, so the order is exact unless two phases agree in all the
+// bits kept and disagree below: the caller checks the gathered phases and falls back to the exact
+// network then.
+constexpr int FAST_IDX_BITS = 12;
+constexpr unsigned long long FAST_IDX_MASK = (1ull << FAST_IDX_BITS) - 1ull;
+
+__device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int m)
+{
+    return __shfl_xor_sync(0xffffffffu, v, m);
+}
+
+// the halving steps of one merge phase inside a warp: lane strides 16..1, then register strides S/2..1
+template <int S>
+__device__ __forceinline__ void merge_tail64(unsigned long long (&key)[S], int lane, int first_lane_stride)
+{
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) {
+        if (m > first_lane_stride) continue;
+        const bool lower = (lane & m) == 0;
+#pragma unroll
+        for (int s = 0; s < S; s++) {
+            const unsigned long long o = shfl_xor_u64(key[s], m);
+            key[s] = lower ? min(key[s], o) : max(key[s], o);
+        }
+    }
+#pragma unroll
+    for (int j = S >> 1; j >= 1; j >>= 1) {
+#pragma unroll
+        for (int s = 0; s < S; s++)
+            if ((s & j) == 0) {
+                const unsigned long long lo = min(key[s], key[s + j]), hi = max(key[s], key[s + j]);
+                key[s] = lo; key[s + j] = hi;
+            }
+    }
+}
+
+// sorts the 32*S keys of each warp ascending (blocked within the warp: position = lane*S + s)
+template <int S>
+__device__ __forceinline__ void warp_sort64(unsigned long long (&key)[S], int lane)
+{
+#pragma unroll
+    for (int k = 2; k <= 32 * S; k <<= 1) {
+        if (k <= S) {
+#pragma unroll
+            for (int s = 0; s < S; s++) {
+                const int t = s ^ (k - 1);
+                if (t > s) {
+                    const unsigned long long lo = min(key[s], key[t]), hi = max(key[s], key[t]);
+                    key[s] = lo; key[t] = hi;
+                }
+            }
+#pragma unroll
+            for (int j = k >> 2; j >= 1; j >>= 1) {
+#pragma unroll
+                for (int s = 0; s < S; s++)
+                    if ((s & j) == 0) {
+                        const unsigned long long lo = min(key[s], key[s + j]), hi = max(key[s], key[s + j]);
+                        key[s] = lo; key[s + j] = hi;
+                    }
+            }
+        } else {
+            const int m = k / S - 1;               // lane mask of the mirror step
+            const bool lower = (lane & (k / S / 2)) == 0;
+            unsigned long long other[S];
+#pragma unroll
+            for (int s = 0; s < S; s++) other[s] = shfl_xor_u64(key[S - 1 - s], m);
+#pragma unroll
+            for (int s = 0; s < S; s++) key[s] = lower ? min(key[s], other[s]) : max(key[s], other[s]);
+            merge_tail64<S>(key, lane, k / S / 4);
+        }
+    }
+}
+
+// Whole-CTA sort; writes the sorted permutation idx[0..n).  kbuf: T*S words of exchange space.
+template <int T, int S>
+__device__ __forceinline__ void block_sort_fast(int n, const double* tt, double f, unsigned long long* kbuf,
+                                                unsigned int* idx)
+{
+    constexpr int NW = T / 32;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    unsigned long long key[S];
+#pragma unroll
+    for (int s = 0; s < S; s++) {
+        const int i = tid + T * s;
+        key[s] = ~0ull;
+        if (i < n)
+            key[s] = ((unsigned long long)__double_as_longlong(fold_phase(tt[i], f)) & ~FAST_IDX_MASK) | (unsigned long long)i;
+    }
+    warp_sort64<S>(key, lane);
+#pragma unroll
+    for (int kw = 2; kw <= NW; kw <<= 1) {
+        // mirror step across warps: partner position = pos ^ (kw*32*S - 1)
+        {
+            const int ptid = ((warp ^ (kw - 1)) << 5) + (31 - lane);
+            const bool lower = (warp & (kw >> 1)) == 0;
+#pragma unroll
+            for (int s = 0; s < S; s++) kbuf[s * T + tid] = key[s];
+            __syncthreads();
+#pragma unroll
+            for (int s = 0; s < S; s++) {
+                const unsigned long long o = kbuf[(S - 1 - s) * T + ptid];
+                key[s] = lower ? min(key[s], o) : max(key[s], o);
+            }
+            __syncthreads();
+        }
+#pragma unroll
+        for (int jw = kw >> 2; jw >= 1; jw >>= 1) {
+            const int ptid = ((warp ^ jw) << 5) + lane;
+            const bool lower = (warp & jw) == 0;
+#pragma unroll
+            for (int s = 0; s < S; s++) kbuf[s * T + tid] = key[s];
+            __syncthreads();
+#pragma unroll
+            for (int s = 0; s < S; s++) {
+                const unsigned long long o = kbuf[s * T + ptid];
+                key[s] = lower ? min(key[s], o) : max(key[s], o);
+            }
+            __syncthreads();
+        }
+        merge_tail64<S>(key, lane, 16);
+    }
+#pragma unroll
+    for (int s = 0; s < S; s++) {
+        const int pos = tid * S + s;
+        if (pos < n) idx[pos] = (unsigned int)(key[s] & FAST_IDX_MASK);
+    }
+}
+
 // One eval.  S = base of BLOCK_SLOTS arrays of `sl` doubles (shared or global memory).
 // Returns P (valid in every thread).  If smo_dbg != null the smooth (phase order, un-centred) and the
 // permutation are written out (ss_debug_eval).
@@ -152,56 +283,83 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
     double* Ewy = S + 6 * sl;      double* Ewxy = S + 7 * sl;
     double* A0 = S + 8 * sl;       double* A1 = S + 9 * sl;       double* A2 = S + 10 * sl;
     double* r0 = S + 11 * sl;      double* r1 = S + 12 * sl;      double* r2 = S + 13 * sl;
-    // sort arrays overlay r0/r1 (dead until pass 1); the keys are kept for tie detection
+    // sort scratch overlays slots that are dead until pass 1: exact keys / exchange buffer in r0..r1,
+    // the sorted permutation in A2, the sorted phases in A0
     unsigned long long* key = reinterpret_cast<unsigned long long*>(r0);
-    unsigned int* idx = reinterpret_cast<unsigned int*>(r1);
+    unsigned int* idx = reinterpret_cast<unsigned int*>(A2);
+    double* phi = A0;
 
-    if (tid < 4) cx.flags[tid] = 0;
-    // ---- P1 fold + key init
-    for (int j = tid; j < n; j += T) {
-        key[j] = (unsigned long long)__double_as_longlong(fold_phase(tt[j], f));
-        idx[j] = (unsigned int)j;
+    // fast path: packed keys in registers (S per thread); needs T*S exchange words inside r0..r1
+    int fs = 0;
+    if (n <= T * 8 && n <= (int)FAST_IDX_MASK) {
+        fs = 1;
+        while (T * fs < n) fs <<= 1;
+        if ((int64_t)T * fs > 2 * sl) fs = 0;
     }
-    __syncthreads();
-    // ---- P2 bitonic network for arbitrary n (all exchanges ascending; indices >= n act as +inf)
-    int np2 = 1;
-    while (np2 < n) np2 <<= 1;
-    const int half = np2 >> 1;
-    for (int lk = 1; (1 << (lk - 1)) < n; lk++) {
-        const int k = 1 << lk, hk = k >> 1;           // strides are powers of two: shifts, no division
-        for (int t = tid; t < half; t += T) {
-            int blk = t >> (lk - 1), o = t & (hk - 1);
-            int a = (blk << lk) + o, b = (blk << lk) + k - 1 - o;
-            if (b < n) cex(key, idx, a, b);
-        }
-        __syncthreads();
-        for (int lj = lk - 2; lj >= 0; lj--) {
-            const int jj = 1 << lj;
-            for (int t = tid; t < half; t += T) {
-                int blk = t >> lj, o = t & (jj - 1);
-                int a = (blk << (lj + 1)) + o, b = a + jj;
-                if (b < n) cex(key, idx, a, b);
+    for (;;) {
+        if (tid < 4) cx.flags[tid] = 0;
+        if (fs == 1) block_sort_fast<T, 1>(n, tt, f, key, idx);
+        else if (fs == 2) block_sort_fast<T, 2>(n, tt, f, key, idx);
+        else if (fs == 4) block_sort_fast<T, 4>(n, tt, f, key, idx);
+        else if (fs == 8) block_sort_fast<T, 8>(n, tt, f, key, idx);
+        else {
+            // ---- exact path: P1 fold + key init
+            for (int j = tid; j < n; j += T) {
+                key[j] = (unsigned long long)__double_as_longlong(fold_phase(tt[j], f));
+                idx[j] = (unsigned int)j;
             }
             __syncthreads();
+            // ---- P2 bitonic network for arbitrary n (all exchanges ascending; indices >= n act as +inf)
+            int np2 = 1;
+            while (np2 < n) np2 <<= 1;
+            const int half = np2 >> 1;
+            for (int lk = 1; (1 << (lk - 1)) < n; lk++) {
+                const int k = 1 << lk, hk = k >> 1;           // strides are powers of two: shifts, no division
+                for (int t = tid; t < half; t += T) {
+                    int blk = t >> (lk - 1), o = t & (hk - 1);
+                    int a = (blk << lk) + o, b = (blk << lk) + k - 1 - o;
+                    if (b < n) cex(key, idx, a, b);
+                }
+                __syncthreads();
+                for (int lj = lk - 2; lj >= 0; lj--) {
+                    const int jj = 1 << lj;
+                    for (int t = tid; t < half; t += T) {
+                        int blk = t >> lj, o = t & (jj - 1);
+                        int a = (blk << (lj + 1)) + o, b = a + jj;
+                        if (b < n) cex(key, idx, a, b);
+                    }
+                    __syncthreads();
+                }
+            }
         }
+        __syncthreads();
+        // ---- gather: exact phases again from the permutation, x centred by 0.5,
+        // y already centred by ybar_w
+        for (int j = tid; j < n; j += T) {
+            const unsigned int i = idx[j];
+            const double ph = fold_phase(tt[i], f);
+            phi[j] = ph;
+            x[j] = ph - 0.5;
+            ys[j] = yc[i];
+            ws[j] = wo[i];
+            if (perm_dbg) perm_dbg[j] = (int32_t)i;
+        }
+        __syncthreads();
+        for (int j = tid; j + 1 < n; j += T) {
+            if (phi[j + 1] == phi[j]) cx.flags[0] = 1;                                   // tie (stable by index)
+            if (phi[j + 1] < phi[j] || (phi[j + 1] == phi[j] && idx[j + 1] < idx[j])) cx.flags[1] = 1;   // truncated keys misordered
+        }
+        __syncthreads();
+        if (fs != 0 && cx.flags[1] != 0) { fs = 0; __syncthreads(); continue; }        // redo with the exact network
+        break;
     }
-    // ---- gather: x centred by 0.5, y already centred by ybar_w
-    for (int j = tid; j < n; j += T) {
-        unsigned int i = idx[j];
-        x[j] = __longlong_as_double((long long)key[j]) - 0.5;
-        ys[j] = yc[i];
-        ws[j] = wo[i];
-        if (perm_dbg) perm_dbg[j] = (int32_t)i;
-        if (j + 1 < n && key[j + 1] <= key[j]) cx.flags[0] = 1;
-    }
-    __syncthreads();
     const bool has_ties = cx.flags[0] != 0;
-    // keys must survive pass 1 when there are ties: move them to A2's slot is not possible (A2 is
-    // written in pass 1), so in the tie path they are re-derived from x (x + 0.5 is monotone in key).
+    __syncthreads();
+    if (tid == 1) cx.flags[1] = 0;
 
     double chi2_part = 0.0;
-    const double phi_first = __longlong_as_double((long long)key[0]);
-    const double phi_last = __longlong_as_double((long long)key[n - 1]);
+    const double phi_first = phi[0];
+    const double phi_last = phi[n - 1];
     if (phi_last <= phi_first) {
         // Listing 1 lines 25-36: all phases equal -> weighted mean
         double sw = 0.0, sy = 0.0;
@@ -217,9 +375,9 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
         double chi2 = block_sum<T>(chi2_part, cx.red);
         return rec.chi0 > 0.0 ? (rec.chi0 - chi2) / rec.chi0 : 0.0;
     }
-    const double scale = __longlong_as_double((long long)key[rec.q3]) - __longlong_as_double((long long)key[rec.q1]);
+    const double scale = phi[rec.q3] - phi[rec.q1];
     const double vsmlsq = 1.e-6 * scale * scale;
-    __syncthreads();                               // key[] (in r0) is dead from here on
+    __syncthreads();                               // phi[] (in A0) and idx[] (in A2) are dead from here on
 
     const int ibw0 = rec.ibw[0], ibw1 = rec.ibw[1], ibw2 = rec.ibw[2];
     const int K0 = min(2 * ibw0 + 1, n), K1 = min(2 * ibw1 + 1, n), K2 = min(2 * ibw2 + 1, n);
