@@ -26,6 +26,10 @@ struct BlockCtx {
 };
 
 // Exclusive prefix sums of NA value streams at once; E[a][0..n], E[a][n] = total.
+// Blocked: a thread owns SCAN_CB consecutive elements (odd, so its 64-bit accesses at stride SCAN_CB
+// are bank-conflict free), sums them in registers, and the warp runs ONE Kogge-Stone per stream for
+// 32*SCAN_CB elements.
+constexpr int SCAN_CB = 5;
 template <int T, int NA, typename F>
 __device__ __forceinline__ void block_scan(int n, F vals, double* const (&E)[NA], double (*wsum)[T / 32])
 {
@@ -34,24 +38,31 @@ __device__ __forceinline__ void block_scan(int n, F vals, double* const (&E)[NA]
     double carry[NA];
 #pragma unroll
     for (int a = 0; a < NA; a++) carry[a] = 0.0;
-    for (int base = 0; base < n; base += T) {
-        const int j = base + tid;
-        double v[NA], inc[NA];
-        if (j < n) vals(j, v);
-        else {
+    for (int base = 0; base < n; base += T * SCAN_CB) {
+        const int j0 = base + tid * SCAN_CB;
+        double v[SCAN_CB][NA], run[NA], inc[NA];
 #pragma unroll
-            for (int a = 0; a < NA; a++) v[a] = 0.0;
+        for (int a = 0; a < NA; a++) run[a] = 0.0;
+#pragma unroll
+        for (int s = 0; s < SCAN_CB; s++) {
+            if (j0 + s < n) vals(j0 + s, v[s]);
+            else {
+#pragma unroll
+                for (int a = 0; a < NA; a++) v[s][a] = 0.0;
+            }
+#pragma unroll
+            for (int a = 0; a < NA; a++) run[a] += v[s][a];
         }
 #pragma unroll
         for (int a = 0; a < NA; a++) {
-            double s = v[a];
+            double t = run[a];
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
-                double o = __shfl_up_sync(0xffffffffu, s, d);
-                if (lane >= d) s += o;
+                double o = __shfl_up_sync(0xffffffffu, t, d);
+                if (lane >= d) t += o;
             }
-            inc[a] = s;
-            if (lane == 31) wsum[a][warp] = s;
+            inc[a] = t;
+            if (lane == 31) wsum[a][warp] = t;
         }
         __syncthreads();
 #pragma unroll
@@ -67,7 +78,12 @@ __device__ __forceinline__ void block_scan(int n, F vals, double* const (&E)[NA]
             }
             const double woff = __shfl_sync(0xffffffffu, sc - mine, warp);
             const double tot = __shfl_sync(0xffffffffu, sc, NW - 1);
-            if (j < n) E[a][j] = carry[a] + woff + (inc[a] - v[a]);
+            double out = carry[a] + woff + (inc[a] - run[a]);
+#pragma unroll
+            for (int s = 0; s < SCAN_CB; s++) {
+                if (j0 + s < n) E[a][j0 + s] = out;
+                out += v[s][a];
+            }
             carry[a] += tot;
         }
         __syncthreads();
@@ -562,7 +578,7 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
 
 // Persistent kernel: work item = (list entry, frequency chunk).  STAGE = per-eval arrays in global.
 template <int T, bool STAGE>
-__global__ void __launch_bounds__(T) block_kernel(const EvalParams p)
+__global__ void __launch_bounds__(T, (T <= 256 ? 2 : 1)) block_kernel(const EvalParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NW = T / 32;
