@@ -155,6 +155,59 @@ __device__ __forceinline__ void warp_sort(unsigned (&key)[S], int lane)
     }
 }
 
+// Optimal comparator networks for the lane-local sort of C = 3, 5, 6, 7 keys (3 / 9 / 12 / 16
+// compare-exchanges; each verified on all 0-1 inputs).
+template <int C> __device__ __forceinline__ void local_sort(unsigned (&k)[C]);
+#define SS_CX(a, b) cex32(k[a], k[b]);
+template <> __device__ __forceinline__ void local_sort<3>(unsigned (&k)[3]) { SS_CX(0, 2) SS_CX(0, 1) SS_CX(1, 2) }
+template <> __device__ __forceinline__ void local_sort<5>(unsigned (&k)[5])
+{
+    SS_CX(0, 3) SS_CX(1, 4) SS_CX(0, 2) SS_CX(1, 3) SS_CX(0, 1) SS_CX(2, 4) SS_CX(1, 2) SS_CX(3, 4) SS_CX(2, 3)
+}
+template <> __device__ __forceinline__ void local_sort<6>(unsigned (&k)[6])
+{
+    SS_CX(0, 5) SS_CX(1, 3) SS_CX(2, 4) SS_CX(1, 2) SS_CX(3, 4) SS_CX(0, 3) SS_CX(2, 5) SS_CX(0, 1) SS_CX(2, 3) SS_CX(4, 5)
+    SS_CX(1, 2) SS_CX(3, 4)
+}
+template <> __device__ __forceinline__ void local_sort<7>(unsigned (&k)[7])
+{
+    SS_CX(0, 6) SS_CX(2, 3) SS_CX(4, 5) SS_CX(0, 2) SS_CX(1, 4) SS_CX(3, 6) SS_CX(0, 1) SS_CX(2, 5) SS_CX(3, 4) SS_CX(1, 2)
+    SS_CX(4, 6) SS_CX(2, 3) SS_CX(4, 5) SS_CX(1, 2) SS_CX(3, 4) SS_CX(5, 6)
+}
+#undef SS_CX
+
+// Blocked bitonic sort of 32*C keys for any C (position = lane*C + s): lane-local network, then for
+// k = 2..32 lanes a mirror step (lane ^ (k-1), slots reversed), half-cleaners at lane strides k/4..1
+// (each half has even length, so the half-cleaner property holds) and the lane-local network again on
+// the bitonic remainder.  15 cross-lane steps of C shuffles instead of the 15 x 8 of the padded
+// power-of-two network, and the sorted keys sit in the slots that own them (no re-blocking).
+template <int C>
+__device__ __forceinline__ void warp_sort_any(unsigned (&key)[C], int lane)
+{
+    local_sort<C>(key);
+#pragma unroll
+    for (int k = 2; k <= 32; k <<= 1) {
+        {
+            const bool lower = (lane & (k >> 1)) == 0;
+            unsigned other[C];
+#pragma unroll
+            for (int s = 0; s < C; s++) other[s] = __shfl_xor_sync(0xffffffffu, key[C - 1 - s], k - 1);
+#pragma unroll
+            for (int s = 0; s < C; s++) key[s] = lower ? min(key[s], other[s]) : max(key[s], other[s]);
+        }
+#pragma unroll
+        for (int m = k >> 2; m >= 1; m >>= 1) {
+            const bool lower = (lane & m) == 0;
+#pragma unroll
+            for (int s = 0; s < C; s++) {
+                const unsigned o = __shfl_xor_sync(0xffffffffu, key[s], m);
+                key[s] = lower ? min(key[s], o) : max(key[s], o);
+            }
+        }
+        local_sort<C>(key);
+    }
+}
+
 // Halo of one register array: u[t] = element at j = lane*C - IBW0 + t (fill outside 0..32C-1).
 template <int C, int IBW0, bool FILL = true>
 __device__ __forceinline__ void make_halo(const double (&v)[C], double (&u)[C + 2 * IBW0], int lane, double fill)
@@ -660,9 +713,10 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
     defer = false;
 
     // ---- P1 fold + 32-bit keys (24 phase bits | 8 index bits); P2 sort
-    unsigned key[S];
+    constexpr int SK = (S == C) ? S : C;       // keys per lane: C itself (power of two or not)
+    unsigned key[SK];
 #pragma unroll
-    for (int s = 0; s < S; s++) {
+    for (int s = 0; s < SK; s++) {
         const int i = lane + 32 * s;
         unsigned k = 0xffffffffu;
         if (i < n) {
@@ -671,19 +725,11 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
         }
         key[s] = k;
     }
-    warp_sort<S>(key, lane);
+    if constexpr (S == C) warp_sort<S>(key, lane);
+    else warp_sort_any<C>(key, lane);
     int idx[C];
-    if (S == C) {
 #pragma unroll
-        for (int s = 0; s < C; s++) idx[s] = (int)(key[s < S ? s : 0] & 0xffu);
-    } else {
-#pragma unroll
-        for (int s = 0; s < S; s++) M.perm[lane * S + s] = (unsigned char)(key[s] & 0xffu);
-        __syncwarp();
-#pragma unroll
-        for (int s = 0; s < C; s++) idx[s] = M.perm[lane * C + s];
-        __syncwarp();
-    }
+    for (int s = 0; s < C; s++) idx[s] = (int)(key[s] & 0xffu);
     // ---- gather and exact-order check on the full 64-bit phases
     double x[C], y[C], w[C], phi[C];
 #pragma unroll
