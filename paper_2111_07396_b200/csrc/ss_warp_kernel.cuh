@@ -73,18 +73,19 @@ template <int C>
 __device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const double (&b)[C], double2* E, int lane,
                                                   const ScanMask& mk)
 {
-    double ea[C], eb[C];
     double ra = a[0], rb = b[0];
-    ea[0] = 0.0; eb[0] = 0.0;
 #pragma unroll
-    for (int s = 1; s < C; s++) { ea[s] = ra; ra += a[s]; eb[s] = rb; rb += b[s]; }
+    for (int s = 1; s < C; s++) { ra += a[s]; rb += b[s]; }
     double ia = ra, ib = rb;
 #pragma unroll
     for (int i = 0; i < 5; i++) { scan_step(ia, i, mk); scan_step(ib, i, mk); }
-    const double xa = ia - ra, xb = ib - rb;
-    E[lane] = make_double2(xa, xb);
+    // exclusive prefixes are re-accumulated from the lane's offset (no second register array)
+    double xa = ia - ra, xb = ib - rb;
 #pragma unroll
-    for (int s = 1; s < C; s++) E[s * WROW + lane] = make_double2(xa + ea[s], xb + eb[s]);
+    for (int s = 0; s < C; s++) {
+        E[s * WROW + lane] = make_double2(xa, xb);
+        xa += a[s]; xb += b[s];
+    }
     if (lane == 31) E[32] = make_double2(ia, ib);     // E[32*C] lives at row 0, column 32
 }
 
@@ -92,18 +93,15 @@ __device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const do
 template <int C>
 __device__ __forceinline__ void single_prefix_store(const double (&a)[C], double* E, int lane, const ScanMask& mk)
 {
-    double ea[C];
     double ra = a[0];
-    ea[0] = 0.0;
 #pragma unroll
-    for (int s = 1; s < C; s++) { ea[s] = ra; ra += a[s]; }
+    for (int s = 1; s < C; s++) ra += a[s];
     double ia = ra;
 #pragma unroll
     for (int i = 0; i < 5; i++) scan_step(ia, i, mk);
-    const double xa = ia - ra;
-    E[lane] = xa;
+    double xa = ia - ra;
 #pragma unroll
-    for (int s = 1; s < C; s++) E[s * WROW + lane] = xa + ea[s];
+    for (int s = 0; s < C; s++) { E[s * WROW + lane] = xa; xa += a[s]; }
     if (lane == 31) E[32] = ia;
 }
 
