@@ -383,10 +383,10 @@ struct EvalConst {
     int n, ibw1, ibw2, K1, K2;
     int lane_r, slot_r;      // owner of the right-end tweeter window, jr = n-1-IBW0
     int q1l, q1s, q3l, q3s;  // owners of the quartile points
-    double gk1[2], gk2[2];   // 1/(1 - p/K) for p = 1, 2 (GV score, R12)
+    const double* kc;        // shared memory: {gk1[0], gk1[1], gk2[0], gk2[1], chi0, 1/chi0}; gk = 1/(1 - p/K), p = 1, 2
+                             // (GV score, R12).  Read, not kept: in registers the compiler re-derives the divisions per eval
     double alpha, bexp;      // bass enhancement
     int bass;                // 0 = off, 1 = exponent 1 (alpha = 9), 2 = general pow
-    double chi0, inv_chi0;
 };
 
 // Listing 1 lines 63-77 with the loop-invariant tests hoisted.
@@ -532,7 +532,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
                 const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
                 A1 = yb + b * (xj - xb);
                 const double rss = (Syy - yb * Sy) - b * sxy;
-                G1 = sqrt64(rss * isw) * (isxx != 0.0 ? K.gk1[1] : K.gk1[0]);
+                G1 = sqrt64(rss * isw) * (isxx != 0.0 ? K.kc[1] : K.kc[0]);
             }
             {
                 const int a2 = w2[s], b2 = w2[C + s];
@@ -545,7 +545,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
                 const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
                 A2 = yb + b * (xj - xb);
                 const double rss = (Syy - yb * Sy) - b * sxy;
-                G2 = sqrt64(rss * isw) * (isxx != 0.0 ? K.gk2[1] : K.gk2[0]);
+                G2 = sqrt64(rss * isw) * (isxx != 0.0 ? K.kc[3] : K.kc[2]);
             }
             const double sp = pick_span_w(t_g[s], G1, G2, K);
             const double smo = interp_spans(sp, A0, A1, A2);
@@ -698,7 +698,7 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
 #undef SS_CLAMP
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, d);
-    return (K.chi0 - chi2) * K.inv_chi0;
+    return (K.kc[4] - chi2) * K.kc[5];
 }
 
 // One eval.  Returns P in every lane; `defer` is set (warp-uniform) when the fast path cannot
@@ -805,11 +805,15 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
         const int q1 = uni(rec.q1), q3 = uni(rec.q3);
         K.q1l = q1 / C; K.q1s = q1 % C; K.q3l = q3 / C; K.q3s = q3 % C;
     }
-    K.gk1[0] = 1.0 / (1.0 - 1.0 / (double)K.K1); K.gk1[1] = 1.0 / (1.0 - 2.0 / (double)K.K1);
-    K.gk2[0] = 1.0 / (1.0 - 1.0 / (double)K.K2); K.gk2[1] = 1.0 / (1.0 - 2.0 / (double)K.K2);
+    __shared__ double s_kc[6];
+    if (tid == 0) {
+        s_kc[0] = 1.0 / (1.0 - 1.0 / (double)K.K1); s_kc[1] = 1.0 / (1.0 - 2.0 / (double)K.K1);
+        s_kc[2] = 1.0 / (1.0 - 1.0 / (double)K.K2); s_kc[3] = 1.0 / (1.0 - 2.0 / (double)K.K2);
+        s_kc[4] = rec.chi0; s_kc[5] = rec.chi0 > 0.0 ? 1.0 / rec.chi0 : 0.0;
+    }
+    K.kc = s_kc;
     K.alpha = p.alpha; K.bexp = 10.0 - p.alpha;
     K.bass = (p.alpha > 0.0 && p.alpha <= 10.0) ? (K.bexp == 1.0 ? 1 : 2) : 0;
-    K.chi0 = rec.chi0; K.inv_chi0 = rec.chi0 > 0.0 ? 1.0 / rec.chi0 : 0.0;
 
     double* o_tt = reinterpret_cast<double*>(smem_raw);
     double* o_y = o_tt + 32 * C;
