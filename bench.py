@@ -51,6 +51,9 @@ def parse():
     ap.add_argument("--mode", default="cv", choices=["cv", "gv"])
     ap.add_argument("--objects", type=int, default=10000, help="(debug) fewer objects than config 3")
     ap.add_argument("--freqs", type=int, default=50000, help="(debug) fewer frequencies than config 3")
+    ap.add_argument("--iper", type=int, default=1, help="(sweep) 2 = periodic windows, PAPER.md:199-200")
+    ap.add_argument("--span", type=float, default=0.0, help="(sweep) > 0 = fixed span, PAPER.md:202-210")
+    ap.add_argument("--path", type=int, default=0, help="(sweep) force a path class: 1 warp, 2 CTA, 3 staging")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -230,7 +233,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     def step(m=mode, profile=False):
-        o = ss.default_options(profile=1 if profile else 0)
+        o = ss.default_options(profile=1 if profile else 0, iper=args.iper, span=args.span, force_path=args.path)
         ss.ss_periodogram(t, y, e, off, n_obj, cat.f_min, cat.f_max, n_freq, m, pg, bf, bi, o)
 
     for _ in range(args.warmup):
@@ -277,7 +280,8 @@ def run_ours(args):
         hbf = torch.empty(n_obj, dtype=torch.float64).pin_memory()
         hbi = torch.empty(n_obj, dtype=torch.int64).pin_memory()
         def estep():
-            ss.ss_periodogram_host(ht, hy, he, hoff, n_obj, cat.f_min, cat.f_max, n_freq, mode, hpg, hbf, hbi)
+            ss.ss_periodogram_host(ht, hy, he, hoff, n_obj, cat.f_min, cat.f_max, n_freq, mode, hpg, hbf, hbi,
+                                   ss.default_options(iper=args.iper, span=args.span, force_path=args.path))
         estep()
         barrier()
         t0 = time.perf_counter()
@@ -323,7 +327,9 @@ def run_ours(args):
            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": f"config3: {n_obj} objects (n~U[50,200], {cat.n_points} points) x {n_freq} "
-                      f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised",
+                      f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised"
+                      + (f", iper={args.iper}" if args.iper != 1 else "") + (f", span={args.span}" if args.span else "")
+                      + (f", forced path {args.path}" if args.path else ""),
                       "objects_per_second": world * n_obj * args.steps / (elapsed_ms * 1e-3),
                       "l2": "catalog (30 MB) is re-read per frequency by design; the 4 GB periodogram "
                             "written every step exceeds L2, nothing is cached between steps",

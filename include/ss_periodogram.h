@@ -48,7 +48,7 @@ typedef enum {
     SS_ERR_INVALID_ARG = 1,   /* null pointer, bad sizes/grid, non-monotone offsets, non-finite data, err <= 0 */
     SS_ERR_OUT_OF_MEMORY = 2, /* workspace could not be allocated / cap too small for one tile           */
     SS_ERR_CUDA = 3,          /* a CUDA runtime call or kernel failed                                   */
-    SS_ERR_UNSUPPORTED = 4    /* option not implemented (iper = 2, fixed span: see DESIGN.md "next")     */
+    SS_ERR_UNSUPPORTED = 4    /* an object above 2^24 points, or more work items than one tile can index  */
 } ss_status_t;
 
 /* Which kernel family serves an object (chosen by its number of points n). */
@@ -63,8 +63,12 @@ typedef enum {
 
 typedef struct {
     double alpha;           /* bass enhancement.  Default 9.0.                 */
-    double span;            /* 0 = variable span (default).  > 0 (fixed span): UNSUPPORTED */
-    int iper;               /* 1 = non-periodic windows (default, R8).  2: UNSUPPORTED for now          */
+    double span;            /* 0 = variable span (default).  In (0, 1]: Listing 1's fixed-span branch
+                               (PAPER.md:202-210): one running-line smooth at this span, in both modes.
+                               Served by the CTA-per-eval kernels for every n.                           */
+    int iper;               /* 1 = windows pinned at the ends (default, R8).  2 = periodic windows
+                               (PAPER.md:199-200): the window of point j is j-ibw..j+ibw modulo n, phases
+                               that wrapped count as x-1 / x+1.  Served by the CTA-per-eval kernels.     */
     int force_path;         /* ss_path_t; SS_PATH_AUTO = choose by n.  For tests and sweeps.            */
     void *stream;           /* cudaStream_t the work is enqueued on (NULL = legacy default stream)      */
     size_t workspace_cap;   /* bytes of device workspace the library may allocate; 0 = 75 % of free

@@ -295,11 +295,13 @@ static ss_status_t validate_scalars(int64_t n_objects, double f_min, double f_ma
     if (!(f_max > f_min) || !std::isfinite(f_max)) return fail(SS_ERR_INVALID_ARG, "f_max must be finite and > f_min");
     if (mode != SS_MODE_CROSS_VALIDATION && mode != SS_MODE_GENERALIZED_VALIDATION)
         return fail(SS_ERR_INVALID_ARG, "unknown mode %d", mode);
-    if (o.span != 0.0) return fail(SS_ERR_UNSUPPORTED, "fixed span is not implemented (DESIGN.md: next)");
-    if (o.iper != 1) return fail(SS_ERR_UNSUPPORTED, "iper = %d is not implemented (DESIGN.md: next)", o.iper);
+    if (!(o.span >= 0.0) || !(o.span <= 1.0)) return fail(SS_ERR_INVALID_ARG, "span must be 0 (variable) or in (0, 1]");
+    if (o.iper != 1 && o.iper != 2) return fail(SS_ERR_INVALID_ARG, "iper = %d (1 = non-periodic, 2 = periodic)", o.iper);
     if (!std::isfinite(o.alpha)) return fail(SS_ERR_INVALID_ARG, "alpha is not finite");
     return SS_OK;
 }
+
+static bool has_listing_options(const ss_options_t& o) { return o.iper == 2 || o.span > 0.0; }
 
 static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
@@ -332,6 +334,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         r.off = off[i]; r.obj = i; r.n = (int32_t)n;
         r.ibw[0] = half_width(n, SPAN0); r.ibw[1] = half_width(n, SPAN1); r.ibw[2] = half_width(n, SPAN2);
         r.q1 = (int32_t)(n / 4 - 1); r.q3 = 3 * (r.q1 + 1) - 1;
+        r.ibw_fixed = o.span > 0.0 ? half_width(n, o.span) : 0;
         recs.push_back(r);
         max_n = std::max(max_n, (int)n);
     }
@@ -363,11 +366,13 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             const ObjRec& r = recs[ri];
             if (r.obj < o0 || r.obj >= o1) continue;
             int path = o.force_path != SS_PATH_AUTO ? o.force_path : path_for_n(r.n, md);
+            // periodic windows and the fixed span live in the generic CTA-per-eval code only
+            if (path == SS_PATH_WARP && has_listing_options(o)) path = SS_PATH_BLOCK;
             if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_BLOCK;
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
             if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
-            else if (path == SS_PATH_BLOCK) variant = r.n <= 500 ? 0 : (r.n <= 1020 ? 1 : 2);
+            else if (path == SS_PATH_BLOCK) variant = r.n <= 256 ? 3 : (r.n <= 500 ? 0 : (r.n <= 1020 ? 1 : 2));
             ClassList& c = find(path, variant);
             c.recs.push_back((int32_t)ri);
             c.max_n = std::max(c.max_n, (int)r.n);
@@ -467,7 +472,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         cpo = (nk + chunk - 1) / chunk;
         p.chunk = (int32_t)chunk; p.chunks_per_obj = (int32_t)cpo;
         p.chunks_total = (int32_t)cpo_cap; p.chunk_base = 0;
-        p.alpha = opt.alpha; p.mode = mode;
+        p.alpha = opt.alpha; p.mode = mode; p.iper = opt.iper; p.span = opt.span;
         p.pgram = pgram; p.pgram_row_stride = row_stride; p.pgram_k0 = k0; p.pgram_row0 = row0;
         p.part_val = part_val; p.part_idx = part_idx;
         p.counter = counters + (next_counter % n_counters);
@@ -490,21 +495,31 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else {
+            const bool optk = has_listing_options(opt);
             if (c.path == SS_PATH_BLOCK) {
                 const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(c.max_n) * 8;
                 if (c.variant == 2) {
-                    SS_CUDA(cudaFuncSetAttribute(block_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    auto kern = optk ? block_kernel<512, false, true> : block_kernel<512, false, false>;
+                    SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                     int grid = (int)std::min<int64_t>(n_items, sm_count);
-                    block_kernel<512, false><<<grid, 512, smem, stream>>>(p);
+                    kern<<<grid, 512, smem, stream>>>(p);
+                } else if (c.variant == 3) {
+                    // short light curves reach this path only through the listing's options or a forced path
+                    auto kern = optk ? block_kernel<128, false, true> : block_kernel<128, false, false>;
+                    SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 4);
+                    kern<<<grid, 128, smem, stream>>>(p);
                 } else {
-                    SS_CUDA(cudaFuncSetAttribute(block_kernel<256, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    auto kern = optk ? block_kernel<256, false, true> : block_kernel<256, false, false>;
+                    SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                     int per_sm = c.variant == 0 ? 4 : 2;
                     int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * per_sm);
-                    block_kernel<256, false><<<grid, 256, smem, stream>>>(p);
+                    kern<<<grid, 256, smem, stream>>>(p);
                 }
             } else {
+                auto kern = optk ? block_kernel<512, true, true> : block_kernel<512, true, false>;
                 int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 2);
-                block_kernel<512, true><<<grid, 512, 0, stream>>>(p);
+                kern<<<grid, 512, 0, stream>>>(p);
             }
         }
         if (ev1) SS_CUDA(cudaEventRecord(ev1, stream));
@@ -776,8 +791,10 @@ ss_status_t ss_debug_eval(const double* times, const double* mags, const double*
     if (st != SS_OK) return st;
     EvalParams p{};
     p.tt = eng.tt; p.yc = eng.yc; p.w = eng.w; p.recs = eng.d_recs; p.alpha = o.alpha; p.mode = (int)mode;
+    p.iper = o.iper; p.span = o.span;
     p.stage = eng.stage; p.stage_stride = eng.stage_stride;
-    block_debug_kernel<512><<<1, 512, 0, eng.stream>>>(p, freq, smo_out, perm_out, p_out);
+    if (has_listing_options(o)) block_debug_kernel<512, true><<<1, 512, 0, eng.stream>>>(p, freq, smo_out, perm_out, p_out);
+    else block_debug_kernel<512, false><<<1, 512, 0, eng.stream>>>(p, freq, smo_out, perm_out, p_out);
     g_launches++;
     SS_CUDA(cudaGetLastError());
     SS_CUDA(cudaStreamSynchronize(eng.stream));

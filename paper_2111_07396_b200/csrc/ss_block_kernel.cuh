@@ -281,10 +281,58 @@ __device__ __forceinline__ void block_sort_fast(int n, const double* tt, double 
     }
 }
 
+// Window of point j as ranges of the prefix arrays (O4).  Non-periodic (jper = 1): [lo, hi) =
+// the K points centred on j, pinned at the ends.  Periodic (jper = 2, only with OPT):
+// j-ibw .. j+ibw modulo n -- the part inside [0, n) is [lo, hi), the part that wrapped is [blo, bhi)
+// and its abscissae count as x + s, s = -1 (wrapped below 0) or +1 (wrapped above n-1).
+template <bool OPT>
+struct Win {
+    int lo, hi, blo, bhi;
+    double s;
+    __device__ __forceinline__ Win(int j, int ibw, int K, int n, bool per)
+    {
+        blo = bhi = 0; s = 0.0;
+        if (OPT && per) {
+            lo = j - ibw; hi = j + ibw + 1;
+            if (lo < 0) { blo = lo + n; bhi = n; lo = 0; s = -1.0; }
+            else if (hi > n) { bhi = hi - n; hi = n; s = 1.0; }
+        } else {
+            lo = window_lo(j, ibw, K, n);
+            hi = lo + K;
+        }
+    }
+    __device__ __forceinline__ double wrapped(const double* E) const { return OPT ? E[bhi] - E[blo] : 0.0; }
+    __device__ __forceinline__ double sum(const double* E) const
+    {
+        double v = E[hi] - E[lo];
+        if (OPT) v += E[bhi] - E[blo];
+        return v;
+    }
+    // sum w x^q over the window, q = 0, 1, 2, with the wrapped part shifted by s
+    __device__ __forceinline__ XMom xmom(const double* Ew, const double* Ewx, const double* Ewxx, double vsmlsq) const
+    {
+        double Sw = sum(Ew), Swx = sum(Ewx), Swxx = sum(Ewxx);
+        if (OPT) {
+            const double bw = wrapped(Ew), bwx = wrapped(Ewx);
+            Swx += s * bw;
+            Swxx += 2.0 * s * bwx + bw;      // s*s = 1 where bw != 0
+        }
+        return x_moments(Sw, Swx, Swxx, vsmlsq);
+    }
+    // sum w z and sum w x z over the window
+    __device__ __forceinline__ void zmom(const double* Ewz, const double* Ewxz, double& Swz, double& Swxz) const
+    {
+        Swz = sum(Ewz); Swxz = sum(Ewxz);
+        if (OPT) Swxz += s * wrapped(Ewz);
+    }
+};
+
 // One eval.  S = base of BLOCK_SLOTS arrays of `sl` doubles (shared or global memory).
+// OPT = true adds the options Listing 1 has beside the default call: periodic windows (p.iper = 2)
+// and a fixed span (p.span > 0); the default instantiation carries none of that code.
 // Returns P (valid in every thread).  If smo_dbg != null the smooth (phase order, un-centred) and the
 // permutation are written out (ss_debug_eval).
-template <int T>
+template <int T, bool OPT>
 __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, double* S, int64_t sl,
                              const BlockCtx<T>& cx, double* smo_dbg, int32_t* perm_dbg)
 {
@@ -397,7 +445,9 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
 
     const int ibw0 = rec.ibw[0], ibw1 = rec.ibw[1], ibw2 = rec.ibw[2];
     const int K0 = min(2 * ibw0 + 1, n), K1 = min(2 * ibw1 + 1, n), K2 = min(2 * ibw2 + 1, n);
-    const bool gv = p.mode == 1;
+    const bool per = OPT && p.iper == 2;           // phases are in [0,1): jper = iper
+    const bool fixed = OPT && p.span > 0.0;
+    const bool gv = p.mode == 1 && !fixed;
 
     // ---- P3: prefix sums of the weighted moments
     if (!gv) {
@@ -416,7 +466,14 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
     }
     const double* Ewyy = A0;   // GV only
 
-    auto wsum2 = [&](const double* E, int lo, int K) { return E[lo + K] - E[lo]; };
+    // one running-line smooth of the stream whose prefix sums are (Ez, Exz), at half-width ibw
+    auto fit_at = [&](int j, int ibw, int K, const double* Ez, const double* Exz) {
+        const Win<OPT> wn(j, ibw, K, n, per);
+        XMom m = wn.xmom(Ew, Ewx, Ewxx, vsmlsq);
+        double Swz, Swxz, b, zb;
+        wn.zmom(Ez, Exz, Swz, Swxz);
+        return line_fit(m, Swz, Swxz, x[j], b, zb);
+    };
 
     if (gv) {
         // ---- O6: one sweep, three windows, score, pick, interpolate
@@ -427,12 +484,13 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
             const int ib[3] = {ibw0, ibw1, ibw2}, KK[3] = {K0, K1, K2};
 #pragma unroll
             for (int i = 0; i < 3; i++) {
-                int lo = window_lo(j, ib[i], KK[i], n);
-                XMom m = x_moments(wsum2(Ew, lo, KK[i]), wsum2(Ewx, lo, KK[i]), wsum2(Ewxx, lo, KK[i]), vsmlsq);
-                double Swy = wsum2(Ewy, lo, KK[i]), Swxy = wsum2(Ewxy, lo, KK[i]);
+                const Win<OPT> wn(j, ib[i], KK[i], n, per);
+                XMom m = wn.xmom(Ew, Ewx, Ewxx, vsmlsq);
+                double Swy, Swxy;
+                wn.zmom(Ewy, Ewxy, Swy, Swxy);
                 double b, yb;
                 A[i] = line_fit(m, Swy, Swxy, xj, b, yb);
-                G[i] = gv_score(m, Swy, Swxy, wsum2(Ewyy, lo, KK[i]), b, yb, KK[i]);
+                G[i] = gv_score(m, Swy, Swxy, wn.sum(Ewyy), b, yb, KK[i]);
             }
             double sp = pick_span(G[0], G[1], G[2], p.alpha);
             smo[j] = interp_spans(sp, A[0], A[1], A[2]);
@@ -472,6 +530,29 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
         }
     };
 
+    if (fixed) {
+        // ---- Listing 1 lines 51-55: one smooth of y at the caller's span, both modes
+        int ibwf = rec.ibw_fixed, Kf = 2 * ibwf + 1;
+        if (Kf > n) {
+            Kf = n;
+            if (per) { ibwf = (n - 1) / 2; Kf = 2 * ibwf + 1; }
+        }
+        double* smo = A1;
+        for (int j = tid; j < n; j += T) smo[j] = fit_at(j, ibwf, Kf, Ewy, Ewxy);
+        __syncthreads();
+        if (has_ties) {
+            if (tid == 0) tie_avg(smo);
+            __syncthreads();
+        }
+        for (int j = tid; j < n; j += T) {
+            double r = ys[j] - smo[j];
+            chi2_part += ws[j] * r * r;
+            if (smo_dbg) smo_dbg[j] = smo[j] + rec.ybar;
+        }
+        double chi2 = block_sum<T>(chi2_part, cx.red);
+        return rec.chi0 > 0.0 ? (rec.chi0 - chi2) / rec.chi0 : 0.0;
+    }
+
     // ---- CV pass 1: three smooths of y with leave-one-out residuals
     for (int j = tid; j < n; j += T) {
         const double xj = x[j], yj = ys[j], wj = ws[j];
@@ -480,10 +561,11 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
         double* const ro[3] = {r0, r1, r2};
 #pragma unroll
         for (int i = 0; i < 3; i++) {
-            int lo = window_lo(j, ib[i], KK[i], n);
-            XMom m = x_moments(wsum2(Ew, lo, KK[i]), wsum2(Ewx, lo, KK[i]), wsum2(Ewxx, lo, KK[i]), vsmlsq);
-            double b, yb;
-            double s = line_fit(m, wsum2(Ewy, lo, KK[i]), wsum2(Ewxy, lo, KK[i]), xj, b, yb);
+            const Win<OPT> wn(j, ib[i], KK[i], n, per);
+            XMom m = wn.xmom(Ew, Ewx, Ewxx, vsmlsq);
+            double Swy, Swxy, b, yb;
+            wn.zmom(Ewy, Ewxy, Swy, Swxy);
+            double s = line_fit(m, Swy, Swxy, xj, b, yb);
             double r = loo_residual(m, xj, wj, yj, s);
             if (r < 0.0) cx.flags[1 + i] = 1;
             Ao[i][j] = s;
@@ -510,12 +592,7 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
                 double wz = ws[j] * z[j];
                 v[0] = wz; v[1] = wz * x[j];
             }, E, cx.wsum);
-            for (int j = tid; j < n; j += T) {
-                int lo = window_lo(j, ibw1, K1, n);
-                XMom m = x_moments(wsum2(Ew, lo, K1), wsum2(Ewx, lo, K1), wsum2(Ewxx, lo, K1), vsmlsq);
-                double b, zb;
-                z[j] = line_fit(m, wsum2(Ewy, lo, K1), wsum2(Ewxy, lo, K1), x[j], b, zb);
-            }
+            for (int j = tid; j < n; j += T) z[j] = fit_at(j, ibw1, K1, Ewy, Ewxy);
             __syncthreads();
         }
         if (has_ties) {
@@ -533,12 +610,7 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
             double wz = ws[j] * r0[j];
             v[0] = wz; v[1] = wz * x[j];
         }, E, cx.wsum);
-        for (int j = tid; j < n; j += T) {
-            int lo = window_lo(j, ibw1, K1, n);
-            XMom m = x_moments(wsum2(Ew, lo, K1), wsum2(Ewx, lo, K1), wsum2(Ewxx, lo, K1), vsmlsq);
-            double b, zb;
-            r1[j] = line_fit(m, wsum2(Ewy, lo, K1), wsum2(Ewxy, lo, K1), x[j], b, zb);
-        }
+        for (int j = tid; j < n; j += T) r1[j] = fit_at(j, ibw1, K1, Ewy, Ewxy);
         __syncthreads();
         if (has_ties) {
             if (tid == 0) tie_avg(r1);
@@ -555,12 +627,7 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
             double wz = ws[j] * r2[j];
             v[0] = wz; v[1] = wz * x[j];
         }, E, cx.wsum);
-        for (int j = tid; j < n; j += T) {
-            int lo = window_lo(j, ibw0, K0, n);
-            XMom m = x_moments(wsum2(Ew, lo, K0), wsum2(Ewx, lo, K0), wsum2(Ewxx, lo, K0), vsmlsq);
-            double b, zb;
-            r0[j] = line_fit(m, wsum2(Ewy, lo, K0), wsum2(Ewxy, lo, K0), x[j], b, zb);
-        }
+        for (int j = tid; j < n; j += T) r0[j] = fit_at(j, ibw0, K0, Ewy, Ewxy);
         __syncthreads();
         if (has_ties) {
             if (tid == 0) tie_avg(r0);
@@ -577,8 +644,8 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
 }
 
 // Persistent kernel: work item = (list entry, frequency chunk).  STAGE = per-eval arrays in global.
-template <int T, bool STAGE>
-__global__ void __launch_bounds__(T, (T <= 256 ? 2 : 1)) block_kernel(const EvalParams p)
+template <int T, bool STAGE, bool OPT = false>
+__global__ void __launch_bounds__(T, (T <= 128 ? 4 : (T <= 256 ? 2 : 1))) block_kernel(const EvalParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NW = T / 32;
@@ -610,7 +677,7 @@ __global__ void __launch_bounds__(T, (T <= 256 ? 2 : 1)) block_kernel(const Eval
         int64_t best_k = k0;
         for (int64_t k = k0; k < k1; k++) {
             const double f = freq_of(p.f_min, p.df, k);
-            double P = block_eval<T>(p, rec, f, S, sl, cx, nullptr, nullptr);
+            double P = block_eval<T, OPT>(p, rec, f, S, sl, cx, nullptr, nullptr);
             if (threadIdx.x == 0) {
                 if (p.pgram)
                     p.pgram[(rec.obj - p.pgram_row0) * p.pgram_row_stride + (k - p.pgram_k0)] = P;
@@ -626,7 +693,7 @@ __global__ void __launch_bounds__(T, (T <= 256 ? 2 : 1)) block_kernel(const Eval
 }
 
 // ss_debug_eval: one eval, one CTA, arrays staged in global memory.
-template <int T>
+template <int T, bool OPT>
 __global__ void __launch_bounds__(T) block_debug_kernel(const EvalParams p, double f, double* smo_out,
                                                         int32_t* perm_out, double* p_out)
 {
@@ -637,7 +704,7 @@ __global__ void __launch_bounds__(T) block_debug_kernel(const EvalParams p, doub
     BlockCtx<T> cx;
     cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
     const ObjRec rec = p.recs[0];
-    double P = block_eval<T>(p, rec, f, p.stage, block_slot_len(rec.n), cx, smo_out, perm_out);
+    double P = block_eval<T, OPT>(p, rec, f, p.stage, block_slot_len(rec.n), cx, smo_out, perm_out);
     if (threadIdx.x == 0 && p_out) *p_out = P;
 }
 

@@ -22,7 +22,8 @@ struct ObjRec {
     int32_t n;       // number of points
     int32_t ibw[3];  // window half-widths for the three spans: max(2, floor(0.5*span*n + 0.5))
     int32_t q1, q3;  // quartile indices n/4-1, 3*(q1+1)-1
-    int32_t pad[2];
+    int32_t ibw_fixed;  // half-width of the caller's fixed span, 0 if span == 0
+    int32_t pad;
 };
 
 // Per-launch parameters.
@@ -41,6 +42,8 @@ struct EvalParams {
     int32_t chunk_base;       // index of this tile's first chunk in the partials row
     double alpha;             // bass enhancement
     int32_t mode;             // 0 = CV, 1 = GV
+    int32_t iper;             // 1 = windows pinned at the ends, 2 = periodic windows
+    double span;              // > 0: one smooth at this fixed span
     double* pgram;            // tile buffer or caller's array (may be null)
     int64_t pgram_row_stride; // elements between consecutive object rows
     int64_t pgram_k0;         // column 0 of `pgram` is frequency index pgram_k0

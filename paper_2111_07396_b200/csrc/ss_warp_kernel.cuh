@@ -927,7 +927,7 @@ __global__ void __launch_bounds__(DEFER_T) deferred_eval_kernel(const EvalParams
         const int64_t k = p.k_begin + (int64_t)(ent & 0xffffffffull);
         const ObjRec rec = p.recs[ri];
         __syncthreads();
-        const double P = block_eval<DEFER_T>(p, rec, freq_of(p.f_min, p.df, k), reinterpret_cast<double*>(smem_raw),
+        const double P = block_eval<DEFER_T, false>(p, rec, freq_of(p.f_min, p.df, k), reinterpret_cast<double*>(smem_raw),
                                              block_slot_len(rec.n), cx, nullptr, nullptr);
         if (threadIdx.x == 0) {
             if (p.pgram) p.pgram[(rec.obj - p.pgram_row0) * p.pgram_row_stride + (k - p.pgram_k0)] = P;

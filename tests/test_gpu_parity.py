@@ -31,7 +31,7 @@ def _tol(ref):
     return RTOL * np.abs(ref) + ATOL
 
 
-def check_parity(cat, pg, ref, mode, max_ambiguous=3, label=""):
+def check_parity(cat, pg, ref, mode, max_ambiguous=3, label="", oracle_opts=None):
     """pg, ref: [n_objects, n_freq].  Returns number of branch-ambiguous evals."""
     assert pg.shape == ref.shape
     both_nan = np.isnan(pg) & np.isnan(ref)
@@ -42,7 +42,8 @@ def check_parity(cat, pg, ref, mode, max_ambiguous=3, label=""):
     for o, k in zip(*np.nonzero(bad)):
         t, y, e = cat.obj(int(o))
         f = oracle.freq(cat.f_min, cat.f_max, cat.n_freq, int(k))
-        r = oracle.eval_one(t, y, e, f, mode=mode, variant=oracle.DEFINITION, alt_threshold=1e-7)
+        r = oracle.eval_one(t, y, e, f, mode=mode, variant=oracle.DEFINITION, alt_threshold=1e-7,
+                            **(oracle_opts or {}))
         if abs(pg[o, k] - r["P"]) <= _tol(r["P"]):
             continue            # the fast oracle was the inexact side; the definition oracle agrees
         if r["margin"] < 1e-9 and abs(pg[o, k] - r["P_alt"]) <= _tol(r["P_alt"]):
@@ -256,9 +257,11 @@ def test_invalid_arguments(ss):
         with pytest.raises(ss.SSError) as ei:
             call(**kw)
         assert ei.value.status == ss.SS_ERR_INVALID_ARG, kw
-    with pytest.raises(ss.SSError) as ei:
-        ss.periodogram(t, y, e, off, 0.1, 2.0, 16, span=0.3)
-    assert ei.value.status == ss.SS_ERR_UNSUPPORTED
+    for kw in (dict(span=-0.1), dict(span=1.5), dict(span=float("nan")), dict(iper=0), dict(iper=3),
+               dict(alpha=float("inf"))):
+        with pytest.raises(ss.SSError) as ei:
+            ss.periodogram(t, y, e, off, 0.1, 2.0, 16, **kw)
+        assert ei.value.status == ss.SS_ERR_INVALID_ARG, kw
 
 
 def test_alpha_option(ss):
@@ -270,6 +273,73 @@ def test_alpha_option(ss):
         ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
                                        cat.n_freq, mode=CV, variant=oracle.DEFINITION, alpha=alpha)
         check_parity(cat, res.pgram, ref, CV, label=f"alpha{alpha}")
+
+
+# ------------------------------------------------------------------ the options Listing 1 has
+LISTING_OPTIONS = [dict(iper=2), dict(span=0.3), dict(iper=2, span=0.3), dict(span=1.0), dict(iper=2, span=1.0),
+                   dict(iper=2, span=0.01), dict(iper=2, alpha=0.0)]
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("opts", LISTING_OPTIONS, ids=lambda o: ",".join(f"{k}={v}" for k, v in o.items()))
+def test_periodic_windows_and_fixed_span(ss, mode, opts):
+    """iper = 2 (windows wrap around phase 0/1) and span > 0 (one smooth at a fixed span,
+    PAPER.md:202-210), alone and combined, on every path class that serves them: config-3-sized objects
+    (shared-memory CTA kernel), config-4-sized objects (both CTA sizes) and the global-staging kernel."""
+    small = ss_inputs.config3(n_objects=40, n_freq=129)
+    ns = np.diff(small.offsets)
+    cat = small.subset(sorted(set(list(range(10)) + [int(np.argmin(ns)), int(np.argmax(ns))])))
+    ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                                   mode=mode, variant=oracle.DEFINITION, **opts)
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
+    assert ss.last_launch_count() > 0
+    check_parity(cat, res.pgram, ref, mode, label=f"cfg3 {opts}", oracle_opts=opts)
+    check_best(ref, res.best_index, res.best_freq, cat)
+    staged = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                            force_path=ss.PATH_STAGE, **opts)
+    check_parity(cat, staged.pgram, ref, mode, label=f"cfg3/stage {opts}", oracle_opts=opts)
+    big = ss_inputs.config4(n_objects=12, n_freq=41)
+    nb = np.diff(big.offsets)
+    cat = big.subset(sorted(set([0, 9, int(np.argmin(nb)), int(np.argmax(nb))])))
+    ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                                   mode=mode, variant=oracle.FAST, **opts)
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
+    check_parity(cat, res.pgram, ref, mode, label=f"cfg4 {opts}", oracle_opts=opts)
+    check_best(ref, res.best_index, res.best_freq, cat)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("n", [5, 6, 7, 8, 33, 100, 257, 1000])
+def test_smooth_values_with_listing_options(ss, mode, n):
+    """One eval, element by element, under each option set; includes duplicated times (tied phases)."""
+    rng = np.random.default_rng(300 + n)
+    t = np.sort(rng.uniform(0, 30, size=n))
+    if n >= 33:
+        t[7] = t[6]
+    y = 15 + 0.4 * np.sin(2 * np.pi * t / 0.61) + rng.normal(0, 0.05, size=n)
+    e = rng.uniform(0.01, 0.2, size=n)
+    for opts in LISTING_OPTIONS:
+        for f in (0.5, 1.639):
+            P, smo, perm = ss.debug_eval(t, y, e, f, mode, **opts)
+            r = oracle.eval_one(t, y, e, f, mode=mode, variant=oracle.DEFINITION, want_smo=True, **opts)
+            assert np.array_equal(perm, r["perm"])
+            if r["margin"] < 1e-9:
+                continue
+            # element bar: 1e-9 mag (7e-11 relative).  A 5-point window (span = 0.01) of heteroscedastic points
+            # can be near-singular in x; prefix-sum differences in fp64 then keep ~10 digits of the slope where
+            # the long-double definition oracle keeps 13.  The north_star bar is the one on P, held exactly.
+            assert np.abs(smo - r["smo"]).max() < 1e-9, (opts, f)
+            assert abs(P - r["P"]) <= _tol(r["P"]), (opts, f)
+
+
+def test_periodic_config5_staging(ss):
+    """n = 20,000 on the global-staging kernel with periodic windows, and with a fixed span."""
+    cat = ss_inputs.make(5).with_grid(n_freq=6)
+    for mode, opts in ((CV, dict(iper=2)), (GV, dict(iper=2)), (CV, dict(iper=2, span=0.1))):
+        ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                                       mode=mode, variant=oracle.FAST, **opts)
+        res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
+        check_parity(cat, res.pgram, ref, mode, label=f"cfg5 {opts}", oracle_opts=opts)
 
 
 # ------------------------------------------------------------------ device-tensor entry point

@@ -358,3 +358,85 @@ def test_forced_branch_alternative_differs_only_when_asked():
     assert np.isnan(r["P_alt"]) and r["margin"] > 0
     r = oracle.eval_one(t, y, e, 3.3, alt_threshold=1e9)
     assert np.isfinite(r["P_alt"]) and r["P_alt"] != r["P"] and abs(r["P_alt"] - r["P"]) < 0.05
+
+
+# ---------------------------------------------------------------- Listing 1's options
+def _periodic_window(x, j, ibw):
+    """indices and abscissae of the periodic window j-ibw .. j+ibw (x wraps by -1 / +1), written out."""
+    n = len(x)
+    idx, xs = [], []
+    for m in range(j - ibw, j + ibw + 1):
+        if m < 0:
+            idx.append(m + n); xs.append(x[m + n] - 1.0)
+        elif m >= n:
+            idx.append(m - n); xs.append(x[m - n] + 1.0)
+        else:
+            idx.append(m); xs.append(x[m])
+    return np.array(idx), np.array(xs)
+
+
+@pytest.mark.parametrize("variant", [DEF, FAST])
+def test_periodic_smooth_is_brute_force_wls_on_wrapped_windows(variant):
+    """jper = 2: the value at x_j is the WLS line over the 2*ibw+1 cyclic neighbours with wrapped
+    abscissae, and the CV residual is the leave-one-out refit on that same window (numpy.polyfit)."""
+    rng = np.random.default_rng(31)
+    for n in (9, 14, 20, 37):
+        x, y, w = _sorted_xyw(rng, n)
+        for span in (0.3, 0.5, 0.8, 1.0):
+            ibw = max(2, int(np.floor(0.5 * span * n + 0.5)))
+            if 2 * ibw + 1 > n:
+                ibw = (n - 1) // 2
+            smo, acvr = oracle.smooth(x, y, w, span, jper=2, cv=True, variant=variant)
+            for j in range(n):
+                idx, xs = _periodic_window(x, j, ibw)
+                b, a = np.polyfit(xs, y[idx], 1, w=np.sqrt(w[idx]))
+                assert abs(smo[j] - (a + b * x[j])) < 1e-9, (n, span, j)
+                keep = idx != j
+                b, a = np.polyfit(xs[keep], y[idx][keep], 1, w=np.sqrt(w[idx][keep]))
+                ref = abs(y[j] - (a + b * x[j]))
+                assert abs(acvr[j] - ref) <= 1e-8 * max(1.0, ref), (n, span, j)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("variant", [DEF, FAST])
+def test_periodic_supsmu_is_rotation_equivariant(mode, variant):
+    """With iper = 2 the phase origin is arbitrary: x -> (x + c) mod 1 (re-sorted) rotates the smooth.
+    (vsmlsq depends on the origin through the quartile points, but only as a threshold.)  The
+    non-periodic smoother does NOT have this property -- checked too, so the pin can fail."""
+    rng = np.random.default_rng(32)
+    n = 120
+    x, y, w = _sorted_xyw(rng, n)
+    y = np.sin(2 * np.pi * x) + 0.1 * rng.normal(size=n)
+    c = 0.37
+    xr = (x + c) % 1.0
+    order = np.argsort(xr, kind="stable")
+    for opts in (dict(), dict(span=0.25), dict(alpha=0.0)):
+        a = oracle.supsmu(x, y, w, mode=mode, iper=2, variant=variant, **opts)
+        b = oracle.supsmu(xr[order], y[order], w[order], mode=mode, iper=2, variant=variant, **opts)
+        assert np.abs(b - a[order]).max() < 1e-9, opts
+    a = oracle.supsmu(x, y, w, mode=mode, iper=1, variant=variant)
+    b = oracle.supsmu(xr[order], y[order], w[order], mode=mode, iper=1, variant=variant)
+    assert np.abs(b - a[order]).max() > 1e-4
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_fixed_span_is_one_smooth_in_both_modes(mode):
+    """span > 0: supsmu returns S(y; span) with ties averaged, whatever the mode, and
+    the periodogram's eval_one uses it; the whole-window span gives the global WLS line."""
+    rng = np.random.default_rng(33)
+    x, y, w = _sorted_xyw(rng, 80)
+    q1 = 80 // 4 - 1; q3 = 3 * (q1 + 1) - 1
+    vs = 1e-6 * (x[q3] - x[q1]) ** 2
+    for iper in (1, 2):
+        for span in (0.1, 0.45):
+            full = oracle.supsmu(x, y, w, mode=mode, iper=iper, span=span)
+            one, _ = oracle.smooth(x, y, w, span, jper=iper, vsmlsq=vs)
+            assert np.array_equal(full, one)
+    smo = oracle.supsmu(x, y, w, mode=mode, span=1.0)          # K clamps to n, window = everything
+    b, a = np.polyfit(x, y, 1, w=np.sqrt(w))
+    assert np.abs(smo - (a + b * x)).max() < 1e-11
+    # fast variant agrees with the definition under the options too
+    for opts in (dict(iper=2), dict(span=0.3), dict(iper=2, span=0.3)):
+        d = oracle.supsmu(x, y, w, mode=mode, variant=DEF, **opts)
+        f = oracle.supsmu(x, y, w, mode=mode, variant=FAST, **opts)
+        assert np.abs(d - f).max() < 1e-10, opts
