@@ -38,6 +38,11 @@ FLOP_PER_POINT_EVAL = {m: 2.0 * s for m, s in SLOTS_PER_POINT_EVAL.items()}
 # Algorithmic on-chip traffic per point-eval: scan arrays written once + window-end
 # reads, 8 B each: 15 + 50 (CV), 6 + 30 (GV) -- the second, co-limiting roofline (shared-memory pipe).
 SMEM_BYTES_PER_POINT_EVAL = {"cv": 520.0, "gv": 288.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE full-size launch of the heaviest CV kernel, from the
+# ncu --set full capture summarised in profiles/r1e_ncu_warp_kernel_cv.md (39.19 MB + 743.67 MB)
+NCU_TRAFFIC_BYTES = 782.86e6
+NCU_TRAFFIC_NOTE = ("bytes of one launch of warp_kernel<4,3,CV> (1,859 objects x 50,000 frequencies, 328 ms under ncu; "
+                    "profiles/r1e_ncu_warp_kernel_cv.md); algorithmic bytes of that launch: 743.6 MB of periodogram rows")
 FP64_LANES_PER_SM = 64          # B200 fp64 pipe: 64 FMA lanes per SM per clock
 N_SM = 148
 
@@ -308,7 +313,8 @@ def run_ours(args):
     achieved = FLOP_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "kernel": "eval kernel (fold+sort+smoother+statistic fused)",
                 "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                "traffic": None, "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} fp64 FMA lanes x 2 x "
+                "traffic": NCU_TRAFFIC_BYTES if (n_obj, n_freq, args.mode) == (10000, 50000, "cv") else None,
+                "traffic_note": NCU_TRAFFIC_NOTE, "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} fp64 FMA lanes x 2 x "
                 f"{sm_max:.0f} MHz ({pk_src} clock); DFMA microbenchmark on this box: {fp64_meas / 1e12:.2f} TFLOP/s, "
                 f"shared memory {smem_meas / 1e12:.2f} TB/s",
                 "flop_per_point_eval": FLOP_PER_POINT_EVAL[args.mode],
