@@ -372,7 +372,8 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
             if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
-            else if (path == SS_PATH_BLOCK) variant = r.n <= 256 ? 3 : (r.n <= 500 ? 0 : (r.n <= 1020 ? 1 : 2));
+            // CTA size by n (profiles/r1f_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
+            else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);
             ClassList& c = find(path, variant);
             c.recs.push_back((int32_t)ri);
             c.max_n = std::max(c.max_n, (int)r.n);
@@ -504,16 +505,14 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
                     int grid = (int)std::min<int64_t>(n_items, sm_count);
                     kern<<<grid, 512, smem, stream>>>(p);
                 } else if (c.variant == 3) {
-                    // short light curves reach this path only through the listing's options or a forced path
-                    auto kern = optk ? block_kernel<128, false, true> : block_kernel<128, false, false>;
+                                        auto kern = optk ? block_kernel<128, false, true> : block_kernel<128, false, false>;
                     SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
                     int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 4);
                     kern<<<grid, 128, smem, stream>>>(p);
                 } else {
                     auto kern = optk ? block_kernel<256, false, true> : block_kernel<256, false, false>;
                     SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                    int per_sm = c.variant == 0 ? 4 : 2;
-                    int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * per_sm);
+                    int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 2);
                     kern<<<grid, 256, smem, stream>>>(p);
                 }
             } else {

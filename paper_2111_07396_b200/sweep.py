@@ -1,0 +1,106 @@
+"""Path-crossover sweep over the light-curve length n (the analogue of the paper's
+kernel-cascade study).
+
+For each n a catalog of equal-length light curves is timed through the device entry point on every path
+class that can serve it (SS_PATH_WARP for n <= 256, SS_PATH_BLOCK for n <= 2,055, SS_PATH_STAGE for any
+n), in both modes; the table reports point-evals/s (n x frequencies x objects / second), which is flat
+where a path scales and drops where it stops fitting.  The path the library picks by itself is marked.
+
+    python -m paper_2111_07396_b200.sweep [--ns 50,100,...] [--target-ms 150] [--md out.md]
+
+Needs a CUDA device (no CPU fallback).  Inputs are synthetic: times uniform over 30 nights (8 h per
+night), a sinusoid of random period plus Gaussian noise; the arithmetic under test is all in the library.
+"""
+from __future__ import annotations
+
+import argparse
+import sys
+
+import numpy as np
+
+from . import (CROSS_VALIDATION, GENERALIZED_VALIDATION, PATH_BLOCK, PATH_STAGE, PATH_WARP, default_options, load,
+               path_for_n, ss_periodogram)
+
+DEFAULT_NS = [50, 64, 96, 128, 160, 200, 256, 257, 320, 400, 512, 700, 1000, 1400, 2055, 2056, 3000, 5000, 10000, 20000]
+PATH_NAME = {PATH_WARP: "warp", PATH_BLOCK: "cta-smem", PATH_STAGE: "cta-staged"}
+WARP_MAX_N, BLOCK_MAX_N = 256, 2055
+
+
+def catalog(n: int, n_objects: int, seed: int):
+    rng = np.random.default_rng(seed)
+    t = np.sort(rng.integers(0, 30, size=(n_objects, n)) + rng.uniform(0.0, 0.33, size=(n_objects, n)), axis=1)
+    period = np.exp(rng.uniform(np.log(0.1), np.log(2.0), size=(n_objects, 1)))
+    y = 15.0 + 0.4 * np.sin(2 * np.pi * t / period) + rng.normal(0.0, 0.05, size=(n_objects, n))
+    e = np.full((n_objects, n), 0.05)
+    off = np.arange(n_objects + 1, dtype=np.int64) * n
+    return t.ravel(), y.ravel(), e.ravel(), off
+
+
+def time_call(torch, dev, arrs, n_objects, n_freq, mode, path, reps=3):
+    t, y, e, off = arrs
+    pg = torch.empty((n_objects, n_freq), dtype=torch.float64, device=dev)
+    bi = torch.empty(n_objects, dtype=torch.int64, device=dev)
+    opt = default_options(force_path=path, skip_validation=1)
+
+    def call():
+        ss_periodogram(t, y, e, off, n_objects, 0.5, 24.0, n_freq, mode, pg, None, bi, opt)
+
+    call()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    best = float("inf")
+    for _ in range(reps):
+        torch.cuda.synchronize()
+        ev[0].record()
+        call()
+        ev[1].record()
+        torch.cuda.synchronize()
+        best = min(best, ev[0].elapsed_time(ev[1]))
+    return best
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--ns", default=",".join(map(str, DEFAULT_NS)))
+    ap.add_argument("--target-ms", type=float, default=150.0, help="aim each timed call at about this long")
+    ap.add_argument("--md", default=None, help="also write the table as markdown to this file")
+    args = ap.parse_args(argv)
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("sweep needs a CUDA device (the library has no CPU path)")
+    load()
+    dev = torch.device("cuda")
+    lines = ["| n | path | auto | objects x frequencies | CV point-evals/s | CV evals/s | GV point-evals/s | GV evals/s |",
+             "|---|---|---|---|---|---|---|---|"]
+    for n in [int(v) for v in args.ns.split(",")]:
+        paths = [p for p in (PATH_WARP, PATH_BLOCK, PATH_STAGE)
+                 if (p != PATH_WARP or n <= WARP_MAX_N) and (p != PATH_BLOCK or n <= BLOCK_MAX_N)]
+        auto = path_for_n(n)
+        for path in paths:
+            # size the call: enough (object, frequency) items to fill 148 SMs several times over
+            n_objects = 296 if n <= 2055 else 8
+            arrs_h = catalog(n, n_objects, seed=1000 + n)
+            arrs = tuple(torch.as_tensor(a, device=dev) for a in arrs_h)
+            row = []
+            for mode in (CROSS_VALIDATION, GENERALIZED_VALIDATION):
+                # grow the grid until one call lasts about target-ms (the per-call overhead -- workspace
+                # allocation, one host sync -- is about a millisecond and must not dominate)
+                nf, ms = 64, 0.0
+                for _ in range(6):
+                    ms = time_call(torch, dev, arrs, n_objects, nf, mode, path, reps=2)
+                    if ms >= 0.5 * args.target_ms or nf >= 400000:
+                        break
+                    nf = int(min(400000, max(2 * nf, nf * args.target_ms / max(ms, 0.05))))
+                ms = time_call(torch, dev, arrs, n_objects, nf, mode, path)
+                ev = n_objects * nf / (ms * 1e-3)
+                row.append((nf, ev * n, ev))
+            lines.append(f"| {n} | {PATH_NAME[path]} | {'*' if path == auto else ''} | {n_objects} x {row[0][0]} / {row[1][0]} | "
+                         f"{row[0][1]:.3g} | {row[0][2]:.3g} | {row[1][1]:.3g} | {row[1][2]:.3g} |")
+            print(lines[-1], flush=True)
+    if args.md:
+        with open(args.md, "w") as f:
+            f.write("\n".join(lines) + "\n")
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
