@@ -150,23 +150,23 @@ __device__ __forceinline__ void cex(unsigned long long* key, unsigned int* idx, 
     }
 }
 
-// ---- fast sort: packed (phase bits | index) 64-bit keys in registers --------------------------------
+// ---- fast sort: packed 32-bit keys (quantised phase | index) in registers --------------------------
 // S keys per thread, blocked (position = tid*S + s).  Warp-local phases run on registers and shuffles,
-// only the log2(NW)*(log2(NW)+1)/2 cross-warp steps go through shared memory.  The low IDX_BITS mantissa
-// bits of the phase give way to the index, so the order is exact unless two phases agree in all the
-// bits kept and disagree below: the caller checks the gathered phases and falls back to the exact
-// network then.
-constexpr int FAST_IDX_BITS = 12;
-constexpr unsigned long long FAST_IDX_MASK = (1ull << FAST_IDX_BITS) - 1ull;
-
-__device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int m)
-{
-    return __shfl_xor_sync(0xffffffffu, v, m);
-}
+// only the log2(NW)*(log2(NW)+1)/2 cross-warp steps go through shared memory.  A key keeps the top
+// 32 - IDX_BITS bits of the phase, so the network leaves the points in exact order except inside a
+// quantisation bucket (phases that agree in all the bits kept: a pair every few evals), where they sit
+// in index order; block_eval restores the exact order there by odd-even transposition on the full
+// 64-bit phases, and falls back to the exact network if that does not settle.  A 32-bit key costs one
+// shuffle and one min/max per exchange where the 64-bit key cost two shuffles and a compare-select chain.
+template <int T> struct FastKey {
+    static constexpr int IDX_BITS = T <= 128 ? 10 : (T <= 256 ? 11 : 12);      // log2(8 T) positions
+    static constexpr unsigned IDX_MASK = (1u << IDX_BITS) - 1u;
+    static constexpr double PHASE_SCALE = (double)(1u << (32 - IDX_BITS));
+};
 
 // the halving steps of one merge phase inside a warp: lane strides 16..1, then register strides S/2..1
 template <int S>
-__device__ __forceinline__ void merge_tail64(unsigned long long (&key)[S], int lane, int first_lane_stride)
+__device__ __forceinline__ void merge_tail32(unsigned (&key)[S], int lane, int first_lane_stride)
 {
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) {
@@ -174,7 +174,7 @@ __device__ __forceinline__ void merge_tail64(unsigned long long (&key)[S], int l
         const bool lower = (lane & m) == 0;
 #pragma unroll
         for (int s = 0; s < S; s++) {
-            const unsigned long long o = shfl_xor_u64(key[s], m);
+            const unsigned o = __shfl_xor_sync(0xffffffffu, key[s], m);
             key[s] = lower ? min(key[s], o) : max(key[s], o);
         }
     }
@@ -183,7 +183,7 @@ __device__ __forceinline__ void merge_tail64(unsigned long long (&key)[S], int l
 #pragma unroll
         for (int s = 0; s < S; s++)
             if ((s & j) == 0) {
-                const unsigned long long lo = min(key[s], key[s + j]), hi = max(key[s], key[s + j]);
+                const unsigned lo = min(key[s], key[s + j]), hi = max(key[s], key[s + j]);
                 key[s] = lo; key[s + j] = hi;
             }
     }
@@ -191,7 +191,7 @@ __device__ __forceinline__ void merge_tail64(unsigned long long (&key)[S], int l
 
 // sorts the 32*S keys of each warp ascending (blocked within the warp: position = lane*S + s)
 template <int S>
-__device__ __forceinline__ void warp_sort64(unsigned long long (&key)[S], int lane)
+__device__ __forceinline__ void warp_sort32(unsigned (&key)[S], int lane)
 {
 #pragma unroll
     for (int k = 2; k <= 32 * S; k <<= 1) {
@@ -200,7 +200,7 @@ __device__ __forceinline__ void warp_sort64(unsigned long long (&key)[S], int la
             for (int s = 0; s < S; s++) {
                 const int t = s ^ (k - 1);
                 if (t > s) {
-                    const unsigned long long lo = min(key[s], key[t]), hi = max(key[s], key[t]);
+                    const unsigned lo = min(key[s], key[t]), hi = max(key[s], key[t]);
                     key[s] = lo; key[t] = hi;
                 }
             }
@@ -209,39 +209,38 @@ __device__ __forceinline__ void warp_sort64(unsigned long long (&key)[S], int la
 #pragma unroll
                 for (int s = 0; s < S; s++)
                     if ((s & j) == 0) {
-                        const unsigned long long lo = min(key[s], key[s + j]), hi = max(key[s], key[s + j]);
+                        const unsigned lo = min(key[s], key[s + j]), hi = max(key[s], key[s + j]);
                         key[s] = lo; key[s + j] = hi;
                     }
             }
         } else {
             const int m = k / S - 1;               // lane mask of the mirror step
             const bool lower = (lane & (k / S / 2)) == 0;
-            unsigned long long other[S];
+            unsigned other[S];
 #pragma unroll
-            for (int s = 0; s < S; s++) other[s] = shfl_xor_u64(key[S - 1 - s], m);
+            for (int s = 0; s < S; s++) other[s] = __shfl_xor_sync(0xffffffffu, key[S - 1 - s], m);
 #pragma unroll
             for (int s = 0; s < S; s++) key[s] = lower ? min(key[s], other[s]) : max(key[s], other[s]);
-            merge_tail64<S>(key, lane, k / S / 4);
+            merge_tail32<S>(key, lane, k / S / 4);
         }
     }
 }
 
-// Whole-CTA sort; writes the sorted permutation idx[0..n).  kbuf: T*S words of exchange space.
+// Whole-CTA sort; writes the (bucket-exact) sorted permutation idx[0..n).  kbuf: T*S words of exchange space.
 template <int T, int S>
-__device__ __forceinline__ void block_sort_fast(int n, const double* tt, double f, unsigned long long* kbuf,
-                                                unsigned int* idx)
+__device__ __forceinline__ void block_sort_fast(int n, const double* tt, double f, unsigned* kbuf, unsigned int* idx)
 {
     constexpr int NW = T / 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    unsigned long long key[S];
+    unsigned key[S];
 #pragma unroll
     for (int s = 0; s < S; s++) {
         const int i = tid + T * s;
-        key[s] = ~0ull;
+        key[s] = 0xffffffffu;
         if (i < n)
-            key[s] = ((unsigned long long)__double_as_longlong(fold_phase(tt[i], f)) & ~FAST_IDX_MASK) | (unsigned long long)i;
+            key[s] = (__double2uint_rz(fold_phase(tt[i], f) * FastKey<T>::PHASE_SCALE) << FastKey<T>::IDX_BITS) | (unsigned)i;
     }
-    warp_sort64<S>(key, lane);
+    warp_sort32<S>(key, lane);
 #pragma unroll
     for (int kw = 2; kw <= NW; kw <<= 1) {
         // mirror step across warps: partner position = pos ^ (kw*32*S - 1)
@@ -253,7 +252,7 @@ __device__ __forceinline__ void block_sort_fast(int n, const double* tt, double 
             __syncthreads();
 #pragma unroll
             for (int s = 0; s < S; s++) {
-                const unsigned long long o = kbuf[(S - 1 - s) * T + ptid];
+                const unsigned o = kbuf[(S - 1 - s) * T + ptid];
                 key[s] = lower ? min(key[s], o) : max(key[s], o);
             }
             __syncthreads();
@@ -267,17 +266,17 @@ __device__ __forceinline__ void block_sort_fast(int n, const double* tt, double 
             __syncthreads();
 #pragma unroll
             for (int s = 0; s < S; s++) {
-                const unsigned long long o = kbuf[s * T + ptid];
+                const unsigned o = kbuf[s * T + ptid];
                 key[s] = lower ? min(key[s], o) : max(key[s], o);
             }
             __syncthreads();
         }
-        merge_tail64<S>(key, lane, 16);
+        merge_tail32<S>(key, lane, 16);
     }
 #pragma unroll
     for (int s = 0; s < S; s++) {
         const int pos = tid * S + s;
-        if (pos < n) idx[pos] = (unsigned int)(key[s] & FAST_IDX_MASK);
+        if (pos < n) idx[pos] = key[s] & FastKey<T>::IDX_MASK;
     }
 }
 
@@ -350,22 +349,26 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
     // sort scratch overlays slots that are dead until pass 1: exact keys / exchange buffer in r0..r1,
     // the sorted permutation in A2, the sorted phases in A0
     unsigned long long* key = reinterpret_cast<unsigned long long*>(r0);
+    unsigned* kbuf = reinterpret_cast<unsigned*>(r0);
     unsigned int* idx = reinterpret_cast<unsigned int*>(A2);
     double* phi = A0;
+    auto misordered = [&](int j) {      // exact stable order (R13): by phase, ties by input index
+        return phi[j + 1] < phi[j] || (phi[j + 1] == phi[j] && idx[j + 1] < idx[j]);
+    };
 
-    // fast path: packed keys in registers (S per thread); needs T*S exchange words inside r0..r1
+    // fast path: packed 32-bit keys in registers (S per thread); needs T*S exchange words inside r0..r1
     int fs = 0;
-    if (n <= T * 8 && n <= (int)FAST_IDX_MASK) {
+    if (n <= T * 8) {
         fs = 1;
         while (T * fs < n) fs <<= 1;
-        if ((int64_t)T * fs > 2 * sl) fs = 0;
+        if ((int64_t)T * fs > 4 * sl) fs = 0;
     }
     for (;;) {
         if (tid < 4) cx.flags[tid] = 0;
-        if (fs == 1) block_sort_fast<T, 1>(n, tt, f, key, idx);
-        else if (fs == 2) block_sort_fast<T, 2>(n, tt, f, key, idx);
-        else if (fs == 4) block_sort_fast<T, 4>(n, tt, f, key, idx);
-        else if (fs == 8) block_sort_fast<T, 8>(n, tt, f, key, idx);
+        if (fs == 1) block_sort_fast<T, 1>(n, tt, f, kbuf, idx);
+        else if (fs == 2) block_sort_fast<T, 2>(n, tt, f, kbuf, idx);
+        else if (fs == 4) block_sort_fast<T, 4>(n, tt, f, kbuf, idx);
+        else if (fs == 8) block_sort_fast<T, 8>(n, tt, f, kbuf, idx);
         else {
             // ---- exact path: P1 fold + key init
             for (int j = tid; j < n; j += T) {
@@ -397,26 +400,42 @@ __device__ double block_eval(const EvalParams& p, const ObjRec& rec, double f, d
             }
         }
         __syncthreads();
-        // ---- gather: exact phases again from the permutation, x centred by 0.5,
-        // y already centred by ybar_w
-        for (int j = tid; j < n; j += T) {
-            const unsigned int i = idx[j];
-            const double ph = fold_phase(tt[i], f);
-            phi[j] = ph;
-            x[j] = ph - 0.5;
-            ys[j] = yc[i];
-            ws[j] = wo[i];
-            if (perm_dbg) perm_dbg[j] = (int32_t)i;
-        }
+        // ---- the exact phases again, in the sorted order
+        for (int j = tid; j < n; j += T) phi[j] = fold_phase(tt[idx[j]], f);
         __syncthreads();
-        for (int j = tid; j + 1 < n; j += T) {
-            if (phi[j + 1] == phi[j]) cx.flags[0] = 1;                                   // tie (stable by index)
-            if (phi[j + 1] < phi[j] || (phi[j + 1] == phi[j] && idx[j + 1] < idx[j])) cx.flags[1] = 1;   // truncated keys misordered
+        if (fs != 0) {
+            // points whose phases share a quantisation bucket sit in index order: odd-even transposition on
+            // the full phases puts them in exact order (a bucket of m points settles in m passes); buckets
+            // that do not settle in 12 passes send the eval to the exact network
+            bool settled = false;
+            for (int it = 0; it < 6; it++) {
+#pragma unroll
+                for (int parity = 0; parity < 2; parity++) {
+                    for (int j = 2 * tid + parity; j + 1 < n; j += 2 * T)
+                        if (misordered(j)) {
+                            const double pa = phi[j]; phi[j] = phi[j + 1]; phi[j + 1] = pa;
+                            const unsigned ia = idx[j]; idx[j] = idx[j + 1]; idx[j + 1] = ia;
+                            cx.flags[1] = it + 1;
+                        }
+                    __syncthreads();
+                }
+                if (cx.flags[1] != it + 1) { settled = true; break; }
+                __syncthreads();      // everyone has read the stamp before the next pass may overwrite it
+            }
+            if (!settled) { fs = 0; __syncthreads(); continue; }
         }
-        __syncthreads();
-        if (fs != 0 && cx.flags[1] != 0) { fs = 0; __syncthreads(); continue; }        // redo with the exact network
         break;
     }
+    // ---- gather: x centred by 0.5, y already centred by ybar_w
+    for (int j = tid; j < n; j += T) {
+        const unsigned int i = idx[j];
+        x[j] = phi[j] - 0.5;
+        ys[j] = yc[i];
+        ws[j] = wo[i];
+        if (perm_dbg) perm_dbg[j] = (int32_t)i;
+        if (j + 1 < n && phi[j + 1] == phi[j]) cx.flags[0] = 1;              // tie: equal-x run averaging (R24)
+    }
+    __syncthreads();
     const bool has_ties = cx.flags[0] != 0;
     __syncthreads();
     if (tid == 1) cx.flags[1] = 0;

@@ -241,6 +241,43 @@ def test_equal_phases_and_tied_runs(ss, mode):
         check_parity(cat, res.pgram, ref, mode, label=f"ties/path{path}")
 
 
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_phase_clusters_below_the_sort_key_resolution(ss, mode):
+    """The CTA kernels sort 32-bit keys (20-22 phase bits | index) and repair the order inside a quantisation
+    bucket on the full phases.  Observation times 1e-9 d apart fold into one bucket with DISTINCT phases.
+    (a) a reversed triple and a reversed pair (repaired by odd-even transposition): full parity at the bar;
+    (b) plus a 40-point burst in reverse time order (does not settle in 12 passes -> exact network): the
+    permutation equals the oracle's bit for bit, and every CTA size gives the same values.  (With 40
+    coincident abscissae the fits themselves are ill-conditioned -- a 7-point window holding 6 of them leaves
+    the seventh a leave-one-out denominator of 0 up to rounding -- so (b) pins the ORDER, not the values.)"""
+    rng = np.random.default_rng(77)
+    for n, path_list in ((700, (ss.PATH_AUTO, ss.PATH_STAGE)), (120, (ss.PATH_AUTO, ss.PATH_BLOCK))):
+        t = np.sort(rng.uniform(0, 40, size=n))
+        t[10:13] = t[10] + np.array([2e-9, 1e-9, 0.0])                # triple, reversed
+        t[30:32] = t[30] + np.array([1e-9, 0.0])                      # pair, reversed
+        y = 15 + 0.3 * np.sin(2 * np.pi * t / 0.7) + rng.normal(0, 0.05, size=n)
+        e = rng.uniform(0.02, 0.1, size=n)
+        off = np.array([0, n], dtype=np.int64)
+        cat = ss_inputs.Catalog("clusters", t, y, e, off, 0.2, 3.0, 64, np.array([1 / 0.7]))
+        ref, _, _ = oracle.periodogram(t, y, e, off, 0.2, 3.0, 64, mode=mode, variant=oracle.DEFINITION)
+        for path in path_list:
+            res = ss.periodogram(t, y, e, off, 0.2, 3.0, 64, mode, force_path=path)
+            check_parity(cat, res.pgram, ref, mode, label=f"clusters n={n} path{path}")
+        # (b) the burst
+        tb = t.copy()
+        tb[60:100] = tb[60] + 1e-9 * np.arange(40)[::-1]
+        Pk = []
+        for k in (3, 17, 40):
+            f = oracle.freq(0.2, 3.0, 64, k)
+            P, smo, perm = ss.debug_eval(tb, y, e, f, mode)            # 512-thread CTA
+            r = oracle.eval_one(tb, y, e, f, mode=mode, variant=oracle.DEFINITION, want_smo=True)
+            assert np.array_equal(perm, r["perm"])
+            Pk.append(P)
+        for path in path_list:                                        # 128- / 256-thread CTAs, deferred hand-over
+            res = ss.periodogram(tb, y, e, off, 0.2, 3.0, 64, mode, force_path=path)
+            assert np.allclose(res.pgram[0, [3, 17, 40]], Pk, rtol=1e-9, atol=1e-12), (n, path)
+
+
 def test_invalid_arguments(ss):
     t = np.linspace(0, 10, 20); y = np.sin(t); e = np.full(20, 0.1)
     off = np.array([0, 20], dtype=np.int64)
