@@ -372,7 +372,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
             if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
-            // CTA size by n (profiles/r1f_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
+            // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
             else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);
             ClassList& c = find(path, variant);
             c.recs.push_back((int32_t)ri);
