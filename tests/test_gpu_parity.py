@@ -459,3 +459,43 @@ def test_config3_full_size_sampled(ss, mode):
                bf[torch.as_tensor(rows, device=dev)].cpu().numpy(), sub)
     del pg
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("cfg", [2, 5])
+def test_single_object_configs_full_size_sampled(ss, cfg, mode):
+    """Configs 2 (n = 1,000 x 100,000 frequencies, shared-memory CTA kernel) and 5 (n = 20,000 x 1,000,000
+    frequencies, global-staging kernel) at BASELINE.json's full sizes through the device entry point; checked on
+    properties that hold at any size and on sampled evals the oracle computes one by one (its fp64 variant, itself
+    held to the long-double variant by the pins and by the reduced-size tests above)."""
+    import torch
+    cat = ss_inputs.make(cfg)
+    assert cat.n_freq == {2: 100000, 5: 1000000}[cfg]
+    dev = torch.device("cuda")
+    t = torch.as_tensor(cat.times, device=dev); y = torch.as_tensor(cat.mags, device=dev)
+    e = torch.as_tensor(cat.errs, device=dev); off = torch.as_tensor(cat.offsets, device=dev)
+    pg = torch.empty((1, cat.n_freq), dtype=torch.float64, device=dev)
+    bf = torch.empty(1, dtype=torch.float64, device=dev); bi = torch.empty(1, dtype=torch.int64, device=dev)
+    ss.ss_periodogram(t, y, e, off, 1, cat.f_min, cat.f_max, cat.n_freq, mode, pg, bf, bi)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(pg).all()) and float(pg.max()) <= 1.0 + 1e-12
+    assert int(torch.argmax(pg[0])) == int(bi[0])
+    kb = int(bi[0])
+    assert float(bf[0]) == oracle.freq(cat.f_min, cat.f_max, cat.n_freq, kb)
+    # the injected period (or a harmonic / the 1-day alias structure around it) carries the highest power
+    f_true = {2: 1 / 2.71, 5: 1 / 0.853}[cfg]
+    ratio = float(bf[0]) / f_true
+    assert min(abs(ratio - r) for r in (0.5, 1.0, 2.0, 3.0, 4.0)) < 0.02, ratio
+    rng = np.random.default_rng(cfg)
+    ks = np.unique(np.concatenate([rng.integers(0, cat.n_freq, size=60 if cfg == 2 else 24), [0, cat.n_freq - 1, kb]]))
+    got = pg[0, torch.as_tensor(ks, device=dev)].cpu().numpy()
+    tt, yy, ee = cat.obj(0)
+    ambiguous = 0
+    for k, g in zip(ks, got):
+        r = oracle.eval_one(tt, yy, ee, oracle.freq(cat.f_min, cat.f_max, cat.n_freq, int(k)), mode=mode,
+                            variant=oracle.FAST, alt_threshold=1e-7)
+        if abs(g - r["P"]) <= _tol(r["P"]):
+            continue
+        assert r["margin"] < 1e-9 and abs(g - r["P_alt"]) <= _tol(r["P_alt"]), (cfg, k, g, r["P"], r["margin"])
+        ambiguous += 1
+    assert ambiguous <= 2
