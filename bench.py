@@ -61,6 +61,7 @@ def parse():
     ap.add_argument("--iper", type=int, default=1, help="(sweep) 2 = periodic windows, PAPER.md:199-200")
     ap.add_argument("--span", type=float, default=0.0, help="(sweep) > 0 = fixed span, PAPER.md:202-210")
     ap.add_argument("--path", type=int, default=0, help="(sweep) force a path class: 1 warp, 2 CTA, 3 staging")
+    ap.add_argument("--no-clocks", action="store_true", help="(debug) do not sample nvidia-smi during the run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -88,7 +89,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "500",
                  "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -257,7 +258,7 @@ def run_ours(args):
         ss.ss_periodogram(t, y, e, off, n_obj, cat.f_min, cat.f_max, n_freq, m, pg, bf, bi, o)
 
     sampler = ClockSampler(local)
-    if rank == 0:
+    if rank == 0 and not args.no_clocks:
         sampler.start()
     for _ in range(args.warmup):
         step()
@@ -283,13 +284,15 @@ def run_ours(args):
     other = ss.GENERALIZED_VALIDATION if mode == ss.CROSS_VALIDATION else ss.CROSS_VALIDATION
     step(other); step(other)
     torch.cuda.synchronize()
-    o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    o0.record(stream)
-    for _ in range(2):
+    other_times = []
+    for _ in range(3):                      # median of three single steps (reported, not the headline)
+        o0, o1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        o0.record(stream)
         step(other)
-    o1.record(stream)
-    torch.cuda.synchronize()
-    other_ms = o0.elapsed_time(o1) / 2
+        o1.record(stream)
+        torch.cuda.synchronize()
+        other_times.append(o0.elapsed_time(o1))
+    other_ms = sorted(other_times)[1]
 
     # ---- e2e: host buffers through ss_periodogram_host, copies inside the timed region
     e2e = None

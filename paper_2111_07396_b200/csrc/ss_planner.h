@@ -50,15 +50,22 @@ constexpr unsigned int DEFER_CAPACITY = 1u << 20;   // evals the warp path may d
 constexpr int STAGE_CTAS = 148 * 2;      // persistent CTAs of the STAGE path (2 per SM)
 constexpr int64_t MIN_CHUNK = 1;          // smallest frequency chunk a work item may cover
 
-// Work items are (object, frequency chunk); aim at >= TARGET_ITEMS items per tile so that
-// persistent CTAs / the hardware scheduler can balance ragged objects.
-constexpr int64_t TARGET_ITEMS = 16384;
+// Work items are (object, frequency chunk).  Launches are per path class (about a tenth of a ragged catalog
+// each), so aim at >= TARGET_ITEMS items per tile: the last wave of a launch is then a per-cent of it, not a
+// tenth (config 3: 16,384 -> 131,072 items bought 3 % CV, 3.6 % GV; 262,144 no more).  Items keep at least 8
+// frequencies each while that still leaves >= 4,096 of them (a single long light curve).
+constexpr int64_t TARGET_ITEMS = 131072;
 inline int64_t chunks_per_object(int64_t n_objects_in_tile, int64_t freq_per_tile)
 {
     if (n_objects_in_tile < 1) n_objects_in_tile = 1;
     int64_t c = (TARGET_ITEMS + n_objects_in_tile - 1) / n_objects_in_tile;
     if (c > freq_per_tile) c = freq_per_tile;
-    return c < 1 ? 1 : c;
+    if (c < 1) c = 1;
+    if (freq_per_tile / c < 8) {
+        const int64_t c8 = freq_per_tile / 8 > 1 ? freq_per_tile / 8 : 1;
+        if (c8 * n_objects_in_tile >= 4096) c = c8;
+    }
+    return c;
 }
 
 struct PlanInput {
