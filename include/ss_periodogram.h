@@ -172,6 +172,11 @@ int64_t ss_last_launch_count(void);
 double ss_last_kernel_ms(void);
 int64_t ss_last_kernel_count(void);
 
+/* The library keeps the device buffers, events and the copy stream of a thread's most recent calls for
+ * reuse by its next call (a call in steady state makes no cudaMalloc/cudaFree; at most 4 buffers per thread:
+ * workspace, and for the host entry point the catalog copy and two output tiles).  This frees them. */
+void ss_release_workspace(void);
+
 const char *ss_last_error(void); /* thread-local, never NULL */
 int ss_version(void);
 

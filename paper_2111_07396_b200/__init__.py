@@ -24,7 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libss_b200.so")
 EXPORTS = ["ss_default_options", "ss_periodogram", "ss_periodogram_ex", "ss_periodogram_host",
            "ss_plan", "ss_workspace_bytes", "ss_paper_footprint_bytes", "ss_paper_batches",
            "ss_path_for_n", "ss_debug_eval", "ss_microbench", "ss_last_launch_count", "ss_last_kernel_ms", "ss_last_kernel_count",
-           "ss_last_error", "ss_version"]
+           "ss_last_error", "ss_version", "ss_release_workspace"]
 
 
 class SSError(RuntimeError):
@@ -82,6 +82,7 @@ def load():
     L.ss_last_kernel_count.restype = i64
     L.ss_last_error.restype = C.c_char_p
     L.ss_version.restype = C.c_int
+    L.ss_release_workspace.restype = None
     _lib = L
     return L
 
@@ -99,6 +100,11 @@ def default_options(**kw) -> Options:
             raise TypeError(f"unknown option {k}")
         setattr(o, k, v)
     return o
+
+
+def release_workspace() -> None:
+    """Free the device buffers the library caches between calls of this thread (ss_release_workspace)."""
+    load().ss_release_workspace()
 
 
 def version() -> int:

@@ -41,6 +41,88 @@ static ss_status_t fail(ss_status_t st, const char* fmt, ...)
     } while (0)
 
 // ------------------------------------------------------------------------------------------------
+// Per-thread device resources kept between calls: a call in steady state makes no cudaMalloc / cudaFree /
+// event or stream creation (each of those enters the driver's resource manager, where it can queue behind
+// other clients of the GPU -- measured: up to 0.4 s per call while nvidia-smi polls the device).  The pool
+// holds at most POOL_SLOTS buffers; ss_release_workspace() frees everything.
+// ------------------------------------------------------------------------------------------------
+constexpr int POOL_SLOTS = 4;
+struct DevicePool {
+    struct Buf { char* p = nullptr; size_t bytes = 0; int dev = -1; };
+    Buf bufs[POOL_SLOTS];
+    std::vector<cudaEvent_t> timing_events, plain_events;
+    cudaStream_t copy_stream = nullptr;
+    int copy_stream_dev = -1;
+
+    // smallest cached buffer of this device that is large enough, else a fresh allocation
+    cudaError_t acquire(size_t bytes, char** out)
+    {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        int best = -1;
+        for (int i = 0; i < POOL_SLOTS; i++)
+            if (bufs[i].p && bufs[i].dev == dev && bufs[i].bytes >= bytes && (best < 0 || bufs[i].bytes < bufs[best].bytes)) best = i;
+        if (best >= 0 && bufs[best].bytes <= 2 * bytes + (64u << 20)) {      // do not pin a huge buffer on a small request
+            *out = bufs[best].p;
+            bufs[best] = Buf{};
+            return cudaSuccess;
+        }
+        e = cudaMalloc((void**)out, bytes);
+        if (e == cudaErrorMemoryAllocation) {      // make room: drop the cache and try once more
+            release_all();
+            cudaGetLastError();
+            e = cudaMalloc((void**)out, bytes);
+        }
+        return e;
+    }
+    void release(char* p, size_t bytes)
+    {
+        if (!p) return;
+        int dev = 0;
+        cudaGetDevice(&dev);
+        int slot = -1;
+        for (int i = 0; i < POOL_SLOTS; i++) if (!bufs[i].p) { slot = i; break; }
+        if (slot < 0) {                            // full: evict the smallest
+            slot = 0;
+            for (int i = 1; i < POOL_SLOTS; i++) if (bufs[i].bytes < bufs[slot].bytes) slot = i;
+            if (bufs[slot].bytes >= bytes) { cudaFree(p); return; }
+            cudaFree(bufs[slot].p);
+        }
+        bufs[slot] = Buf{p, bytes, dev};
+    }
+    cudaError_t event(bool timing, cudaEvent_t* out)
+    {
+        auto& v = timing ? timing_events : plain_events;
+        if (!v.empty()) { *out = v.back(); v.pop_back(); return cudaSuccess; }
+        return timing ? cudaEventCreate(out) : cudaEventCreateWithFlags(out, cudaEventDisableTiming);
+    }
+    void event_back(bool timing, cudaEvent_t e) { if (e) (timing ? timing_events : plain_events).push_back(e); }
+    cudaError_t stream(cudaStream_t* out)
+    {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (copy_stream && copy_stream_dev != dev) { cudaStreamDestroy(copy_stream); copy_stream = nullptr; }
+        if (!copy_stream) {
+            cudaError_t e = cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking);
+            if (e != cudaSuccess) return e;
+            copy_stream_dev = dev;
+        }
+        *out = copy_stream;
+        return cudaSuccess;
+    }
+    void release_all()
+    {
+        for (auto& b : bufs) { if (b.p) cudaFree(b.p); b = Buf{}; }
+        for (auto e : timing_events) cudaEventDestroy(e);
+        for (auto e : plain_events) cudaEventDestroy(e);
+        timing_events.clear(); plain_events.clear();
+        if (copy_stream) { cudaStreamDestroy(copy_stream); copy_stream = nullptr; }
+    }
+};
+static thread_local DevicePool g_pool;
+
+// ------------------------------------------------------------------------------------------------
 // P0 prep: tt = t - min t, w = e^-2, ybar_w, chi0; yc = y - ybar_w.
 // One CTA per object.  Also validates: finite t, y, e and e > 0 (flag[0] |= 1 otherwise).
 // ------------------------------------------------------------------------------------------------
@@ -259,8 +341,10 @@ struct Engine {
 
     ~Engine()
     {
-        for (auto& e : prof) { cudaEventDestroy(e.first); cudaEventDestroy(e.second); }
-        if (ws) cudaFree(ws);
+        // pooled buffers must be idle when they go back (already true unless the call is failing)
+        if (ws) cudaStreamSynchronize(stream);
+        for (auto& e : prof) { g_pool.event_back(true, e.first); g_pool.event_back(true, e.second); }
+        g_pool.release(ws, ws_bytes);
     }
     // After the stream is synchronised: did the deferred list overflow?
     bool defer_overflowed()
@@ -409,7 +493,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     ws_bytes = b;
     if (ws_bytes > cap + (64 << 20))
         return fail(SS_ERR_OUT_OF_MEMORY, "workspace %zu B exceeds the cap %zu B", ws_bytes, cap);
-    SS_CUDA(cudaMalloc((void**)&ws, ws_bytes));
+    SS_CUDA(g_pool.acquire(ws_bytes, &ws));
     tt = (double*)(ws + o_tt); yc = (double*)(ws + o_yc); w = (double*)(ws + o_w);
     d_recs = (ObjRec*)(ws + o_recs); d_list = (int32_t*)(ws + o_list); d_degen = (int64_t*)(ws + o_deg);
     best_val = (double*)(ws + o_bv); best_idx = (int64_t*)(ws + o_bi);
@@ -483,8 +567,8 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (opt.profile) {
-            SS_CUDA(cudaEventCreate(&ev0));
-            SS_CUDA(cudaEventCreate(&ev1));
+            SS_CUDA(g_pool.event(true, &ev0));
+            SS_CUDA(g_pool.event(true, &ev1));
             prof.emplace_back(ev0, ev1);
         }
         if (c.path != SS_PATH_WARP) {
@@ -592,6 +676,7 @@ void ss_default_options(ss_options_t* opt)
 }
 
 const char* ss_last_error(void) { return g_err.c_str(); }
+void ss_release_workspace(void) { g_pool.release_all(); }
 int ss_version(void) { return SS_VERSION; }
 int64_t ss_last_launch_count(void) { return g_launches; }
 double ss_last_kernel_ms(void) { return g_kernel_ms; }
@@ -703,8 +788,9 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
     const size_t out_b = align_up(8 * (size_t)n_objects);
     // the raw copy must exist before setup() runs the prep kernel: allocate it separately first
     char* raw = nullptr;
-    SS_CUDA(cudaMalloc((void**)&raw, 3 * raw_b + 2 * out_b + 256));
-    struct Guard { char* p; ~Guard() { if (p) cudaFree(p); } } guard{raw};
+    const size_t raw_total = 3 * raw_b + 2 * out_b + 256;
+    SS_CUDA(g_pool.acquire(raw_total, &raw));
+    struct Guard { char* p; size_t b; cudaStream_t s; ~Guard() { cudaStreamSynchronize(s); g_pool.release(p, b); } } guard{raw, raw_total, stream};
     double* d_t = (double*)raw; double* d_y = (double*)(raw + raw_b); double* d_e = (double*)(raw + 2 * raw_b);
     double* d_bf = (double*)(raw + 3 * raw_b); int64_t* d_bi = (int64_t*)(raw + 3 * raw_b + out_b);
     if (total > 0) {
@@ -720,20 +806,24 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
     double* tile_buf[2] = {nullptr, nullptr};
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t done[2] = {nullptr, nullptr}, copied[2] = {nullptr, nullptr};
+    const size_t tile_alloc = std::max<size_t>(eng.plan.tile_bytes, 8);
     struct TileRes {
-        double** b; cudaStream_t* s; cudaEvent_t* d; cudaEvent_t* c;
+        double** b; size_t bytes; cudaEvent_t* d; cudaEvent_t* c; cudaStream_t s; cudaStream_t* cs;
         ~TileRes() {
-            for (int i = 0; i < 2; i++) { if (b[i]) cudaFree(b[i]); if (d[i]) cudaEventDestroy(d[i]); if (c[i]) cudaEventDestroy(c[i]); }
-            if (*s) cudaStreamDestroy(*s);
+            cudaStreamSynchronize(s);
+            if (*cs) cudaStreamSynchronize(*cs);
+            for (int i = 0; i < 2; i++) { g_pool.release((char*)b[i], bytes); g_pool.event_back(false, d[i]); g_pool.event_back(false, c[i]); }
         }
-    } tres{tile_buf, &copy_stream, done, copied};
+    } tres{tile_buf, tile_alloc, done, copied, stream, &copy_stream};
     if (pgram_out) {
         for (int i = 0; i < 2; i++) {
-            SS_CUDA(cudaMalloc((void**)&tile_buf[i], std::max<size_t>(eng.plan.tile_bytes, 8)));
-            SS_CUDA(cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming));
-            SS_CUDA(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
+            char* tb_ = nullptr;
+            SS_CUDA(g_pool.acquire(tile_alloc, &tb_));
+            tile_buf[i] = (double*)tb_;
+            SS_CUDA(g_pool.event(false, &done[i]));
+            SS_CUDA(g_pool.event(false, &copied[i]));
         }
-        SS_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        SS_CUDA(g_pool.stream(&copy_stream));
     }
     int it = 0;
     for (int ot = 0; ot < (int)eng.tiles.size(); ot++) {

@@ -499,3 +499,28 @@ def test_single_object_configs_full_size_sampled(ss, cfg, mode):
         assert r["margin"] < 1e-9 and abs(g - r["P_alt"]) <= _tol(r["P_alt"]), (cfg, k, g, r["P"], r["margin"])
         ambiguous += 1
     assert ambiguous <= 2
+
+
+def test_workspace_is_reused_between_calls_and_can_be_released(ss):
+    """Steady-state calls allocate nothing (the per-thread pool serves the workspace, the host entry point's
+    catalog copy and output tiles); ss_release_workspace gives the memory back; results do not change."""
+    import torch
+    cat = ss_inputs.config3(n_objects=50, n_freq=401)
+    ss.release_workspace()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    first = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, CV)
+    free1 = torch.cuda.mem_get_info()[0]
+    assert free1 < free0                                   # the pool now holds the buffers
+    for _ in range(3):
+        again = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, CV)
+        assert torch.cuda.mem_get_info()[0] == free1       # nothing allocated, nothing freed
+        assert np.array_equal(again.pgram, first.pgram) and np.array_equal(again.best_index, first.best_index)
+    # a smaller and a different-shaped request are served from the same buffers
+    sub = cat.subset(list(range(10)))
+    ss.periodogram(sub.times, sub.mags, sub.errs, sub.offsets, sub.f_min, sub.f_max, 100, GV)
+    assert torch.cuda.mem_get_info()[0] == free1
+    ss.release_workspace()
+    assert torch.cuda.mem_get_info()[0] >= free0 - (1 << 20)
+    after = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, CV)
+    assert np.array_equal(after.pgram, first.pgram)
