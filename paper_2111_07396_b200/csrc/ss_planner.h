@@ -98,6 +98,12 @@ inline ss_status_t make_plan(const PlanInput& in, ss_plan_t* out)
     int64_t fpt = in.n_freq, opt = nobj > 0 ? nobj : 1;
     if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) fpt = in.force_freq_tile;
     if (in.host_tiles && in.want_pgram) {
+        // a large output goes back in at least 4 frequency tiles even when one would fit, so that the
+        // device->host copy of a tile overlaps the next tile's kernels instead of trailing the last one
+        if (in.force_freq_tile <= 0 && (size_t)8 * (size_t)in.n_freq * (size_t)opt >= ((size_t)256 << 20) && in.n_freq >= 4) {
+            const int64_t quarter = (in.n_freq + 3) / 4;
+            if (quarter < fpt) fpt = quarter;
+        }
         // exact need of an (f x o) tile: double-buffered output tile + partial rows
         auto need = [&](int64_t f, int64_t o) { return base + partials(f, o) + (size_t)2 * 8 * (size_t)f * (size_t)o; };
         // shrink the frequency tile first (the paper's N_b batches), then objects;
