@@ -78,6 +78,11 @@ typedef struct {
     int skip_validation;    /* 1 = trust the inputs (no device validation pass, no host sync for it)    */
     int profile;            /* 1 = bracket every eval-kernel launch with CUDA events on the stream;
                                read the sum with ss_last_kernel_ms() after the call                     */
+    int64_t k_begin;        /* evaluate only the grid indices [k_begin, k_begin + k_count) of the grid that   */
+    int64_t k_count;        /* (f_min, f_max, n_freq) defines: f_k keeps its bits, pgram_out then has k_count
+                               columns (column 0 = index k_begin), best_index stays an index into the whole
+                               grid.  k_count = 0: up to the end of the grid.  For splitting one object's
+                               frequency range across GPUs.                           */
 } ss_options_t;
 
 /* Fill *opt with the defaults listed above. */

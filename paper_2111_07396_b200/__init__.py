@@ -36,7 +36,8 @@ class SSError(RuntimeError):
 class Options(C.Structure):
     _fields_ = [("alpha", C.c_double), ("span", C.c_double), ("iper", C.c_int),
                 ("force_path", C.c_int), ("stream", C.c_void_p), ("workspace_cap", C.c_size_t),
-                ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int)]
+                ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int),
+                ("k_begin", C.c_int64), ("k_count", C.c_int64)]
 
 
 class Plan(C.Structure):
@@ -228,7 +229,9 @@ def periodogram(times, mags, errs, offsets, f_min, f_max, n_freq, mode=CROSS_VAL
     errs = np.ascontiguousarray(errs, dtype=np.float64)
     offsets = np.ascontiguousarray(offsets, dtype=np.int64)
     n_obj = len(offsets) - 1
-    pg = np.empty((n_obj, int(n_freq))) if want_pgram else None
+    k_begin = int(opts.get("k_begin", 0))
+    n_cols = int(opts.get("k_count", 0)) or int(n_freq) - k_begin
+    pg = np.empty((n_obj, n_cols)) if want_pgram else None
     bf = np.empty(n_obj)
     bi = np.empty(n_obj, dtype=np.int64)
     ss_periodogram_host(times, mags, errs, offsets, n_obj, f_min, f_max, n_freq, mode, pg, bf, bi,

@@ -306,6 +306,7 @@ struct Engine {
     ss_options_t opt{};
     int mode = 0;
     int64_t n_objects = 0, n_freq = 0, total = 0;
+    int64_t k_lo = 0, k_n = 0;         // the sub-range of the grid this call evaluates (opt.k_begin / k_count)
     double f_min = 0, df = 0;
     std::vector<int64_t> off;
     std::vector<ObjRec> recs;          // objects with n >= 5
@@ -382,6 +383,8 @@ static ss_status_t validate_scalars(int64_t n_objects, double f_min, double f_ma
     if (!(o.span >= 0.0) || !(o.span <= 1.0)) return fail(SS_ERR_INVALID_ARG, "span must be 0 (variable) or in (0, 1]");
     if (o.iper != 1 && o.iper != 2) return fail(SS_ERR_INVALID_ARG, "iper = %d (1 = non-periodic, 2 = periodic)", o.iper);
     if (!std::isfinite(o.alpha)) return fail(SS_ERR_INVALID_ARG, "alpha is not finite");
+    if (o.k_begin < 0 || o.k_count < 0 || o.k_begin >= n_freq || o.k_begin + o.k_count > n_freq)
+        return fail(SS_ERR_INVALID_ARG, "k_begin/k_count outside the grid");
     return SS_OK;
 }
 
@@ -399,6 +402,8 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     mode = md;
     n_objects = n_obj;
     n_freq = nfreq;
+    k_lo = o.k_begin;
+    k_n = o.k_count > 0 ? o.k_count : nfreq - o.k_begin;
     f_min = fmin;
     df = (fmax - fmin) / (double)nfreq;
     int dev = 0;
@@ -430,7 +435,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         SS_CUDA(cudaMemGetInfo(&fr, &tot));
         cap = (size_t)(0.75 * (double)fr);   // the paper's beta
     }
-    PlanInput pin{total, max_n, n_obj, nfreq, md, cap, host_tiles ? 1 : 0, want_pgram ? 1 : 0, o.freq_tile};
+    PlanInput pin{total, max_n, n_obj, k_n, md, cap, host_tiles ? 1 : 0, want_pgram ? 1 : 0, o.freq_tile};
     ss_status_t st = make_plan(pin, &plan);
     if (st != SS_OK) return fail(st, "workspace cap %zu B too small for the smallest tile", cap);
 
@@ -734,8 +739,8 @@ ss_status_t ss_periodogram_ex(const double* times, const double* mags, const dou
     // partial-argmax rows
     for (int ot = 0; ot < (int)eng.tiles.size(); ot++) {
         for (int64_t ft = 0; ft < eng.plan.n_freq_tiles; ft++) {
-            int64_t k0 = ft * eng.plan.freq_per_tile, k1 = std::min(n_freq, k0 + eng.plan.freq_per_tile);
-            st = eng.run_tile(ot, k0, k1, (int)ft, pgram_out, n_freq, 0, 0);
+            int64_t k0 = eng.k_lo + ft * eng.plan.freq_per_tile, k1 = std::min(eng.k_lo + eng.k_n, k0 + eng.plan.freq_per_tile);
+            st = eng.run_tile(ot, k0, k1, (int)ft, pgram_out, eng.k_n, 0, eng.k_lo);
             if (st != SS_OK) return st;
         }
     }
@@ -830,7 +835,7 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
         const int64_t o0 = (int64_t)ot * eng.plan.objects_per_tile;
         const int64_t o1 = std::min(n_objects, o0 + eng.plan.objects_per_tile);
         for (int64_t ft = 0; ft < eng.plan.n_freq_tiles; ft++, it++) {
-            const int64_t k0 = ft * eng.plan.freq_per_tile, k1 = std::min(n_freq, k0 + eng.plan.freq_per_tile);
+            const int64_t k0 = eng.k_lo + ft * eng.plan.freq_per_tile, k1 = std::min(eng.k_lo + eng.k_n, k0 + eng.plan.freq_per_tile);
             const int bi = it & 1;
             double* tb = pgram_out ? tile_buf[bi] : nullptr;
             if (pgram_out && it >= 2) SS_CUDA(cudaStreamWaitEvent(stream, copied[bi], 0));
@@ -839,7 +844,7 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
             if (pgram_out) {
                 SS_CUDA(cudaEventRecord(done[bi], stream));
                 SS_CUDA(cudaStreamWaitEvent(copy_stream, done[bi], 0));
-                SS_CUDA(cudaMemcpy2DAsync(pgram_out + o0 * n_freq + k0, 8 * (size_t)n_freq, tb, 8 * (size_t)(k1 - k0),
+                SS_CUDA(cudaMemcpy2DAsync(pgram_out + o0 * eng.k_n + (k0 - eng.k_lo), 8 * (size_t)eng.k_n, tb, 8 * (size_t)(k1 - k0),
                                           8 * (size_t)(k1 - k0), (size_t)(o1 - o0), cudaMemcpyDeviceToHost, copy_stream));
                 SS_CUDA(cudaEventRecord(copied[bi], copy_stream));
             }

@@ -94,3 +94,66 @@ def gather_best(idx, best_freq, best_index, n_objects: int, group=None):
     if not np.all(seen):
         raise ValueError("shards do not cover the catalog")
     return bf, bi
+
+
+# ---- one (or a few) long light curves: split the frequency range instead ------------
+def shard_frequencies(n_freq: int, world_size: int) -> list[tuple[int, int]]:
+    """Contiguous, near-equal ranges (k_begin, k_count) of the grid indices 0..n_freq-1, one per rank
+    (ranks beyond n_freq get an empty range)."""
+    if world_size < 1:
+        raise ValueError("world_size must be >= 1")
+    base, extra = divmod(int(n_freq), world_size)
+    out, k = [], 0
+    for r in range(world_size):
+        c = base + (1 if r < extra else 0)
+        out.append((k, c))
+        k += c
+    return out
+
+
+def periodogram_freq_sharded(times, mags, errs, offsets, f_min, f_max, n_freq, mode=0, *, rank: int, world_size: int,
+                             **opts):
+    """This rank's frequency range of every object, through the library's k_begin / k_count options: the
+    grid (f_min, f_max, n_freq) is unchanged, so every f_k keeps its bits.  Returns ((k_begin, k_count), Result);
+    Result.pgram has k_count columns, Result.best_index indexes the whole grid."""
+    from . import periodogram
+    k_begin, k_count = shard_frequencies(n_freq, world_size)[rank]
+    if k_count == 0:
+        return (k_begin, 0), None
+    return (k_begin, k_count), periodogram(times, mags, errs, offsets, f_min, f_max, n_freq, mode, want_pgram=True,
+                                           k_begin=k_begin, k_count=k_count, **opts)
+
+
+def merge_best_over_ranges(parts, n_objects: int):
+    """parts: iterable of (k_begin, best_index[n_objects], best_power[n_objects]) from disjoint frequency ranges.
+    Per object the highest power wins, ties go to the lowest index (the argmax rule of the single call, O8);
+    best_index -1 (object with fewer than 5 points) stays -1."""
+    bi = np.full(n_objects, -1, dtype=np.int64)
+    bp = np.full(n_objects, -np.inf)
+    for _, idx, pw in sorted(parts, key=lambda t: t[0]):
+        idx = np.asarray(idx, dtype=np.int64)
+        pw = np.asarray(pw, dtype=np.float64)
+        take = (idx >= 0) & ((pw > bp) | (bi < 0))          # ranges come in ascending k: '>' keeps the first maximum
+        bi = np.where(take, idx, bi)
+        bp = np.where(take, pw, bp)
+    return bi, bp
+
+
+def gather_best_over_ranges(k_range, result, n_objects: int, group=None):
+    """All ranks exchange (best index, best power) of their frequency range (all_gather_object, 16 bytes per
+    object) and every rank returns the merged (best_index, best_power)."""
+    if result is None:
+        mine = (k_range[0], np.full(n_objects, -1, dtype=np.int64), np.full(n_objects, -np.inf))
+    else:
+        cols = np.clip(result.best_index - k_range[0], 0, max(k_range[1] - 1, 0))
+        power = np.where(result.best_index >= 0, result.pgram[np.arange(n_objects), cols], -np.inf)
+        mine = (k_range[0], result.best_index, power)
+    parts = [mine]
+    try:
+        import torch.distributed as dist
+        if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+            parts = [None] * dist.get_world_size(group)
+            dist.all_gather_object(parts, mine, group=group)
+    except ImportError:
+        pass
+    return merge_best_over_ranges(parts, n_objects)

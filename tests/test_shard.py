@@ -106,6 +106,69 @@ def test_two_rank_shard_and_gather_over_gloo():
         assert o["bf"] == want_bf and o["bi"] == want_bi
 
 
+def test_frequency_ranges_and_best_merge():
+    for n_freq, world in ((10, 3), (7, 8), (1000000, 4)):
+        r = shard.shard_frequencies(n_freq, world)
+        assert len(r) == world and r[0][0] == 0 and sum(c for _, c in r) == n_freq
+        assert all(r[i][0] + r[i][1] == r[i + 1][0] for i in range(world - 1))
+        assert max(c for _, c in r) - min(c for _, c in r) <= 1
+    # merge = argmax over the concatenated row, first maximum wins; degenerate objects stay -1
+    rng = np.random.default_rng(5)
+    row = rng.normal(size=(4, 90)); row[1, 70] = row[1, 20] = row[1].max() + 1.0     # a tie across ranges
+    parts = []
+    for kb, kc in shard.shard_frequencies(90, 3):
+        seg = row[:, kb:kb + kc]
+        idx = kb + np.argmax(seg, axis=1); pw = seg.max(axis=1)
+        idx[3] = -1; pw[3] = -np.inf
+        parts.append((kb, idx, pw))
+    bi, bp = shard.merge_best_over_ranges(parts[::-1], 4)             # order of arrival must not matter
+    assert np.array_equal(bi[:3], np.argmax(row[:3], axis=1)) and bi[1] == 20 and bi[3] == -1
+    assert np.array_equal(bp[:3], row[:3].max(axis=1))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("mode", [0, 1])
+def test_frequency_ranges_reproduce_the_whole_grid_bit_for_bit(mode):
+    """k_begin / k_count (one object's grid split over 'ranks', run one after the other here): the pieces
+    concatenate to the single-call periodogram exactly and the merged best index is the single call's.
+    Covers the warp, CTA and staging classes and both entry points."""
+    import torch
+    import paper_2111_07396_b200 as ss
+    a = ss_inputs.config3(n_objects=5, n_freq=203)
+    b = ss_inputs.config4(n_objects=2, n_freq=203)
+    times = np.concatenate([a.times, b.times, np.linspace(0, 50, 3)]); mags = np.concatenate([a.mags, b.mags, [15., 15.1, 15.2]])
+    errs = np.concatenate([a.errs, b.errs, [0.1, 0.1, 0.1]])
+    offsets = np.concatenate([a.offsets, a.offsets[-1] + b.offsets[1:], [a.offsets[-1] + b.offsets[-1] + 3]])
+    n_obj = len(offsets) - 1                                                      # the last object has 3 points: NaN row
+    whole = ss.periodogram(times, mags, errs, offsets, 0.5, 24.0, 203, mode)
+    for world in (2, 3):
+        pieces, parts = [], []
+        for rank in range(world):
+            kr, res = shard.periodogram_freq_sharded(times, mags, errs, offsets, 0.5, 24.0, 203, mode, rank=rank,
+                                                     world_size=world)
+            assert res.pgram.shape == (n_obj, kr[1])
+            pieces.append(res.pgram)
+            cols = np.clip(res.best_index - kr[0], 0, kr[1] - 1)
+            parts.append((kr[0], res.best_index, np.where(res.best_index >= 0, res.pgram[np.arange(n_obj), cols], -np.inf)))
+        assert np.array_equal(np.concatenate(pieces, axis=1), whole.pgram, equal_nan=True)
+        bi, _ = shard.merge_best_over_ranges(parts, n_obj)
+        assert np.array_equal(bi, whole.best_index)
+    # device entry point with a sub-range, forced staging path
+    dev = torch.device("cuda")
+    t = torch.as_tensor(times, device=dev); y = torch.as_tensor(mags, device=dev); e = torch.as_tensor(errs, device=dev)
+    off = torch.as_tensor(offsets, device=dev)
+    pg = torch.empty((n_obj, 50), dtype=torch.float64, device=dev)
+    bi_d = torch.empty(n_obj, dtype=torch.int64, device=dev); bf_d = torch.empty(n_obj, dtype=torch.float64, device=dev)
+    ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, 203, mode, pg, bf_d, bi_d,
+                      ss.default_options(k_begin=100, k_count=50, force_path=ss.PATH_STAGE))
+    staged = ss.periodogram(times, mags, errs, offsets, 0.5, 24.0, 203, mode, force_path=ss.PATH_STAGE)   # same kernel, whole grid
+    assert np.array_equal(pg.cpu().numpy(), staged.pgram[:, 100:150], equal_nan=True)
+    k = bi_d.cpu().numpy()
+    assert np.all((k[:-1] >= 100) & (k[:-1] < 150)) and k[-1] == -1
+    with pytest.raises(ss.SSError):
+        ss.periodogram(times, mags, errs, offsets, 0.5, 24.0, 203, mode, k_begin=200, k_count=10)
+
+
 @pytest.mark.gpu
 @pytest.mark.parametrize("mode", [0, 1])
 def test_shards_reproduce_the_unsharded_result_bit_for_bit(mode):
