@@ -111,27 +111,6 @@ __device__ __forceinline__ double block_sum(double v, double* red)
     return s;
 }
 
-// Average z over maximal runs of equal keys, w-weighted (O4 last bullet).  Serial, one thread:
-// exact ties in phase are rare (structured time stamps), this is the slow-but-exact path.
-__device__ inline void tie_average_serial(int n, const unsigned long long* key, const double* w, double* z)
-{
-    int j = 0;
-    while (j < n) {
-        int j0 = j;
-        double sy = z[j] * w[j], fbw = w[j];
-        while (j < n - 1 && key[j + 1] <= key[j]) {
-            j++;
-            sy += w[j] * z[j];
-            fbw += w[j];
-        }
-        if (j > j0) {
-            double a = fbw > 0.0 ? sy / fbw : 0.0;
-            for (int i = j0; i <= j; i++) z[i] = a;
-        }
-        j++;
-    }
-}
-
 // Replace the -1 sentinels of the LOO residuals by the previous valid value (R23).
 __device__ inline void carry_fix_serial(int n, double* r)
 {

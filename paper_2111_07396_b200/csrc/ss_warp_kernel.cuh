@@ -374,7 +374,6 @@ __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.
 struct WarpMem {
     const double* tt; const double* yc; const double* w;   // the object's arrays (CTA-wide)
     double2* E;              // per-warp: 3 pair-prefix arrays of C*WROW double2
-    unsigned char* perm;     // per-warp: 256 bytes (rank -> index), only when S != C
     uint32_t tmem;           // per-warp tensor-memory base (lane quarter + first column), CV only
     ScanMask mk;             // Kogge-Stone masks of this lane
 };
@@ -767,8 +766,8 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
 template <int C, bool GV>
 inline size_t warp_smem_bytes()
 {
-    // object arrays (3 x 32C doubles) + per warp: 3 pair-prefix arrays + 256 B permutation bytes
-    return (size_t)3 * 32 * C * 8 + (size_t)WarpCfg<C, GV>::WPC * ((size_t)3 * C * WROW * 16 + 256);
+    // object arrays (3 x 32C doubles) + per warp: 3 pair-prefix arrays
+    return (size_t)3 * 32 * C * 8 + (size_t)WarpCfg<C, GV>::WPC * ((size_t)3 * C * WROW * 16);
 }
 
 __device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
@@ -819,12 +818,11 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     double* o_tt = reinterpret_cast<double*>(smem_raw);
     double* o_y = o_tt + 32 * C;
     double* o_w = o_y + 32 * C;
-    constexpr size_t WARP_BYTES = (size_t)3 * C * WROW * 16 + 256;
+    constexpr size_t WARP_BYTES = (size_t)3 * C * WROW * 16;
     unsigned char* wbase = smem_raw + (size_t)3 * 32 * C * 8 + (size_t)warp * WARP_BYTES;
     WarpMem M;
     M.tt = o_tt; M.yc = o_y; M.w = o_w;
     M.E = reinterpret_cast<double2*>(wbase);
-    M.perm = wbase + (size_t)3 * C * WROW * 16;
     M.tmem = 0;
     M.mk = make_scan_mask(lane);
     {
