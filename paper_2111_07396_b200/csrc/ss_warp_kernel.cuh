@@ -27,8 +27,9 @@ constexpr int WARPS_PER_CTA = 8;      // frequency chunks are multiples of this 
 // 65536 / (32 * WPC * MINB), rounded down to a multiple of 8).
 template <int C, bool GV> struct WarpCfg {
     static constexpr bool GV20 = GV && C <= 4;      // 4 warps x 5 CTAs = 20 warps/SM at 96 registers (1 % over 16 at 128)
-    static constexpr int WPC = GV20 ? 4 : ((C <= 6 || (!GV && C >= 7)) ? 8 : 4);
-    static constexpr int MINB = GV20 ? 5 : (C <= 6 ? 2 : (GV ? 3 : 1));
+    static constexpr bool CV7 = !GV && C == 7;     // 4 warps x 3 CTAs = 12 warps/SM at 168 registers (4 % over 8 at 255)
+    static constexpr int WPC = (GV20 || CV7) ? 4 : ((C <= 6 || (!GV && C >= 7)) ? 8 : 4);
+    static constexpr int MINB = GV20 ? 5 : (CV7 ? 3 : (C <= 6 ? 2 : (GV ? 3 : 1)));
 };
 constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lanes + the total)
 constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0
