@@ -26,10 +26,11 @@ constexpr int WARPS_PER_CTA = 8;      // frequency chunks are multiples of this 
 // Launch shape per points-per-lane: warps per CTA and resident CTAs per SM (register budget =
 // 65536 / (32 * WPC * MINB), rounded down to a multiple of 8).
 template <int C, bool GV> struct WarpCfg {
-    static constexpr bool GV20 = GV && C <= 4;      // 4 warps x 5 CTAs = 20 warps/SM at 96 registers (1 % over 16 at 128)
-    static constexpr bool CV7 = !GV && C == 7;     // 4 warps x 3 CTAs = 12 warps/SM at 168 registers (4 % over 8 at 255)
-    static constexpr int WPC = (GV20 || CV7) ? 4 : ((C <= 6 || (!GV && C >= 7)) ? 8 : 4);
-    static constexpr int MINB = GV20 ? 5 : (CV7 ? 3 : (C <= 6 ? 2 : (GV ? 3 : 1)));
+    // each shape chosen by measurement on config 3:
+    //   GV: C <= 4: 4 warps x 5 CTAs (20 warps/SM,  96 registers);  C >= 5: 4 x 3 (12 warps, 168)
+    //   CV: C <= 6: 8 warps x 2 CTAs (16 warps/SM, 128 registers);  C = 7: 4 x 3 (12 warps, 168);  C = 8: 8 x 1 (255)
+    static constexpr int WPC = GV ? 4 : (C == 7 ? 4 : 8);
+    static constexpr int MINB = GV ? (C <= 4 ? 5 : 3) : (C <= 6 ? 2 : (C == 7 ? 3 : 1));
 };
 constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lanes + the total)
 constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0
