@@ -83,6 +83,10 @@ typedef struct {
                                columns (column 0 = index k_begin), best_index stays an index into the whole
                                grid.  k_count = 0: up to the end of the grid.  For splitting one object's
                                frequency range across GPUs.                           */
+    unsigned int defer_capacity; /* test hook: entries of the list through which the warp-per-eval kernels hand
+                               tied / undecidable evals to the generic kernel, per tile (0 = 2^20).  When it
+                               overflows the call repeats itself on the CTA-per-eval kernels; results never
+                               depend on it.                                                              */
 } ss_options_t;
 
 /* Fill *opt with the defaults listed above. */

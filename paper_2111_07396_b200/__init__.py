@@ -37,7 +37,7 @@ class Options(C.Structure):
     _fields_ = [("alpha", C.c_double), ("span", C.c_double), ("iper", C.c_int),
                 ("force_path", C.c_int), ("stream", C.c_void_p), ("workspace_cap", C.c_size_t),
                 ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int),
-                ("k_begin", C.c_int64), ("k_count", C.c_int64)]
+                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("defer_capacity", C.c_uint)]
 
 
 class Plan(C.Structure):
@@ -51,13 +51,15 @@ _lib = None
 
 
 def load():
-    """dlopen libss_b200.so (building it with nvcc if the source is newer) and set signatures."""
+    """dlopen libss_b200.so and set signatures.  The library is rebuilt with nvcc first when it is missing or
+    when the hash of the sources it was built from (stored beside it) no longer matches csrc/ and include/: an
+    edited kernel can never be exercised through a stale binary."""
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH) or os.environ.get("SS_REBUILD"):
-        from ._build import build
-        build()
+    from . import _build
+    if os.environ.get("SS_REBUILD") or not _build.is_fresh():
+        _build.build(force=True)
     if not os.path.exists(LIB_PATH):
         raise SSError(SS_ERR_CUDA, f"{LIB_PATH} is missing and could not be built")
     L = C.CDLL(LIB_PATH)

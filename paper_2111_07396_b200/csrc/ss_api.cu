@@ -9,10 +9,9 @@
 #include <vector>
 
 #include "../../include/ss_periodogram.h"
-#include "ss_block_kernel.cuh"
 #include "ss_common.cuh"
+#include "ss_launch.h"
 #include "ss_planner.h"
-#include "ss_warp_kernel.cuh"
 
 namespace ss {
 
@@ -53,6 +52,7 @@ struct DevicePool {
     std::vector<cudaEvent_t> timing_events, plain_events;
     cudaStream_t copy_stream = nullptr;
     int copy_stream_dev = -1;
+    int event_dev = -1;
 
     // smallest cached buffer of this device that is large enough, else a fresh allocation
     cudaError_t acquire(size_t bytes, char** out)
@@ -93,6 +93,15 @@ struct DevicePool {
     }
     cudaError_t event(bool timing, cudaEvent_t* out)
     {
+        // events belong to the device they were created on: a thread that switched devices starts a fresh cache
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (dev != event_dev) {
+            for (auto e : timing_events) cudaEventDestroy(e);
+            for (auto e : plain_events) cudaEventDestroy(e);
+            timing_events.clear(); plain_events.clear();
+            event_dev = dev;
+        }
         auto& v = timing ? timing_events : plain_events;
         if (!v.empty()) { *out = v.back(); v.pop_back(); return cudaSuccess; }
         return timing ? cudaEventCreate(out) : cudaEventCreateWithFlags(out, cudaEventDisableTiming);
@@ -161,6 +170,16 @@ __global__ void __launch_bounds__(PREP_T) prep_kernel(const double* __restrict__
         tmin = fmin(tmin, t);
     }
     if (bad) atomicOr(flag, 1);
+    // duplicated time stamps tie at every frequency: the warp path hands such an object over whole (ObjRec::dup)
+    if (n <= SS_WARP_MAX_N) {
+        int dup = 0;
+        for (int j = tid; j < n; j += PREP_T) {
+            const double t = times[off + j];
+            for (int i = 0; i < j; i++) dup |= (times[off + i] == t);
+        }
+        dup = __syncthreads_or(dup);
+        if (tid == 0) recs[ri].dup = dup ? 1 : 0;
+    }
     // block min
 #pragma unroll
     for (int d = 16; d > 0; d >>= 1) tmin = fmin(tmin, __shfl_xor_sync(0xffffffffu, tmin, d));
@@ -398,6 +417,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
                           bool want_pgram, size_t extra_bytes)
 {
     opt = o;
+    if (o.defer_capacity > 0) defer_capacity = o.defer_capacity;
     stream = (cudaStream_t)o.stream;
     mode = md;
     n_objects = n_obj;
@@ -534,14 +554,6 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     return SS_OK;
 }
 
-template <typename K>
-static ss_status_t set_smem(K kernel, size_t bytes)
-{
-    if (bytes > 48 * 1024)
-        SS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-    return SS_OK;
-}
-
 ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int freq_tile_index,
                              double* pgram, int64_t row_stride, int64_t row0, int64_t k0)
 {
@@ -585,50 +597,30 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else {
-            const bool optk = has_listing_options(opt);
-            if (c.path == SS_PATH_BLOCK) {
-                const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(c.max_n) * 8;
-                if (c.variant == 2) {
-                    auto kern = optk ? block_kernel<512, false, true> : block_kernel<512, false, false>;
-                    SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                    int grid = (int)std::min<int64_t>(n_items, sm_count);
-                    kern<<<grid, 512, smem, stream>>>(p);
-                } else if (c.variant == 3) {
-                                        auto kern = optk ? block_kernel<128, false, true> : block_kernel<128, false, false>;
-                    SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                    int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 4);
-                    kern<<<grid, 128, smem, stream>>>(p);
-                } else {
-                    auto kern = optk ? block_kernel<256, false, true> : block_kernel<256, false, false>;
-                    SS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                    int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 2);
-                    kern<<<grid, 256, smem, stream>>>(p);
-                }
-            } else {
-                auto kern = optk ? block_kernel<512, true, true> : block_kernel<512, true, false>;
-                int grid = (int)std::min<int64_t>(n_items, (int64_t)sm_count * 2);
-                kern<<<grid, 512, 0, stream>>>(p);
-            }
+            const int threads = c.path == SS_PATH_STAGE ? 512 : (c.variant == 2 ? 512 : (c.variant == 3 ? 128 : 256));
+            ss_status_t st = launch_block_kernel(p, c.path, threads, c.max_n, has_listing_options(opt), n_items, sm_count, stream);
+            if (st != SS_OK) return fail(st, "CTA kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         }
         if (ev1) SS_CUDA(cudaEventRecord(ev1, stream));
         g_launches++;
-        SS_CUDA(cudaGetLastError());
+        if (c.path == SS_PATH_WARP) {
+            // what the warp path handed over (tied / misordered phases, leave-one-out denominator <= 0, objects
+            // with duplicated time stamps): recompute with the generic code, patch the periodogram; whole items
+            // write their partial-argmax slot (hence before the fold below), single evals fold into the running best
+            SS_CUDA(cudaMemsetAsync(dmax, 0, 8 * (size_t)n_objects, stream));
+            SS_CUDA(cudaMemsetAsync(dmin, 0xff, 8 * (size_t)n_objects, stream));
+            ss_status_t st = launch_deferred_eval(p, defer_val, dmax, sm_count, stream);
+            if (st != SS_OK) return fail(st, "deferred kernel launch failed");
+            g_launches++;
+        }
         fold_best_kernel<<<(unsigned)((p.n_list * 32 + 255) / 256), 256, 0, stream>>>(
             d_recs, p.list, p.n_list, (int)cpo, p.chunks_total, 0, part_val, part_idx, best_val, best_idx);
         g_launches++;
         SS_CUDA(cudaGetLastError());
         if (c.path == SS_PATH_WARP) {
-            // evals the warp path deferred (tied / misordered phases, LOO denominator <= 0):
-            // recompute with the generic code, patch the periodogram, fold into the running best
-            SS_CUDA(cudaMemsetAsync(dmax, 0, 8 * (size_t)n_objects, stream));
-            SS_CUDA(cudaMemsetAsync(dmin, 0xff, 8 * (size_t)n_objects, stream));
-            const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(SS_WARP_MAX_N) * 8;
-            SS_CUDA(cudaFuncSetAttribute(deferred_eval_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            deferred_eval_kernel<<<sm_count * 4, DEFER_T, smem, stream>>>(p, defer_val, dmax);
-            deferred_min_kernel<<<sm_count, 256, 0, stream>>>(p, defer_val, dmax, dmin);
-            deferred_merge_kernel<<<sm_count, 256, 0, stream>>>(p, defer_val, dmax, dmin, best_val, best_idx);
-            g_launches += 3;
-            SS_CUDA(cudaGetLastError());
+            ss_status_t st = launch_deferred_merge(p, defer_val, dmax, dmin, best_val, best_idx, sm_count, stream);
+            if (st != SS_OK) return fail(st, "deferred merge launch failed");
+            g_launches += 2;
             SS_CUDA(cudaMemsetAsync(defer_count, 0, 4, stream));   // the overflow flag [1] stays
         }
     }
@@ -714,14 +706,14 @@ size_t ss_workspace_bytes(int64_t n_points_total, int64_t max_n, int64_t n_objec
     return pl.total_bytes;
 }
 
-ss_status_t ss_periodogram_ex(const double* times, const double* mags, const double* errs,
-                              const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
-                              int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
-                              int64_t* best_index_out, const ss_options_t* opt_in)
+// One pass over the catalog with DEVICE pointers.  *overflow: the warp path's hand-over list was too short (the
+// outputs are then incomplete; the caller repeats the pass on the CTA path once this pass's buffers are back in the pool).
+static ss_status_t periodogram_device(const double* times, const double* mags, const double* errs,
+                                      const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                                      int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                                      int64_t* best_index_out, const ss_options_t& o, bool* overflow)
 {
-    g_launches = 0;
-    ss_options_t o;
-    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    *overflow = false;
     ss_status_t st = validate_scalars(n_objects, f_min, f_max, n_freq, (int)mode, o);
     if (st != SS_OK) return st;
     if (!offsets) return fail(SS_ERR_INVALID_ARG, "offsets is null");
@@ -748,16 +740,30 @@ ss_status_t ss_periodogram_ex(const double* times, const double* mags, const dou
     if (st != SS_OK) return st;
     SS_CUDA(cudaStreamSynchronize(stream));
     eng.collect_profile();
-    if (eng.defer_overflowed()) {
-        // more exact ties than the hand-over list holds (e.g. duplicated time stamps in every
-        // object): serve everything with the generic kernel instead
-        if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "deferred list overflow on the block path");
-        ss_options_t o2 = o;
-        o2.force_path = SS_PATH_BLOCK;
-        return ss_periodogram_ex(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
-                                 best_freq_out, best_index_out, &o2);
-    }
+    *overflow = eng.defer_overflowed();
     return SS_OK;
+}
+
+ss_status_t ss_periodogram_ex(const double* times, const double* mags, const double* errs,
+                              const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                              int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                              int64_t* best_index_out, const ss_options_t* opt_in)
+{
+    g_launches = 0;
+    ss_options_t o;
+    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    bool overflow = false;
+    ss_status_t st = periodogram_device(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                                        best_freq_out, best_index_out, o, &overflow);
+    if (st == SS_OK && overflow) {
+        // more ties than the hand-over list holds (e.g. integer time stamps at a commensurate frequency in every
+        // object): serve everything with the generic kernel instead.  The first pass's buffers are already released.
+        if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "hand-over list overflow on the CTA path");
+        o.force_path = SS_PATH_BLOCK;
+        st = periodogram_device(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                                best_freq_out, best_index_out, o, &overflow);
+    }
+    return st;
 }
 
 ss_status_t ss_periodogram(const double* times, const double* mags, const double* errs,
@@ -769,14 +775,12 @@ ss_status_t ss_periodogram(const double* times, const double* mags, const double
                              best_freq_out, best_index_out, nullptr);
 }
 
-ss_status_t ss_periodogram_host(const double* times, const double* mags, const double* errs,
-                                const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
-                                int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
-                                int64_t* best_index_out, const ss_options_t* opt_in)
+static ss_status_t periodogram_host(const double* times, const double* mags, const double* errs,
+                                    const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                                    int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                                    int64_t* best_index_out, const ss_options_t& o, bool* overflow)
 {
-    g_launches = 0;
-    ss_options_t o;
-    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    *overflow = false;
     ss_status_t st = validate_scalars(n_objects, f_min, f_max, n_freq, (int)mode, o);
     if (st != SS_OK) return st;
     if (!offsets) return fail(SS_ERR_INVALID_ARG, "offsets is null");
@@ -857,14 +861,28 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
     SS_CUDA(cudaStreamSynchronize(stream));
     if (copy_stream) SS_CUDA(cudaStreamSynchronize(copy_stream));
     eng.collect_profile();
-    if (eng.defer_overflowed()) {
-        if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "deferred list overflow on the block path");
-        ss_options_t o2 = o;
-        o2.force_path = SS_PATH_BLOCK;
-        return ss_periodogram_host(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
-                                   best_freq_out, best_index_out, &o2);
-    }
+    *overflow = eng.defer_overflowed();
     return SS_OK;
+}
+
+ss_status_t ss_periodogram_host(const double* times, const double* mags, const double* errs,
+                                const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
+                                int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
+                                int64_t* best_index_out, const ss_options_t* opt_in)
+{
+    g_launches = 0;
+    ss_options_t o;
+    if (opt_in) o = *opt_in; else ss_default_options(&o);
+    bool overflow = false;
+    ss_status_t st = periodogram_host(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                                      best_freq_out, best_index_out, o, &overflow);
+    if (st == SS_OK && overflow) {
+        if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "hand-over list overflow on the CTA path");
+        o.force_path = SS_PATH_BLOCK;
+        st = periodogram_host(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                              best_freq_out, best_index_out, o, &overflow);
+    }
+    return st;
 }
 
 ss_status_t ss_debug_eval(const double* times, const double* mags, const double* errs, int64_t n,
@@ -887,8 +905,8 @@ ss_status_t ss_debug_eval(const double* times, const double* mags, const double*
     p.tt = eng.tt; p.yc = eng.yc; p.w = eng.w; p.recs = eng.d_recs; p.alpha = o.alpha; p.mode = (int)mode;
     p.iper = o.iper; p.span = o.span;
     p.stage = eng.stage; p.stage_stride = eng.stage_stride;
-    if (has_listing_options(o)) block_debug_kernel<512, true><<<1, 512, 0, eng.stream>>>(p, freq, smo_out, perm_out, p_out);
-    else block_debug_kernel<512, false><<<1, 512, 0, eng.stream>>>(p, freq, smo_out, perm_out, p_out);
+    st = launch_block_debug(p, has_listing_options(o), freq, smo_out, perm_out, p_out, eng.stream);
+    if (st != SS_OK) return fail(st, "debug kernel launch failed");
     g_launches++;
     SS_CUDA(cudaGetLastError());
     SS_CUDA(cudaStreamSynchronize(eng.stream));

@@ -13,10 +13,6 @@
 
 namespace ss {
 
-constexpr int BLOCK_SLOTS = 14;  // per-eval arrays of (n+2) doubles each
-
-__host__ __device__ inline int64_t block_slot_len(int n) { return ((int64_t)n + 2) & ~(int64_t)1; }
-
 template <int T>
 struct BlockCtx {
     static constexpr int NW = T / 32;

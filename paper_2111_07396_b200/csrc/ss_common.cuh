@@ -23,7 +23,8 @@ struct ObjRec {
     int32_t ibw[3];  // window half-widths for the three spans: max(2, floor(0.5*span*n + 0.5))
     int32_t q1, q3;  // quartile indices n/4-1, 3*(q1+1)-1
     int32_t ibw_fixed;  // half-width of the caller's fixed span, 0 if span == 0
-    int32_t pad;
+    int32_t dup;        // 1 = the object has duplicated time stamps (set by the prep kernel for n <= SS_WARP_MAX_N):
+                        // its phases tie at every frequency, so the warp path hands its work items over whole
 };
 
 // Per-launch parameters.
@@ -53,11 +54,18 @@ struct EvalParams {
     unsigned int* counter;    // dynamic work counter (persistent kernels)
     double* stage;            // global staging scratch (STAGE path), stage_stride doubles per CTA
     int64_t stage_stride;
-    // evals the warp path defers to the generic kernel: (record index << 32 | k - k_begin)
+    // what the warp path hands over to the generic kernel: one eval (record index << 32 | k - k_begin) or a
+    // whole work item (DEFER_ITEM | record index << 32 | chunk index)
     unsigned long long* defer_entries;
     unsigned int* defer_count;   // [0] = appended (may exceed capacity), [1] = sticky overflow flag
     unsigned int defer_capacity;
 };
+
+constexpr unsigned long long DEFER_ITEM = 1ull << 63;
+
+// CTA-per-eval kernels (ss_block_kernel.cuh): per-eval arrays of block_slot_len(n) doubles each
+constexpr int BLOCK_SLOTS = 14;
+__host__ __device__ inline int64_t block_slot_len(int n) { return ((int64_t)n + 2) & ~(int64_t)1; }
 
 // f_k = f_min + k*df as one multiply and one add, unfused (R2).
 __device__ __forceinline__ double freq_of(double f_min, double df, int64_t k)

@@ -32,6 +32,20 @@ inline int half_width(int64_t n, double span)
     return ibw < 2 ? 2 : ibw;
 }
 
+constexpr bool WARP_IMPLEMENTED = true;
+constexpr int WARPS_PER_CTA = 8;      // frequency chunks of the warp path are multiples of this
+
+// Warp-path kernel variant of an object: (C, IBW0), C = points per lane = ceil(n/32) (at least 2), IBW0 = tweeter
+// half-width (compile-time in the kernel so the halo registers are statically indexed).  id = C*8 + IBW0.
+inline int warp_variant_for_n(int n)
+{
+    int ibw0 = half_width(n, 0.05);
+    int c = (n + 31) / 32;
+    if (c < 2) c = 2;
+    if (c == 7 && ibw0 == 6) c = 8;      // n = 220..224: the halo of 6 needs IBW0 <= C with room; served by C = 8
+    return c * 8 + ibw0;
+}
+
 // The paper's footprint model.
 inline double paper_footprint_bytes(int64_t n_t, int64_t n_f) { return 15.0 * 8.0 * (double)n_t * (double)n_f; }
 inline double paper_r_gib(int64_t n_t, int64_t n_f, int mode)

@@ -14,14 +14,10 @@
 // CTA-per-eval kernel (ss_block_kernel.cuh), so results never depend on which path ran.
 #pragma once
 #include "../../include/ss_periodogram.h"
-#include "ss_block_kernel.cuh"
 #include "ss_common.cuh"
 #include "ss_planner.h"
 
 namespace ss {
-
-constexpr bool WARP_IMPLEMENTED = true;
-constexpr int WARPS_PER_CTA = 8;      // frequency chunks are multiples of this (host side)
 
 // Launch shape per points-per-lane: warps per CTA and resident CTAs per SM (register budget =
 // 65536 / (32 * WPC * MINB), rounded down to a multiple of 8).
@@ -36,17 +32,6 @@ constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lan
 constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0
 
 template <int C> struct Pow2Ceil { static constexpr int value = C <= 2 ? 2 : (C <= 4 ? 4 : 8); };
-
-// (C, IBW0) variants: C = points per lane, IBW0 = tweeter half-width (compile-time so the halo
-// registers are statically indexed).  Returns variant id = C*8 + IBW0.
-inline int warp_variant_for_n(int n)
-{
-    int ibw0 = half_width(n, SPAN0);
-    int c = (n + 31) / 32;
-    if (c < 2) c = 2;
-    if (c == 7 && ibw0 == 6) c = 8;
-    return c * 8 + ibw0;
-}
 
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_up_d(double v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
@@ -796,6 +781,18 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     const int li = item / p.chunks_per_obj, ch = item - li * p.chunks_per_obj;
     const int ri = p.list[li];
     const ObjRec rec = p.recs[ri];
+    if (rec.dup) {
+        // duplicated time stamps: every eval of this object would tie and be deferred one by one; hand the whole
+        // work item to the generic kernel instead (it also writes the item's partial-argmax slot)
+        if (tid == 0) {
+            const unsigned pos = atomicAdd(p.defer_count, 1u);
+            if (pos < p.defer_capacity)
+                p.defer_entries[pos] = DEFER_ITEM | ((unsigned long long)ri << 32) | (unsigned long long)ch;
+            else
+                p.defer_count[1] = 1u;
+        }
+        return;
+    }
     const int n = uni(rec.n);
 
     EvalConst K;
@@ -902,105 +899,14 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     }
 }
 
-// ---- deferred evals: recomputed exactly by the generic CTA-per-eval code ------------------------
-constexpr int DEFER_T = 128;
-
-__device__ __forceinline__ unsigned long long sortable_bits(double v)
-{
-    unsigned long long u = (unsigned long long)__double_as_longlong(v);
-    return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
-}
-
-__global__ void __launch_bounds__(DEFER_T) deferred_eval_kernel(const EvalParams p, double* dval,
-                                                                unsigned long long* dmax)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int NW = DEFER_T / 32;
-    __shared__ double s_wsum[6][NW];
-    __shared__ double s_red[NW];
-    __shared__ int s_flags[4];
-    BlockCtx<DEFER_T> cx;
-    cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
-    const unsigned cnt = min(p.defer_count[0], p.defer_capacity);
-    for (unsigned e = blockIdx.x; e < cnt; e += gridDim.x) {
-        const unsigned long long ent = p.defer_entries[e];
-        const int ri = (int)(ent >> 32);
-        const int64_t k = p.k_begin + (int64_t)(ent & 0xffffffffull);
-        const ObjRec rec = p.recs[ri];
-        __syncthreads();
-        const double P = block_eval<DEFER_T, false>(p, rec, freq_of(p.f_min, p.df, k), reinterpret_cast<double*>(smem_raw),
-                                             block_slot_len(rec.n), cx, nullptr, nullptr);
-        if (threadIdx.x == 0) {
-            if (p.pgram) p.pgram[(rec.obj - p.pgram_row0) * p.pgram_row_stride + (k - p.pgram_k0)] = P;
-            dval[e] = P;
-            atomicMax(&dmax[rec.obj], sortable_bits(P));
-        }
-    }
-}
-
-__global__ void deferred_min_kernel(const EvalParams p, const double* dval, const unsigned long long* dmax,
-                                    unsigned long long* dmin)
-{
-    const unsigned cnt = min(p.defer_count[0], p.defer_capacity);
-    for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
-        const unsigned long long ent = p.defer_entries[e];
-        const int64_t obj = p.recs[(int)(ent >> 32)].obj;
-        if (sortable_bits(dval[e]) == dmax[obj]) atomicMin(&dmin[obj], (unsigned long long)(p.k_begin + (int64_t)(ent & 0xffffffffull)));
-    }
-}
-
-__global__ void deferred_merge_kernel(const EvalParams p, const double* dval, const unsigned long long* dmax,
-                                      const unsigned long long* dmin, double* best_val, int64_t* best_idx)
-{
-    const unsigned cnt = min(p.defer_count[0], p.defer_capacity);
-    for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < cnt; e += gridDim.x * blockDim.x) {
-        const unsigned long long ent = p.defer_entries[e];
-        const int64_t obj = p.recs[(int)(ent >> 32)].obj;
-        const int64_t k = p.k_begin + (int64_t)(ent & 0xffffffffull);
-        const double v = dval[e];
-        // the unique winner among this object's deferred evals folds itself into the running best
-        if (sortable_bits(v) == dmax[obj] && (unsigned long long)k == dmin[obj]) {
-            const double cv = best_val[obj];
-            const int64_t ck = best_idx[obj];
-            if (ck < 0 || v > cv || (v == cv && k < ck)) { best_val[obj] = v; best_idx[obj] = k; }
-        }
-    }
-}
-
-template <int C, int IBW0>
+template <int C, int IBW0, bool GV>
 inline ss_status_t launch_warp_variant(const EvalParams& p, int64_t n_items, cudaStream_t stream)
 {
-    cudaError_t e;
-    if (p.mode == 1) {
-        const size_t smem = warp_smem_bytes<C, true>();
-        e = cudaFuncSetAttribute(warp_kernel<C, IBW0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return SS_ERR_CUDA;
-        warp_kernel<C, IBW0, true><<<(unsigned)n_items, WarpCfg<C, true>::WPC * 32, smem, stream>>>(p);
-    } else {
-        const size_t smem = warp_smem_bytes<C, false>();
-        e = cudaFuncSetAttribute(warp_kernel<C, IBW0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return SS_ERR_CUDA;
-        warp_kernel<C, IBW0, false><<<(unsigned)n_items, WarpCfg<C, false>::WPC * 32, smem, stream>>>(p);
-    }
+    const size_t smem = warp_smem_bytes<C, GV>();
+    if (cudaFuncSetAttribute(warp_kernel<C, IBW0, GV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return SS_ERR_CUDA;
+    warp_kernel<C, IBW0, GV><<<(unsigned)n_items, WarpCfg<C, GV>::WPC * 32, smem, stream>>>(p);
     return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
-}
-
-inline ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
-{
-    switch (variant) {
-        case 2 * 8 + 2: return launch_warp_variant<2, 2>(p, n_items, stream);
-        case 3 * 8 + 2: return launch_warp_variant<3, 2>(p, n_items, stream);
-        case 4 * 8 + 2: return launch_warp_variant<4, 2>(p, n_items, stream);
-        case 4 * 8 + 3: return launch_warp_variant<4, 3>(p, n_items, stream);
-        case 5 * 8 + 3: return launch_warp_variant<5, 3>(p, n_items, stream);
-        case 5 * 8 + 4: return launch_warp_variant<5, 4>(p, n_items, stream);
-        case 6 * 8 + 4: return launch_warp_variant<6, 4>(p, n_items, stream);
-        case 6 * 8 + 5: return launch_warp_variant<6, 5>(p, n_items, stream);
-        case 7 * 8 + 5: return launch_warp_variant<7, 5>(p, n_items, stream);
-        case 8 * 8 + 5: return launch_warp_variant<8, 5>(p, n_items, stream);
-        case 8 * 8 + 6: return launch_warp_variant<8, 6>(p, n_items, stream);
-        default: return SS_ERR_UNSUPPORTED;
-    }
 }
 
 }  // namespace ss

@@ -524,3 +524,154 @@ def test_workspace_is_reused_between_calls_and_can_be_released(ss):
     assert torch.cuda.mem_get_info()[0] >= free0 - (1 << 20)
     after = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, CV)
     assert np.array_equal(after.pgram, first.pgram)
+
+
+# ------------------------------------------------------------------ round 2: gaps the round-1 review found
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_warp_variants_upper_range(ss, mode):
+    """n = 201..256 on the path the library picks by itself: warp_kernel<7,5> serves 193..219 and <8,6> 220..256
+    (220..224 because the tweeter half-width 6 does not fit 7 points per lane).  Full parity against the
+    definition oracle, best index included."""
+    rng = np.random.default_rng(2024)
+    ns = [201, 219, 220, 224, 225, 240, 255, 256]
+    T, Y, E = [], [], []
+    for i, n in enumerate(ns):
+        assert ss.path_for_n(n) == ss.PATH_WARP
+        t = np.sort(rng.integers(0, 30, size=n) + rng.uniform(0.0, 0.33, size=n))
+        P = np.exp(rng.uniform(np.log(0.1), np.log(2.0)))
+        y = 15 + rng.uniform(0.1, 1.0) * np.sin(2 * np.pi * t / P + i) + rng.normal(0, 0.05, size=n)
+        T.append(t); Y.append(y); E.append(rng.uniform(0.02, 0.1, size=n))
+    off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
+    cat = ss_inputs.Catalog("upper", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
+                            0.5, 24.0, 193, np.full(len(ns), np.nan))
+    res, ref = run_both(ss, cat, mode, oracle.DEFINITION)
+    check_parity(cat, res.pgram, ref, mode, label="n=201..256")
+    check_best(ref, res.best_index, res.best_freq, cat)
+
+
+def _commensurate_catalog():
+    """Quarter-day time stamps (no duplicates): at every frequency j/64 with even j many phases tie exactly, so
+    the warp path hands those evals over one by one; the signal has period 1 d, so the PEAK (f = 1.0 = f_32) is
+    one of them.  Second object: the same with duplicated time stamps (handed over as whole work items).  Third:
+    an ordinary object."""
+    rng = np.random.default_rng(99)
+    m = np.sort(rng.choice(120, size=100, replace=False))
+    t1 = m / 4.0
+    y1 = 15 + 0.4 * np.sin(2 * np.pi * t1 / 1.0 + 0.3) + rng.normal(0, 0.02, size=100)
+    t2 = t1.copy(); t2[17] = t2[16]; t2[60] = t2[58]
+    y2 = 15 + 0.4 * np.sin(2 * np.pi * t2 / 1.0 + 1.1) + rng.normal(0, 0.02, size=100)
+    t3 = np.sort(rng.uniform(0, 30, size=77))
+    y3 = 15 + 0.3 * np.sin(2 * np.pi * t3 / 1.31) + rng.normal(0, 0.03, size=77)
+    off = np.array([0, 100, 200, 277], dtype=np.int64)
+    return ss_inputs.Catalog("commensurate", np.concatenate([t1, t2, t3]), np.concatenate([y1, y2, y3]),
+                             np.concatenate([np.full(100, 0.02), np.full(100, 0.02), np.full(77, 0.03)]), off,
+                             0.5, 1.5, 64, np.array([1.0, 1.0, 1 / 1.31]))
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_best_index_when_the_peak_is_a_handed_over_eval(ss, mode):
+    """The argmax has three sources on the warp path: the warp kernel's own partial maxima, single evals recomputed
+    by the generic kernel (merged through atomics) and whole work items recomputed by it (objects with duplicated
+    time stamps).  Here the true peak of objects 0 and 1 is a handed-over eval: values AND best index against the
+    oracle, on both entry points and with forced frequency tiles."""
+    import torch
+    cat = _commensurate_catalog()
+    assert oracle.freq(cat.f_min, cat.f_max, cat.n_freq, 32) == 1.0
+    ref, _, bi_ref = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                                        mode=mode, variant=oracle.DEFINITION)
+    assert bi_ref[0] == 32 and bi_ref[1] == 32                  # the peak sits on the tied frequency
+    for opts in (dict(), dict(freq_tile=16), dict(freq_tile=5)):
+        res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
+        check_parity(cat, res.pgram, ref, mode, label=f"handed-over {opts}")
+        check_best(ref, res.best_index, res.best_freq, cat)
+    dev = torch.device("cuda")
+    t = torch.as_tensor(cat.times, device=dev); y = torch.as_tensor(cat.mags, device=dev)
+    e = torch.as_tensor(cat.errs, device=dev); off = torch.as_tensor(cat.offsets, device=dev)
+    for want_pg in (True, False):
+        pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev) if want_pg else None
+        bf = torch.empty(cat.n_objects, dtype=torch.float64, device=dev)
+        bi = torch.empty(cat.n_objects, dtype=torch.int64, device=dev)
+        ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, bf, bi)
+        if want_pg:
+            check_parity(cat, pg.cpu().numpy(), ref, mode, label="handed-over/device")
+        check_best(ref, bi.cpu().numpy(), bf.cpu().numpy(), cat)
+    # the generic kernel serves the handed-over work with the code of the CTA path: identical bits
+    blk = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                         force_path=ss.PATH_BLOCK)
+    assert np.array_equal(res.pgram[1], blk.pgram[1])           # the object with duplicated time stamps, whole
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_hand_over_list_overflow_repeats_the_call_on_the_cta_path(ss, mode):
+    """With the list shrunk to 8 entries (test hook `defer_capacity`) the commensurate catalog overflows it: the
+    call must then return exactly what the CTA path returns, periodogram and best index, on both entry points."""
+    import torch
+    cat = _commensurate_catalog()
+    blk = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                         force_path=ss.PATH_BLOCK)
+    n_block = ss.last_launch_count()
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                         defer_capacity=8)
+    assert np.array_equal(res.pgram, blk.pgram) and np.array_equal(res.best_index, blk.best_index)
+    assert np.array_equal(res.best_freq, blk.best_freq)
+    dev = torch.device("cuda")
+    t = torch.as_tensor(cat.times, device=dev); y = torch.as_tensor(cat.mags, device=dev)
+    e = torch.as_tensor(cat.errs, device=dev); off = torch.as_tensor(cat.offsets, device=dev)
+    pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev)
+    bi = torch.empty(cat.n_objects, dtype=torch.int64, device=dev)
+    ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, None, bi,
+                      ss.default_options(defer_capacity=8))
+    assert np.array_equal(pg.cpu().numpy(), blk.pgram) and np.array_equal(bi.cpu().numpy(), blk.best_index)
+    # and a list that is long enough is not an overflow: the warp path's own values stand (parity, not bits)
+    ok = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                        defer_capacity=4096)
+    assert np.allclose(ok.pgram, blk.pgram, rtol=1e-9, atol=1e-12) and n_block > 0
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_config4_full_size_sampled(ss, mode):
+    """Config 4 at BASELINE.json's full size (1,000 objects of 500..2,000 points x 500,000 frequencies, 4 GB of
+    output: the config whose frequency range the planner tiles), device entry point, default options -- the launch
+    configuration of `bench.py --config 4`.  Checked on properties that hold at any size, on 300 random
+    (object, k) evals the definition oracle computes one by one, and on two whole rows (shortest and longest
+    object) with their best index."""
+    import torch
+    cat = ss_inputs.config4()
+    assert cat.n_objects == 1000 and cat.n_freq == 500000
+    dev = torch.device("cuda")
+    t = torch.as_tensor(cat.times, device=dev); y = torch.as_tensor(cat.mags, device=dev)
+    e = torch.as_tensor(cat.errs, device=dev); off = torch.as_tensor(cat.offsets, device=dev)
+    pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev)
+    bf = torch.empty(cat.n_objects, dtype=torch.float64, device=dev)
+    bi = torch.empty(cat.n_objects, dtype=torch.int64, device=dev)
+    ss.ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, bf, bi)
+    torch.cuda.synchronize()
+    assert ss.last_launch_count() > 0
+    assert bool(torch.isfinite(pg).all()) and float(pg.max()) <= 1.0 + 1e-12
+    rowmax, rowarg = pg.max(dim=1)
+    assert torch.equal(rowarg, bi)
+    assert torch.equal(bf, cat.f_min + bi.to(torch.float64) * ((cat.f_max - cat.f_min) / cat.n_freq))
+    rng = np.random.default_rng(4321)
+    objs = rng.integers(0, cat.n_objects, size=300); ks = rng.integers(0, cat.n_freq, size=300)
+    got = pg[torch.as_tensor(objs, device=dev), torch.as_tensor(ks, device=dev)].cpu().numpy()
+    ambiguous = 0
+    for o, k, g in zip(objs, ks, got):
+        tt, yy, ee = cat.obj(int(o))
+        r = oracle.eval_one(tt, yy, ee, oracle.freq(cat.f_min, cat.f_max, cat.n_freq, int(k)), mode=mode,
+                            variant=oracle.DEFINITION, alt_threshold=1e-7)
+        if abs(g - r["P"]) <= _tol(r["P"]):
+            continue
+        assert r["margin"] < 1e-9 and abs(g - r["P_alt"]) <= _tol(r["P_alt"]), (o, k, g, r["P"], r["margin"])
+        ambiguous += 1
+    assert ambiguous <= 2
+    ns = np.diff(cat.offsets)
+    rows = [int(np.argmin(ns)), int(np.argmax(ns))]
+    sub = cat.subset(rows)
+    ref, _, _ = oracle.periodogram(sub.times, sub.mags, sub.errs, sub.offsets, sub.f_min, sub.f_max, sub.n_freq,
+                                   mode=mode, variant=oracle.FAST)
+    got_rows = pg[torch.as_tensor(rows, device=dev)].cpu().numpy()
+    check_parity(sub, got_rows, ref, mode, max_ambiguous=6, label="cfg4-full")
+    check_best(ref, bi[torch.as_tensor(rows, device=dev)].cpu().numpy(),
+               bf[torch.as_tensor(rows, device=dev)].cpu().numpy(), sub)
+    del pg
+    torch.cuda.empty_cache()
