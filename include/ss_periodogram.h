@@ -56,10 +56,13 @@ typedef enum {
     SS_PATH_AUTO = 0,
     SS_PATH_WARP = 1,  /* one warp per (object, frequency); n <= SS_WARP_MAX_N; registers + shuffles   */
     SS_PATH_BLOCK = 2, /* one CTA per (object, frequency); per-eval arrays in shared memory            */
-    SS_PATH_STAGE = 3  /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
+    SS_PATH_STAGE = 3, /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
+    SS_PATH_GROUP = 4  /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_MAX_N;
+                          points in registers, prefix sums in shared memory, smooths in tensor memory     */
 } ss_path_t;
 
 #define SS_WARP_MAX_N 256
+#define SS_GROUP_MAX_N 2055
 
 typedef struct {
     double alpha;           /* bass enhancement.  Default 9.0.                 */
@@ -158,7 +161,8 @@ size_t ss_workspace_bytes(int64_t n_points_total, int64_t max_n, int64_t n_objec
 double ss_paper_footprint_bytes(int64_t n_t, int64_t n_f);
 int64_t ss_paper_batches(int64_t n_t, int64_t n_f, ss_mode_t mode, double device_gib, double beta);
 
-/* Path class the library picks for an object of n points (SS_PATH_WARP/BLOCK/STAGE). */
+/* Path class the library picks for an object of n points (SS_PATH_WARP / GROUP / STAGE; SS_PATH_BLOCK serves
+ * the listing's options and whatever the other paths hand over). */
 int ss_path_for_n(int64_t n, ss_mode_t mode);
 
 /* ------------------------------------------------------------------ diagnostics */

@@ -150,16 +150,19 @@ __device__ __forceinline__ double prep_block_sum(double v, double* red)
     return s;
 }
 
+// raw_off[ri]: the object's first element in the caller's arrays; recs[ri].off: its first element in tt / yc / w
+// (every object starts at an even element there: 16-byte aligned for the bulk copies of the group kernel).
 __global__ void __launch_bounds__(PREP_T) prep_kernel(const double* __restrict__ times,
                                                       const double* __restrict__ mags,
                                                       const double* __restrict__ errs, ObjRec* recs,
+                                                      const int64_t* __restrict__ raw_off,
                                                       int n_recs, double* tt, double* yc, double* w,
                                                       int* flag)
 {
     __shared__ double red[PREP_T / 32];
     const int ri = blockIdx.x;
     if (ri >= n_recs) return;
-    const int64_t off = recs[ri].off;
+    const int64_t off = raw_off[ri], poff = recs[ri].off;
     const int n = recs[ri].n;
     const int tid = threadIdx.x;
     double tmin = INFINITY;
@@ -194,8 +197,8 @@ __global__ void __launch_bounds__(PREP_T) prep_kernel(const double* __restrict__
     for (int j = tid; j < n; j += PREP_T) {
         double e = errs[off + j];
         double wj = 1.0 / (e * e);
-        w[off + j] = wj;
-        tt[off + j] = times[off + j] - tmin;
+        w[poff + j] = wj;
+        tt[poff + j] = times[off + j] - tmin;
         sw += wj;
         swy += wj * (mags[off + j] - y0);
     }
@@ -205,11 +208,12 @@ __global__ void __launch_bounds__(PREP_T) prep_kernel(const double* __restrict__
     double c0 = 0.0;
     for (int j = tid; j < n; j += PREP_T) {
         double d = mags[off + j] - ybar;
-        yc[off + j] = d;
-        c0 += w[off + j] * d * d;
+        yc[poff + j] = d;
+        c0 += w[poff + j] * d * d;
     }
     c0 = prep_block_sum(c0, red);
     if (tid == 0) {
+        if (n & 1) { tt[poff + n] = 0.0; yc[poff + n] = 0.0; w[poff + n] = 0.0; }      // the padding element
         recs[ri].chi0 = c0;
         recs[ri].ybar = ybar;
     }
@@ -330,6 +334,9 @@ struct Engine {
     std::vector<int64_t> off;
     std::vector<ObjRec> recs;          // objects with n >= 5
     std::vector<int64_t> degenerate;   // object indices with n < 5
+    std::vector<int64_t> raw_off;      // per record: first element in the caller's arrays
+    int64_t padded_total = 0;          // elements of tt / yc / w (every object padded to an even length)
+    int64_t* d_raw_off = nullptr;
     int max_n = 0;
     // device workspace
     char* ws = nullptr;
@@ -440,7 +447,9 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         if (n > (int64_t)1 << 24) return fail(SS_ERR_UNSUPPORTED, "object %lld has %lld points (limit 2^24)", (long long)i, (long long)n);
         if (n < MIN_POINTS) { degenerate.push_back(i); continue; }
         ObjRec r{};
-        r.off = off[i]; r.obj = i; r.n = (int32_t)n;
+        r.off = padded_total; r.obj = i; r.n = (int32_t)n;
+        raw_off.push_back(off[i]);
+        padded_total += (n + 1) & ~(int64_t)1;
         r.ibw[0] = half_width(n, SPAN0); r.ibw[1] = half_width(n, SPAN1); r.ibw[2] = half_width(n, SPAN2);
         r.q1 = (int32_t)(n / 4 - 1); r.q3 = 3 * (r.q1 + 1) - 1;
         r.ibw_fixed = o.span > 0.0 ? half_width(n, o.span) : 0;
@@ -476,11 +485,13 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (r.obj < o0 || r.obj >= o1) continue;
             int path = o.force_path != SS_PATH_AUTO ? o.force_path : path_for_n(r.n, md);
             // periodic windows and the fixed span live in the generic CTA-per-eval code only
-            if (path == SS_PATH_WARP && has_listing_options(o)) path = SS_PATH_BLOCK;
-            if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_BLOCK;
+            if ((path == SS_PATH_WARP || path == SS_PATH_GROUP) && has_listing_options(o)) path = SS_PATH_BLOCK;
+            if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_GROUP;
+            if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N) path = SS_PATH_STAGE;
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
             if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
+            else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
             else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);
             ClassList& c = find(path, variant);
@@ -504,8 +515,9 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     n_counters = 64;
     size_t b = 0;
     auto carve = [&](size_t bytes) { size_t o_ = b; b += align_up(bytes); return o_; };
-    size_t o_tt = carve(8 * (size_t)total), o_yc = carve(8 * (size_t)total), o_w = carve(8 * (size_t)total);
+    size_t o_tt = carve(8 * (size_t)padded_total), o_yc = carve(8 * (size_t)padded_total), o_w = carve(8 * (size_t)padded_total);
     size_t o_recs = carve(sizeof(ObjRec) * std::max<size_t>(recs.size(), 1));
+    size_t o_raw = carve(8 * std::max<size_t>(recs.size(), 1));
     size_t o_list = carve(4 * std::max<size_t>(all_lists.size(), 1));
     size_t o_deg = carve(8 * std::max<size_t>(degenerate.size(), 1));
     size_t o_bv = carve(8 * (size_t)std::max<int64_t>(n_obj, 1)), o_bi = carve(8 * (size_t)std::max<int64_t>(n_obj, 1));
@@ -520,6 +532,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         return fail(SS_ERR_OUT_OF_MEMORY, "workspace %zu B exceeds the cap %zu B", ws_bytes, cap);
     SS_CUDA(g_pool.acquire(ws_bytes, &ws));
     tt = (double*)(ws + o_tt); yc = (double*)(ws + o_yc); w = (double*)(ws + o_w);
+    d_raw_off = (int64_t*)(ws + o_raw);
     d_recs = (ObjRec*)(ws + o_recs); d_list = (int32_t*)(ws + o_list); d_degen = (int64_t*)(ws + o_deg);
     best_val = (double*)(ws + o_bv); best_idx = (int64_t*)(ws + o_bi);
     part_val = (double*)(ws + o_pv); part_idx = (int64_t*)(ws + o_pi);
@@ -531,6 +544,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
     extra = ws + o_extra;
 
     if (!recs.empty()) SS_CUDA(cudaMemcpyAsync(d_recs, recs.data(), sizeof(ObjRec) * recs.size(), cudaMemcpyHostToDevice, stream));
+    if (!recs.empty()) SS_CUDA(cudaMemcpyAsync(d_raw_off, raw_off.data(), 8 * raw_off.size(), cudaMemcpyHostToDevice, stream));
     if (!all_lists.empty()) SS_CUDA(cudaMemcpyAsync(d_list, all_lists.data(), 4 * all_lists.size(), cudaMemcpyHostToDevice, stream));
     if (!degenerate.empty()) SS_CUDA(cudaMemcpyAsync(d_degen, degenerate.data(), 8 * degenerate.size(), cudaMemcpyHostToDevice, stream));
     SS_CUDA(cudaMemsetAsync(counters, 0, 4 * (size_t)n_counters, stream));
@@ -541,7 +555,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         g_launches++;
     }
     if (!recs.empty()) {
-        prep_kernel<<<(unsigned)recs.size(), PREP_T, 0, stream>>>(times, mags, errs, d_recs, (int)recs.size(), tt, yc, w, flag);
+        prep_kernel<<<(unsigned)recs.size(), PREP_T, 0, stream>>>(times, mags, errs, d_recs, d_raw_off, (int)recs.size(), tt, yc, w, flag);
         g_launches++;
         SS_CUDA(cudaGetLastError());
     }
@@ -588,7 +602,8 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             SS_CUDA(g_pool.event(true, &ev1));
             prof.emplace_back(ev0, ev1);
         }
-        if (c.path != SS_PATH_WARP) {
+        const bool hands_over = c.path == SS_PATH_WARP || c.path == SS_PATH_GROUP;   // one CTA per item, hand-over list
+        if (!hands_over) {
             SS_CUDA(cudaMemsetAsync(p.counter, 0, 4, stream));
             next_counter++;
         }
@@ -596,6 +611,9 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         if (c.path == SS_PATH_WARP) {
             ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        } else if (c.path == SS_PATH_GROUP) {
+            ss_status_t st = launch_group_kernel(p, c.variant, n_items, stream);
+            if (st != SS_OK) return fail(st, "group kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else {
             const int threads = c.path == SS_PATH_STAGE ? 512 : (c.variant == 2 ? 512 : (c.variant == 3 ? 128 : 256));
             ss_status_t st = launch_block_kernel(p, c.path, threads, c.max_n, has_listing_options(opt), n_items, sm_count, stream);
@@ -603,13 +621,13 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         }
         if (ev1) SS_CUDA(cudaEventRecord(ev1, stream));
         g_launches++;
-        if (c.path == SS_PATH_WARP) {
-            // what the warp path handed over (tied / misordered phases, leave-one-out denominator <= 0, objects
+        if (hands_over) {
+            // what the warp / group path handed over (tied / misordered phases, leave-one-out denominator <= 0, objects
             // with duplicated time stamps): recompute with the generic code, patch the periodogram; whole items
             // write their partial-argmax slot (hence before the fold below), single evals fold into the running best
             SS_CUDA(cudaMemsetAsync(dmax, 0, 8 * (size_t)n_objects, stream));
             SS_CUDA(cudaMemsetAsync(dmin, 0xff, 8 * (size_t)n_objects, stream));
-            ss_status_t st = launch_deferred_eval(p, defer_val, dmax, sm_count, stream);
+            ss_status_t st = launch_deferred_eval(p, defer_val, dmax, c.max_n, sm_count, stream);
             if (st != SS_OK) return fail(st, "deferred kernel launch failed");
             g_launches++;
         }
@@ -617,7 +635,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             d_recs, p.list, p.n_list, (int)cpo, p.chunks_total, 0, part_val, part_idx, best_val, best_idx);
         g_launches++;
         SS_CUDA(cudaGetLastError());
-        if (c.path == SS_PATH_WARP) {
+        if (hands_over) {
             ss_status_t st = launch_deferred_merge(p, defer_val, dmax, dmin, best_val, best_idx, sm_count, stream);
             if (st != SS_OK) return fail(st, "deferred merge launch failed");
             g_launches += 2;

@@ -71,6 +71,21 @@ ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items
          : g == 1 ? launch_warp_tu_0_1(p, variant, n_items, stream) : launch_warp_tu_0_2(p, variant, n_items, stream);
 }
 
+// ---- group-kernel translation units (ss_group_tu.cu) -------------------------------------------------
+#define SS_DECL(gv, g) ss_status_t launch_group_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
+SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
+#undef SS_DECL
+
+ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
+{
+    const int g = variant / 8, c = variant % 8;
+    if (p.mode == 1)
+        return g == 4 ? launch_group_tu_1_4(p, c, n_items, stream)
+             : g == 8 ? launch_group_tu_1_8(p, c, n_items, stream) : launch_group_tu_1_16(p, c, n_items, stream);
+    return g == 4 ? launch_group_tu_0_4(p, c, n_items, stream)
+         : g == 8 ? launch_group_tu_0_8(p, c, n_items, stream) : launch_group_tu_0_16(p, c, n_items, stream);
+}
+
 // ---- CTA-per-eval kernels ---------------------------------------------------------------------------
 ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int max_n, bool opt, int64_t n_items,
                                 int sm_count, cudaStream_t stream)
@@ -189,10 +204,10 @@ __global__ void deferred_merge_kernel(const EvalParams p, const double* dval, co
     }
 }
 
-ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int sm_count,
+ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, int sm_count,
                                  cudaStream_t stream)
 {
-    const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(SS_WARP_MAX_N) * 8;
+    const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(max_n) * 8;
     if (cudaFuncSetAttribute(deferred_eval_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return SS_ERR_CUDA;
     deferred_eval_kernel<<<sm_count * 4, DEFER_T, smem, stream>>>(p, dval, dmax);

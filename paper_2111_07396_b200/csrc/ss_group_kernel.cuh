@@ -1,0 +1,608 @@
+// ss_group_kernel.cuh -- G warps per (object, frequency) eval, 256 < n <= 2,055 (SS_PATH_GROUP).
+//
+// The warp-per-eval design (ss_warp_kernel.cuh) carried over to light curves that do not fit one warp: the CTA
+// (G = 4, 8 or 16 warps) owns one eval at a time, thread t owns the C consecutive phase-ordered points
+// j = t*C .. t*C+C-1 in registers, and the warps meet only where the method forces them to:
+//   fold -> 32-bit keys (phase bits | index) -> blocked bitonic network: inside a warp on registers and shuffles,
+//           across warps through one shared-memory exchange + one barrier per step ->
+//   gather of the exact phases, repair of the order inside a quantisation bucket (adjacent swap), exact-order check ->
+//   prefix sums of the weighted moments: lane-local + Kogge-Stone inside the warp, ONE carry exchange across warps,
+//           stored pair-interleaved and transposed ([slot][thread]) so every window-end access is conflict-free ->
+//   all three spans by differences of those prefix arrays; CV (Listing 1) keeps the primary smooths
+//           and the tweeter x-moments parked in tensor memory; GV (R12) needs no second pass -> chi2 -> P.
+// The object's tt / yc / w are staged into shared memory ONCE per work item by three 1-D bulk copies
+// (cp.async.bulk + mbarrier).  32 values of P are stashed and stored as one coalesced row segment.
+// Evals this path cannot decide exactly (tied phases, a bucket that one adjacent swap does not settle, a
+// leave-one-out denominator <= 0) are handed to the generic CTA-per-eval kernel through the same list the warp path
+// uses, so results never depend on which path ran.
+#pragma once
+#include "ss_warp_kernel.cuh"
+
+namespace ss {
+
+template <int G, int C> struct GroupCfg {
+    static constexpr int NT = 32 * G;               // threads
+    static constexpr int NP = NT * C;               // capacity in points
+    static constexpr int ROW = NT + 1;              // row of a transposed prefix array: NT threads + the total
+    static constexpr int MINB = G == 4 ? 4 : (G == 8 ? 2 : 1);      // 16 warps per SM at 128 registers
+    static constexpr int IDX_BITS = NP <= 512 ? 9 : (NP <= 1024 ? 10 : (NP <= 2048 ? 11 : 12));
+    static constexpr unsigned IDX_MASK = (1u << IDX_BITS) - 1u;
+    // tensor memory per warp: 14C columns of parked doubles (A0, A1, A2, tweeter isw / xbar / g, y) + 6C window indices
+    static constexpr uint32_t TCOLS_WARP = 20 * C;
+    static constexpr uint32_t TCOLS_NEED = TCOLS_WARP * (G / 4);
+    static constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
+    static_assert(TCOLS * MINB <= 512, "tensor memory over-subscribed");
+};
+
+template <> __device__ __forceinline__ void local_sort<2>(unsigned (&k)[2]) { cex32(k[0], k[1]); }
+template <> __device__ __forceinline__ void local_sort<4>(unsigned (&k)[4])
+{
+    cex32(k[0], k[1]); cex32(k[2], k[3]); cex32(k[0], k[2]); cex32(k[1], k[3]); cex32(k[1], k[2]);
+}
+
+// ---- 1-D bulk copy global -> shared with mbarrier completion (PTX cp.async.bulk; SASS UBLKCP) ------------
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+                 "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+}
+// bytes: multiple of 16; src and dst 16-byte aligned
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src), "r"(bytes),
+                    "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
+}
+
+template <int G, int C, bool GV>
+inline size_t group_smem_bytes()
+{
+    using Cfg = GroupCfg<G, C>;
+    // object arrays (3 x NP doubles) + 3 pair-prefix arrays of C*ROW double2 (the sort's exchange buffers overlay them)
+    return (size_t)3 * Cfg::NP * 8 + (size_t)3 * C * Cfg::ROW * 16;
+}
+
+// Exclusive prefix sums of two streams over the whole CTA (C values per thread, blocked), stored interleaved and
+// transposed: E[(j % C)*ROW + j/C] = (sum_{i<j} a_i, sum_{i<j} b_i).  Phase 1 (before the barrier): lane-local sums,
+// Kogge-Stone over the warp, the warp's totals to `tot`; phase 2 (after it): the carry of the warps in front.
+struct PairScan { double ra, rb, ia, ib; };
+template <int C>
+__device__ __forceinline__ PairScan pair_scan_begin(const double (&a)[C], const double (&b)[C], double2* tot, int warp,
+                                                    int lane, const ScanMask& mk)
+{
+    PairScan s;
+    s.ra = a[0]; s.rb = b[0];
+#pragma unroll
+    for (int i = 1; i < C; i++) { s.ra += a[i]; s.rb += b[i]; }
+    s.ia = s.ra; s.ib = s.rb;
+#pragma unroll
+    for (int i = 0; i < 5; i++) { scan_step(s.ia, i, mk); scan_step(s.ib, i, mk); }
+    if (lane == 31) tot[warp] = make_double2(s.ia, s.ib);
+    return s;
+}
+template <int G, int C>
+__device__ __forceinline__ void pair_scan_finish(const PairScan& s, const double (&a)[C], const double (&b)[C],
+                                                 const double2* tot, double2* E, int warp, int tid)
+{
+    constexpr int ROW = GroupCfg<G, C>::ROW;
+    double ca = 0.0, cb = 0.0;
+    for (int q = 0; q < warp; q++) { const double2 t = tot[q]; ca += t.x; cb += t.y; }      // warp-uniform: broadcast loads
+    double xa = ca + (s.ia - s.ra), xb = cb + (s.ib - s.rb);
+#pragma unroll
+    for (int i = 0; i < C; i++) {
+        E[i * ROW + tid] = make_double2(xa, xb);
+        xa += a[i]; xb += b[i];
+    }
+    if (tid == 32 * G - 1) E[32 * G] = make_double2(xa, xb);       // position NP lives at row 0, column NT
+}
+// one stream, plain doubles (row length ROW doubles)
+struct OneScan { double ra, ia; };
+template <int C>
+__device__ __forceinline__ OneScan one_scan_begin(const double (&a)[C], double* tot, int warp, int lane, const ScanMask& mk)
+{
+    OneScan s;
+    s.ra = a[0];
+#pragma unroll
+    for (int i = 1; i < C; i++) s.ra += a[i];
+    s.ia = s.ra;
+#pragma unroll
+    for (int i = 0; i < 5; i++) scan_step(s.ia, i, mk);
+    if (lane == 31) tot[warp] = s.ia;
+    return s;
+}
+template <int G, int C>
+__device__ __forceinline__ void one_scan_finish(const OneScan& s, const double (&a)[C], const double* tot, double* E,
+                                                int warp, int tid)
+{
+    constexpr int ROW = GroupCfg<G, C>::ROW;
+    double ca = 0.0;
+    for (int q = 0; q < warp; q++) ca += tot[q];
+    double xa = ca + (s.ia - s.ra);
+#pragma unroll
+    for (int i = 0; i < C; i++) { E[i * ROW + tid] = xa; xa += a[i]; }
+    if (tid == 32 * G - 1) E[32 * G] = xa;
+}
+
+// Exchange of the C keys with thread (tid ^ mask); REV: the partner's slots in reverse order (mirror step).
+// mask < 32: shuffles.  Otherwise through shared memory: kb = this step's exchange buffer (two alternate, so one
+// barrier per step is enough).
+template <int G, int C, bool REV>
+__device__ __forceinline__ void key_exchange(const unsigned (&key)[C], unsigned (&other)[C], int mask, int tid,
+                                             unsigned* kb)
+{
+    constexpr int NT = 32 * G;
+    if (mask < 32) {
+#pragma unroll
+        for (int s = 0; s < C; s++) other[s] = __shfl_xor_sync(0xffffffffu, key[REV ? C - 1 - s : s], mask);
+    } else {
+#pragma unroll
+        for (int s = 0; s < C; s++) kb[s * NT + tid] = key[s];
+        __syncthreads();
+        const int pt = tid ^ mask;
+#pragma unroll
+        for (int s = 0; s < C; s++) other[s] = kb[(REV ? C - 1 - s : s) * NT + pt];
+    }
+}
+
+// Blocked bitonic sort of NT*C keys over the CTA (position = tid*C + s): the network of warp_sort_any with 32*G lanes.
+template <int G, int C>
+__device__ __forceinline__ void group_sort(unsigned (&key)[C], int tid, unsigned* kbuf)
+{
+    constexpr int NT = 32 * G;
+    int flip = 0;
+    local_sort<C>(key);
+#pragma unroll
+    for (int k = 2; k <= NT; k <<= 1) {
+        {
+            const bool lower = (tid & (k >> 1)) == 0;
+            unsigned other[C];
+            key_exchange<G, C, true>(key, other, k - 1, tid, kbuf + flip * NT * C);
+            if (k - 1 >= 32) flip ^= 1;
+#pragma unroll
+            for (int s = 0; s < C; s++) key[s] = lower ? min(key[s], other[s]) : max(key[s], other[s]);
+        }
+#pragma unroll
+        for (int m = k >> 2; m >= 1; m >>= 1) {
+            const bool lower = (tid & m) == 0;
+            unsigned other[C];
+            key_exchange<G, C, false>(key, other, m, tid, kbuf + flip * NT * C);
+            if (m >= 32) flip ^= 1;
+#pragma unroll
+            for (int s = 0; s < C; s++) key[s] = lower ? min(key[s], other[s]) : max(key[s], other[s]);
+        }
+        local_sort<C>(key);
+    }
+}
+
+// Per-object constants (CTA-uniform).
+struct GroupConst {
+    int n;
+    const double* kc;        // shared: gk[span][p-1] = 1/(1 - p/K_span) (6 values), then chi0, 1/chi0
+    int q1t, q1s, q3t, q3s;  // owners (thread, slot) of the quartile points
+    int bass; double bexp;
+};
+
+// ------------------------------------------------------------------------------------------------
+// Kernel: one CTA = one work item (object, chunk of frequencies), evals one after the other.
+// ------------------------------------------------------------------------------------------------
+template <int G, int C, bool GV>
+__global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) group_kernel(const EvalParams p)
+{
+    using Cfg = GroupCfg<G, C>;
+    constexpr int NT = Cfg::NT, NP = Cfg::NP, ROW = Cfg::ROW, ASZ = C * ROW;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ __align__(16) double2 s_tot[3][G];          // warp totals of up to three pair scans
+    __shared__ double s_red[G];
+    __shared__ double s_edge[2][G][2];                       // [first|last][warp]{phase, index} across warp boundaries
+    __shared__ double s_q[2];                                // phases of the quartile points
+    __shared__ double s_kc[8];
+    __shared__ __align__(8) uint64_t s_bar;
+    __shared__ uint32_t s_tmem;
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // provably warp-uniform (see warp_kernel)
+    const int item = blockIdx.x;
+    const int li = item / p.chunks_per_obj, ch = item - li * p.chunks_per_obj;
+    const int ri = p.list[li];
+    const ObjRec rec = p.recs[ri];
+    if (rec.dup) {
+        // duplicated time stamps: every eval ties; the generic kernel takes the whole work item
+        if (tid == 0) {
+            const unsigned pos = atomicAdd(p.defer_count, 1u);
+            if (pos < p.defer_capacity)
+                p.defer_entries[pos] = DEFER_ITEM | ((unsigned long long)ri << 32) | (unsigned long long)ch;
+            else
+                p.defer_count[1] = 1u;
+        }
+        return;
+    }
+    const int n = rec.n;
+
+    double* o_tt = reinterpret_cast<double*>(smem_raw);
+    double* o_y = o_tt + NP;
+    double* o_w = o_y + NP;
+    double2* E01 = reinterpret_cast<double2*>(smem_raw + (size_t)3 * NP * 8);      // (w, wx)      | residual 0 | spans
+    double2* E23 = E01 + ASZ;                                                      // (wxx, wy)    | residual 1 | final
+    double2* E45 = E23 + ASZ;                                                      // (wxy[, wyy]) | residual 2
+    unsigned* kbuf = reinterpret_cast<unsigned*>(E01);                             // sort exchange (2 x NT*C words)
+
+    // ---- stage the object once per work item: three bulk copies, one mbarrier
+    if (tid == 0) {
+        mbar_init(&s_bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                     :: "r"((uint32_t)__cvta_generic_to_shared(&s_tmem)), "n"(Cfg::TCOLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    if (tid == 0) {
+        const unsigned bytes = (unsigned)(((n + 1) & ~1) * 8);      // the workspace pads every object to an even length
+        mbar_expect_tx(&s_bar, 3 * bytes);
+        bulk_g2s(o_tt, p.tt + rec.off, bytes, &s_bar);
+        bulk_g2s(o_y, p.yc + rec.off, bytes, &s_bar);
+        bulk_g2s(o_w, p.w + rec.off, bytes, &s_bar);
+    }
+
+    const int ibw0 = rec.ibw[0], ibw1 = rec.ibw[1], ibw2 = rec.ibw[2];
+    const int K0 = min(2 * ibw0 + 1, n), K1 = min(2 * ibw1 + 1, n), K2 = min(2 * ibw2 + 1, n);
+    GroupConst K;
+    K.n = n;
+    K.q1t = rec.q1 / C; K.q1s = rec.q1 % C; K.q3t = rec.q3 / C; K.q3s = rec.q3 % C;
+    if (tid == 0) {
+        s_kc[0] = 1.0 / (1.0 - 1.0 / (double)K0); s_kc[1] = 1.0 / (1.0 - 2.0 / (double)K0);
+        s_kc[2] = 1.0 / (1.0 - 1.0 / (double)K1); s_kc[3] = 1.0 / (1.0 - 2.0 / (double)K1);
+        s_kc[4] = 1.0 / (1.0 - 1.0 / (double)K2); s_kc[5] = 1.0 / (1.0 - 2.0 / (double)K2);
+        s_kc[6] = rec.chi0; s_kc[7] = rec.chi0 > 0.0 ? 1.0 / rec.chi0 : 0.0;
+    }
+    K.kc = s_kc;
+    K.bexp = 10.0 - p.alpha;
+    K.bass = (p.alpha > 0.0 && p.alpha <= 10.0) ? (K.bexp == 1.0 ? 1 : 2) : 0;
+    EvalConst KW;      // what pick_span_w reads
+    KW.bass = K.bass; KW.bexp = K.bexp;
+
+    const ScanMask mk = make_scan_mask(lane);
+    const uint32_t tmem = s_tmem + ((uint32_t)(warp & 3) << 21) + (uint32_t)(warp >> 2) * Cfg::TCOLS_WARP;
+    // tensor-memory columns (32-bit words) of this warp
+    constexpr uint32_t T_A0 = 0, T_A1 = 2 * C, T_A2 = 4 * C, T_ISW = 6 * C, T_XB = 8 * C, T_G0 = 10 * C, T_Y = 12 * C;
+    constexpr uint32_t T_W0 = 14 * C, T_W1 = 16 * C, T_W2 = 18 * C;      // window indices (lo[C], hi[C]) per span
+    {
+        int w0[2 * C], w1[2 * C], w2[2 * C];
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            const int j = tid * C + s;
+            const int l0 = window_lo(j, ibw0, K0, n), l1 = window_lo(j, ibw1, K1, n), l2 = window_lo(j, ibw2, K2, n);
+            w0[s] = ((l0 % C) * ROW + l0 / C); w0[C + s] = (((l0 + K0) % C) * ROW + (l0 + K0) / C);
+            w1[s] = ((l1 % C) * ROW + l1 / C); w1[C + s] = (((l1 + K1) % C) * ROW + (l1 + K1) / C);
+            w2[s] = ((l2 % C) * ROW + l2 / C); w2[C + s] = (((l2 + K2) % C) * ROW + (l2 + K2) / C);
+        }
+        tmem_park_words<2 * C>(tmem + T_W0, w0);
+        tmem_park_words<2 * C>(tmem + T_W1, w1);
+        tmem_park_words<2 * C>(tmem + T_W2, w2);
+        tmem_wait_st();
+    }
+    mbar_wait(&s_bar, 0);
+    __syncthreads();
+
+    const int64_t k0 = p.k_begin + (int64_t)ch * p.chunk;
+    const int64_t k1 = min(k0 + (int64_t)p.chunk, p.k_end);
+    double best = -INFINITY;
+    int64_t best_k = INT64_MAX;
+    double* prow = p.pgram ? p.pgram + (rec.obj - p.pgram_row0) * p.pgram_row_stride - p.pgram_k0 : nullptr;
+    double stash = 0.0;
+    int64_t kb = k0;
+
+    for (int64_t k = k0; k < k1; k++) {
+        const double f = freq_of(p.f_min, p.df, k);
+        bool bad = false;
+
+        // ---- P1 fold + 32-bit keys; P2 sort
+        unsigned key[C];
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            const int i = tid + NT * s;
+            unsigned kk = 0xffffffffu;
+            if (i < n)
+                kk = (__double2uint_rz(fold_phase(o_tt[i], f) * (double)(1u << (32 - Cfg::IDX_BITS))) << Cfg::IDX_BITS) | (unsigned)i;
+            key[s] = kk;
+        }
+        group_sort<G, C>(key, tid, kbuf);
+
+        // ---- exact phases in the sorted order; order repair inside a quantisation bucket (keys that agree in all
+        // the phase bits kept sit in index order): one adjacent swap settles a bucket of two
+        double phi[C];
+        int idx[C];
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            idx[s] = (int)(key[s] & Cfg::IDX_MASK);
+            phi[s] = (tid * C + s < n) ? fold_phase(o_tt[idx[s]], f) : 4.0 + (double)s;
+        }
+#pragma unroll
+        for (int s = 0; s + 1 < C; s++) {
+            if (phi[s + 1] < phi[s]) {
+                const double tp = phi[s]; phi[s] = phi[s + 1]; phi[s + 1] = tp;
+                const int ti = idx[s]; idx[s] = idx[s + 1]; idx[s + 1] = ti;
+            }
+        }
+        if (lane == 0) { s_edge[0][warp][0] = phi[0]; s_edge[0][warp][1] = (double)idx[0]; }
+        if (lane == 31) { s_edge[1][warp][0] = phi[C - 1]; s_edge[1][warp][1] = (double)idx[C - 1]; }
+        __syncthreads();                                                                    // BAR 1
+        {
+            double nphi = shfl_down_d(phi[0], 1), pphi = shfl_up_d(phi[C - 1], 1);
+            int nidx = __shfl_down_sync(0xffffffffu, idx[0], 1), pidx = __shfl_up_sync(0xffffffffu, idx[C - 1], 1);
+            if (lane == 31) {
+                if (warp + 1 < G) { nphi = s_edge[0][warp + 1][0]; nidx = (int)s_edge[0][warp + 1][1]; }
+                else nphi = 1.0e3;
+            }
+            if (lane == 0) {
+                if (warp > 0) { pphi = s_edge[1][warp - 1][0]; pidx = (int)s_edge[1][warp - 1][1]; }
+                else pphi = -1.0;
+            }
+            // both sides of a boundary see the same two phases and take the same decision
+            const bool swap_next = nphi < phi[C - 1], swap_prev = phi[0] < pphi;
+            if (tid * C + C - 1 < n && nphi == phi[C - 1]) bad = true;                     // exact tie (R24): generic path
+            if (swap_next) { phi[C - 1] = nphi; idx[C - 1] = nidx; }
+            if (swap_prev) { phi[0] = pphi; idx[0] = pidx; }
+        }
+#pragma unroll
+        for (int s = 0; s + 1 < C; s++)
+            if (tid * C + s + 1 < n && phi[s + 1] <= phi[s]) bad = true;                   // tie, or a bucket of three
+
+        // ---- gather; x centred by 0.5, padded slots carry x = 0, y = 0, w = W_PAD
+        double x[C], y[C], w[C];
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            if (tid * C + s < n) { x[s] = phi[s] - 0.5; y[s] = o_y[idx[s]]; w[s] = o_w[idx[s]]; }
+            else { x[s] = 0.0; y[s] = 0.0; w[s] = W_PAD; }
+        }
+        // quartile phases for vsmlsq
+        if (tid == K.q1t) {
+#pragma unroll
+            for (int s = 0; s < C; s++) if (s == K.q1s) s_q[0] = phi[s];
+        }
+        if (tid == K.q3t) {
+#pragma unroll
+            for (int s = 0; s < C; s++) if (s == K.q3s) s_q[1] = phi[s];
+        }
+
+        // ---- prefix sums of the weighted moments
+        double ma[C], mb[C], mc[C], md[C], me[C];
+#pragma unroll
+        for (int s = 0; s < C; s++) {
+            ma[s] = w[s]; mb[s] = w[s] * x[s]; mc[s] = mb[s] * x[s]; md[s] = w[s] * y[s]; me[s] = mb[s] * y[s];
+        }
+        const PairScan ps0 = pair_scan_begin<C>(ma, mb, s_tot[0], warp, lane, mk);
+        const PairScan ps1 = pair_scan_begin<C>(mc, md, s_tot[1], warp, lane, mk);
+        PairScan ps2; OneScan os2;
+        double mf[C];
+        if (GV) {
+#pragma unroll
+            for (int s = 0; s < C; s++) mf[s] = md[s] * y[s];
+            ps2 = pair_scan_begin<C>(me, mf, s_tot[2], warp, lane, mk);
+        } else {
+            os2 = one_scan_begin<C>(me, reinterpret_cast<double*>(s_tot[2]), warp, lane, mk);
+        }
+        bad = __syncthreads_or(bad);                                                        // BAR 2 (also: sort buffers dead)
+        if (bad) {
+            if (tid == 0) {
+                const unsigned pos = atomicAdd(p.defer_count, 1u);
+                if (pos < p.defer_capacity)
+                    p.defer_entries[pos] = ((unsigned long long)ri << 32) | (unsigned long long)(k - p.k_begin);
+                else
+                    p.defer_count[1] = 1u;
+            }
+        }
+        double P = 0.0;
+        if (!bad) {
+            pair_scan_finish<G, C>(ps0, ma, mb, s_tot[0], E01, warp, tid);
+            pair_scan_finish<G, C>(ps1, mc, md, s_tot[1], E23, warp, tid);
+            if (GV) pair_scan_finish<G, C>(ps2, me, mf, s_tot[2], E45, warp, tid);
+            else one_scan_finish<G, C>(os2, me, reinterpret_cast<const double*>(s_tot[2]), reinterpret_cast<double*>(E45), warp, tid);
+            const double scale = s_q[1] - s_q[0];
+            const double vsmlsq = 1.e-6 * scale * scale;
+            __syncthreads();                                                                // BAR 3
+            double chi2 = 0.0;
+            if (GV) {
+                // ---- O6: three windows, scores, pick, interpolate
+                double A[3][C], Gs[3][C];
+#pragma unroll
+                for (int i = 0; i < 3; i++) {
+                    int wi[2 * C];
+                    tmem_fetch_words<2 * C>(tmem + T_W0 + 2 * C * i, wi);
+#pragma unroll
+                    for (int s = 0; s < C; s++) {
+                        const int a_ = wi[s], b_ = wi[C + s];
+                        const double2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_], l2 = E45[a_], h2 = E45[b_];
+                        const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                        const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                        const double isw = rcp64(Sw), xb = Swx * isw;
+                        const double sxx = Swxx - xb * Swx;
+                        const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+                        const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
+                        A[i][s] = yb + b * (x[s] - xb);
+                        const double rss = (Syy - yb * Sy) - b * sxy;
+                        Gs[i][s] = sqrt64(rss * isw) * (isxx != 0.0 ? K.kc[2 * i + 1] : K.kc[2 * i]);
+                    }
+                }
+#pragma unroll
+                for (int s = 0; s < C; s++) {
+                    const double sp = pick_span_w(Gs[0][s], Gs[1][s], Gs[2][s], KW);
+                    const double smo = interp_spans(sp, A[0][s], A[1][s], A[2][s]);
+                    const double r = y[s] - smo;
+                    chi2 += w[s] * r * r;
+                }
+            } else {
+                // ---- CV pass 1: one span at a time; smooths parked in tensor memory
+                double r0[C], r1[C], r2[C];
+                double m_isw[C], m_xb[C], m_g[C];
+                const double* E4 = reinterpret_cast<const double*>(E45);
+                int amin = 0x7fffffff;
+#pragma unroll
+                for (int i = 0; i < 3; i++) {
+                    int wi[2 * C];
+                    tmem_fetch_words<2 * C>(tmem + T_W0 + 2 * C * i, wi);
+                    double Ai[C], q_isw[C], q_xb[C], q_g[C];
+#pragma unroll
+                    for (int s = 0; s < C; s++) {
+                        const int a_ = wi[s], b_ = wi[C + s];
+                        const double2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_];
+                        const double lxy = E4[a_], hxy = E4[b_];
+                        const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                        const double Sxy = hxy - lxy;
+                        const double isw = rcp64(Sw), xb = Swx * isw;
+                        const double sxx = Swxx - xb * Swx;
+                        const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
+                        const double dx = x[s] - xb, g = isxx * dx;
+                        q_isw[s] = isw; q_xb[s] = xb; q_g[s] = g;
+                        Ai[s] = Sy * isw + (Sxy - xb * Sy) * g;
+                        const double a = 1.0 - w[s] * (isw + dx * g);
+                        const double r = fabs(y[s] - Ai[s]) * rcp64(a);
+                        if (i == 0) r0[s] = r; else if (i == 1) r1[s] = r; else r2[s] = r;
+                        amin = min(amin, __double2hiint(a));
+                    }
+                    tmem_park<C>(tmem + T_A0 + 2 * C * i, Ai);
+                    if (i == 0) { tmem_park<C>(tmem + T_ISW, q_isw); tmem_park<C>(tmem + T_XB, q_xb); tmem_park<C>(tmem + T_G0, q_g); }
+                    if (i == 1) {
+#pragma unroll
+                        for (int s = 0; s < C; s++) { m_isw[s] = q_isw[s]; m_xb[s] = q_xb[s]; m_g[s] = q_g[s]; }
+                    }
+                }
+                tmem_park<C>(tmem + T_Y, y);
+                // ---- pass 2: the three residuals smoothed at the midrange span
+                double za[C], zb[C], zc[C], zd[C], ze[C], zf[C];
+#pragma unroll
+                for (int s = 0; s < C; s++) {
+                    za[s] = w[s] * r0[s]; zb[s] = za[s] * x[s];
+                    zc[s] = w[s] * r1[s]; zd[s] = zc[s] * x[s];
+                    ze[s] = w[s] * r2[s]; zf[s] = ze[s] * x[s];
+                }
+                const PairScan qs0 = pair_scan_begin<C>(za, zb, s_tot[0], warp, lane, mk);
+                const PairScan qs1 = pair_scan_begin<C>(zc, zd, s_tot[1], warp, lane, mk);
+                const PairScan qs2 = pair_scan_begin<C>(ze, zf, s_tot[2], warp, lane, mk);
+                // a <= 0 (or below the smallest normal): the residual carries (R23) -> generic path
+                const bool carry = __syncthreads_or(amin < 0x00100000);                    // BAR 4 (primary arrays dead)
+                if (carry) {
+                    if (tid == 0) {
+                        const unsigned pos = atomicAdd(p.defer_count, 1u);
+                        if (pos < p.defer_capacity)
+                            p.defer_entries[pos] = ((unsigned long long)ri << 32) | (unsigned long long)(k - p.k_begin);
+                        else
+                            p.defer_count[1] = 1u;
+                    }
+                    bad = true;
+                } else {
+                    pair_scan_finish<G, C>(qs0, za, zb, s_tot[0], E01, warp, tid);
+                    pair_scan_finish<G, C>(qs1, zc, zd, s_tot[1], E23, warp, tid);
+                    pair_scan_finish<G, C>(qs2, ze, zf, s_tot[2], E45, warp, tid);
+                    __syncthreads();                                                        // BAR 5
+                    int w1i[2 * C];
+                    tmem_fetch_words<2 * C>(tmem + T_W1, w1i);
+                    auto mid_load = [&](const double2* Ez, double (&out)[C]) {
+#pragma unroll
+                        for (int s = 0; s < C; s++) {
+                            const double2 l = Ez[w1i[s]], h = Ez[w1i[C + s]];
+                            const double Sz = h.x - l.x, Sxz = h.y - l.y;
+                            out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
+                        }
+                    };
+                    double sp[C];
+                    {
+                        double R0[C], R1[C], R2[C];
+                        mid_load(E01, R0); mid_load(E23, R1); mid_load(E45, R2);
+#pragma unroll
+                        for (int s = 0; s < C; s++) sp[s] = pick_span_w(R0[s], R1[s], R2[s], KW);
+                    }
+                    // ---- the spans smoothed at midrange
+#pragma unroll
+                    for (int s = 0; s < C; s++) { za[s] = w[s] * sp[s]; zb[s] = za[s] * x[s]; }
+                    const PairScan ss0 = pair_scan_begin<C>(za, zb, s_tot[0], warp, lane, mk);
+                    __syncthreads();                                                        // BAR 6 (residual arrays dead)
+                    pair_scan_finish<G, C>(ss0, za, zb, s_tot[0], E01, warp, tid);
+                    __syncthreads();                                                        // BAR 7
+                    double B[C];
+                    mid_load(E01, B);
+                    tmem_wait_st();
+                    {
+                        double a0[C], a1[C], a2[C];
+                        tmem_fetch<C>(tmem + T_A0, a0); tmem_fetch<C>(tmem + T_A1, a1); tmem_fetch<C>(tmem + T_A2, a2);
+#pragma unroll
+                        for (int s = 0; s < C; s++) B[s] = interp_spans(B[s], a0[s], a1[s], a2[s]);
+                    }
+                    // ---- final tweeter smooth
+#pragma unroll
+                    for (int s = 0; s < C; s++) { zc[s] = w[s] * B[s]; zd[s] = zc[s] * x[s]; }
+                    const PairScan fs0 = pair_scan_begin<C>(zc, zd, s_tot[1], warp, lane, mk);
+                    __syncthreads();                                                        // BAR 8
+                    pair_scan_finish<G, C>(fs0, zc, zd, s_tot[1], E23, warp, tid);
+                    __syncthreads();                                                        // BAR 9
+                    int w0i[2 * C];
+                    tmem_fetch_words<2 * C>(tmem + T_W0, w0i);
+                    double t_isw[C], t_xb[C], t_g[C], yy[C];
+                    tmem_fetch<C>(tmem + T_ISW, t_isw); tmem_fetch<C>(tmem + T_XB, t_xb); tmem_fetch<C>(tmem + T_G0, t_g);
+                    tmem_fetch<C>(tmem + T_Y, yy);
+#pragma unroll
+                    for (int s = 0; s < C; s++) {
+                        const double2 l = E23[w0i[s]], h = E23[w0i[C + s]];
+                        const double Sz = h.x - l.x, Sxz = h.y - l.y;
+                        const double smo = Sz * t_isw[s] + (Sxz - t_xb[s] * Sz) * t_g[s];
+                        const double r = yy[s] - smo;
+                        chi2 += w[s] * r * r;
+                    }
+                }
+            }
+            if (!bad) {
+#pragma unroll
+                for (int d = 16; d > 0; d >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, d);
+                if (lane == 0) s_red[warp] = chi2;
+                __syncthreads();                                                            // BAR 10
+                double c2 = 0.0;
+#pragma unroll
+                for (int q = 0; q < G; q++) c2 += s_red[q];
+                P = (K.kc[6] - c2) * K.kc[7];
+            }
+        }
+        if (!bad && P > best) { best = P; best_k = k; }
+        if (tid == (int)(k - kb)) stash = bad ? 0.0 : P;      // a handed-over eval is patched by the generic kernel
+        if (k - kb == 31 || k == k1 - 1) {
+            if (prow && tid < 32 && kb + tid <= k) prow[kb + tid] = stash;
+            kb = k + 1;
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (warp == 0) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s_tmem), "n"(Cfg::TCOLS) : "memory");
+    }
+    if (tid == 0) {
+        const int64_t slot = (int64_t)ri * p.chunks_total + p.chunk_base + ch;
+        p.part_val[slot] = best;
+        p.part_idx[slot] = best_k == INT64_MAX ? k0 : best_k;
+    }
+}
+
+template <int G, int C, bool GV>
+inline ss_status_t launch_group_variant(const EvalParams& p, int64_t n_items, cudaStream_t stream)
+{
+    const size_t smem = group_smem_bytes<G, C, GV>();
+    if (cudaFuncSetAttribute(group_kernel<G, C, GV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return SS_ERR_CUDA;
+    group_kernel<G, C, GV><<<(unsigned)n_items, GroupCfg<G, C>::NT, smem, stream>>>(p);
+    return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
+}
+
+}  // namespace ss

@@ -12,6 +12,9 @@ namespace ss {
 // warp-per-eval kernels (ss_warp_kernel.cuh); variant = warp_variant_for_n(n)
 ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 
+// G-warps-per-eval kernels (ss_group_kernel.cuh); variant = group_variant_for_n(n)
+ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
+
 // CTA-per-eval kernels (ss_block_kernel.cuh): path = SS_PATH_BLOCK (threads = 128 / 256 / 512, per-eval arrays in
 // shared memory sized for max_n) or SS_PATH_STAGE (512 threads, arrays in p.stage); opt = listing options compiled in
 ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int max_n, bool opt, int64_t n_items,
@@ -19,7 +22,7 @@ ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int 
 
 // evals / whole work items the warp path handed over (p.defer_entries): recompute with the generic code, patch the
 // periodogram and the item's partial-argmax slot (item entries) or fold into best_val / best_idx (eval entries)
-ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int sm_count,
+ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, int sm_count,
                                  cudaStream_t stream);
 ss_status_t launch_deferred_merge(const EvalParams& p, const double* dval, const unsigned long long* dmax,
                                   unsigned long long* dmin, double* best_val, int64_t* best_idx, int sm_count,

@@ -14,11 +14,24 @@ constexpr int64_t BLOCK_SMEM_MAX = 232448 - 2048;   // dynamic part; 2 KB left f
 constexpr int64_t BLOCK_BYTES_PER_POINT = 14 * 8;
 constexpr int64_t BLOCK_MAX_N = BLOCK_SMEM_MAX / BLOCK_BYTES_PER_POINT - 2;   // 2055
 
+static_assert(SS_GROUP_MAX_N <= BLOCK_MAX_N, "what the group path hands over must fit the generic shared-memory kernel");
+
 inline int path_for_n(int64_t n, int /*mode*/)
 {
     if (n <= SS_WARP_MAX_N) return SS_PATH_WARP;
-    if (n <= BLOCK_MAX_N) return SS_PATH_BLOCK;
+    if (n <= SS_GROUP_MAX_N) return SS_PATH_GROUP;
     return SS_PATH_STAGE;
+}
+
+// Group-path kernel variant of an object: G warps x C points per thread, the smallest capacity 32*G*C >= n
+// (384, 512, 640, 768, 1024, 1280, 1536, 2048, 2560).  id = G*8 + C.
+inline int group_variant_for_n(int n)
+{
+    const int gs[3] = {4, 8, 16};
+    for (int gi = 0; gi < 3; gi++)
+        for (int c = 3; c <= 5; c++)
+            if (32 * gs[gi] * c >= n) return gs[gi] * 8 + c;
+    return 16 * 8 + 5;
 }
 
 // Window half-width of Friedman's smoother (O4/R21): max(2, floor(0.5*span*n + 0.5)),
@@ -101,7 +114,7 @@ inline ss_status_t make_plan(const PlanInput& in, ss_plan_t* out)
     // tt, yc, w (+ the raw catalog copy when the caller's arrays live on the host), records, lists,
     // running best (value, index), offsets, scheduler counters
     p.fixed_bytes = (size_t)((in.host_tiles ? 6 : 3) * 8 * in.n_points_total)
-                  + (size_t)(nobj * (64 + 4 + 8 + 8 + 8 + 16)) + 8192
+                  + (size_t)(nobj * (64 + 4 + 8 + 8 + 8 + 16 + 24 + 8)) + 8192   // + even-length padding of tt/yc/w, raw offsets
                   + (size_t)DEFER_CAPACITY * 16;   // warp-path hand-over list (entries + values)
     if (in.max_n > BLOCK_MAX_N)
         p.stage_bytes = (size_t)STAGE_CTAS * (size_t)(14 * 8 * (((in.max_n + 2) + 1) & ~(int64_t)1));

@@ -18,11 +18,11 @@ import sys
 
 import numpy as np
 
-from . import (CROSS_VALIDATION, GENERALIZED_VALIDATION, PATH_BLOCK, PATH_STAGE, PATH_WARP, default_options, load,
+from . import (CROSS_VALIDATION, GENERALIZED_VALIDATION, PATH_BLOCK, PATH_GROUP, PATH_STAGE, PATH_WARP, default_options, load,
                path_for_n, ss_periodogram)
 
 DEFAULT_NS = [50, 64, 96, 128, 160, 200, 256, 257, 320, 400, 512, 700, 1000, 1400, 2055, 2056, 3000, 5000, 10000, 20000]
-PATH_NAME = {PATH_WARP: "warp", PATH_BLOCK: "cta-smem", PATH_STAGE: "cta-staged"}
+PATH_NAME = {PATH_WARP: "warp", PATH_GROUP: "group", PATH_BLOCK: "cta-smem", PATH_STAGE: "cta-staged"}
 WARP_MAX_N, BLOCK_MAX_N = 256, 2055
 
 
@@ -72,8 +72,8 @@ def main(argv=None):
     lines = ["| n | path | auto | objects x frequencies | CV point-evals/s | CV evals/s | GV point-evals/s | GV evals/s |",
              "|---|---|---|---|---|---|---|---|"]
     for n in [int(v) for v in args.ns.split(",")]:
-        paths = [p for p in (PATH_WARP, PATH_BLOCK, PATH_STAGE)
-                 if (p != PATH_WARP or n <= WARP_MAX_N) and (p != PATH_BLOCK or n <= BLOCK_MAX_N)]
+        paths = [p for p in (PATH_WARP, PATH_GROUP, PATH_BLOCK, PATH_STAGE)
+                 if (p != PATH_WARP or n <= WARP_MAX_N) and (p not in (PATH_BLOCK, PATH_GROUP) or n <= BLOCK_MAX_N)]
         auto = path_for_n(n)
         for path in paths:
             # size the call: enough (object, frequency) items to fill 148 SMs several times over

@@ -181,7 +181,7 @@ def test_forced_paths_agree(ss, mode):
     cat = ss_inputs.config3(n_objects=12, n_freq=257)
     ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
                                    cat.n_freq, mode=mode, variant=oracle.DEFINITION)
-    for path in (ss.PATH_WARP, ss.PATH_BLOCK, ss.PATH_STAGE):
+    for path in (ss.PATH_WARP, ss.PATH_GROUP, ss.PATH_BLOCK, ss.PATH_STAGE):
         res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
                              mode, force_path=path)
         check_parity(cat, res.pgram, ref, mode, label=f"path{path}")
@@ -232,7 +232,7 @@ def test_equal_phases_and_tied_runs(ss, mode):
                             np.concatenate([rng.uniform(0.05, 0.2, size=n), np.full(60, 0.05)]), off,
                             0.25, 1.25, 4, np.array([np.nan, 1 / 1.3]))      # f = 0.25, 0.5, 0.75, 1.0
     assert oracle.freq(cat.f_min, cat.f_max, cat.n_freq, 3) == 1.0
-    for path in (ss.PATH_AUTO, ss.PATH_BLOCK, ss.PATH_STAGE):
+    for path in (ss.PATH_AUTO, ss.PATH_GROUP, ss.PATH_BLOCK, ss.PATH_STAGE):
         res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
                              mode, force_path=path)
         ref, bf, bi = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max,
@@ -251,7 +251,7 @@ def test_phase_clusters_below_the_sort_key_resolution(ss, mode):
     coincident abscissae the fits themselves are ill-conditioned -- a 7-point window holding 6 of them leaves
     the seventh a leave-one-out denominator of 0 up to rounding -- so (b) pins the ORDER, not the values.)"""
     rng = np.random.default_rng(77)
-    for n, path_list in ((700, (ss.PATH_AUTO, ss.PATH_STAGE)), (120, (ss.PATH_AUTO, ss.PATH_BLOCK))):
+    for n, path_list in ((700, (ss.PATH_AUTO, ss.PATH_BLOCK, ss.PATH_STAGE)), (120, (ss.PATH_AUTO, ss.PATH_GROUP, ss.PATH_BLOCK))):
         t = np.sort(rng.uniform(0, 40, size=n))
         t[10:13] = t[10] + np.array([2e-9, 1e-9, 0.0])                # triple, reversed
         t[30:32] = t[30] + np.array([1e-9, 0.0])                      # pair, reversed
@@ -675,3 +675,38 @@ def test_config4_full_size_sampled(ss, mode):
                bf[torch.as_tensor(rows, device=dev)].cpu().numpy(), sub)
     del pg
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_group_kernel_every_variant(ss, mode):
+    """The G-warps-per-eval kernels, one object per (G, C) variant at both ends of its range of n (capacities 384,
+    512, 640, 768, 1,024, 1,280, 1,536, 2,048, 2,560 points; the path ends at n = 2,055), heteroscedastic errors,
+    config-4 time sampling; against the definition oracle, best index included."""
+    rng = np.random.default_rng(515)
+    ns = [257, 384, 385, 512, 513, 640, 641, 768, 769, 1024, 1025, 1280, 1281, 1536, 1537, 2048, 2049, 2055]
+    T, Y, E = [], [], []
+    for i, n in enumerate(ns):
+        assert ss.path_for_n(n) == ss.PATH_GROUP
+        kept = np.nonzero(np.mod(np.arange(1827), 365.25) < 243.5)[0]
+        t = np.sort(rng.choice(kept, size=n, replace=True) + rng.uniform(0.0, 0.3, size=n))
+        P = np.exp(rng.uniform(np.log(0.1), np.log(2.0)))
+        e = rng.uniform(0.01, 0.2, size=n)
+        y = 15 + rng.uniform(0.1, 1.0) * np.sin(2 * np.pi * t / P + i) + rng.normal(0, 1.0, size=n) * e
+        T.append(t); Y.append(y); E.append(e)
+    off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
+    cat = ss_inputs.Catalog("group", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
+                            0.01, 10.0, 67, np.full(len(ns), np.nan))
+    res, ref = run_both(ss, cat, mode, oracle.DEFINITION)
+    check_parity(cat, res.pgram, ref, mode, label="group variants")
+    check_best(ref, res.best_index, res.best_freq, cat)
+    # small objects forced onto the group path (n below one warp's worth, n = 5)
+    small = ss_inputs.config3(n_objects=6, n_freq=65)
+    tiny_t = np.array([0.1, 0.9, 1.7, 3.2, 4.4]); tiny_y = 15 + np.array([0.1, -0.2, 0.3, 0.0, -0.1])
+    times = np.concatenate([small.times, tiny_t]); mags = np.concatenate([small.mags, tiny_y])
+    errs = np.concatenate([small.errs, np.full(5, 0.05)])
+    offs = np.concatenate([small.offsets, [small.offsets[-1] + 5]])
+    cat2 = ss_inputs.Catalog("group-small", times, mags, errs, offs, 0.5, 24.0, 65, np.full(7, np.nan))
+    ref2, _, _ = oracle.periodogram(times, mags, errs, offs, 0.5, 24.0, 65, mode=mode, variant=oracle.DEFINITION)
+    res2 = ss.periodogram(times, mags, errs, offs, 0.5, 24.0, 65, mode, force_path=ss.PATH_GROUP)
+    check_parity(cat2, res2.pgram, ref2, mode, label="group small")
+    check_best(ref2, res2.best_index, res2.best_freq, cat2)

@@ -54,8 +54,10 @@ def test_paper_batch_count_eq1():
 def test_path_classes():
     assert ss.path_for_n(5) == ss.PATH_WARP
     assert ss.path_for_n(256) == ss.PATH_WARP
-    assert ss.path_for_n(257) == ss.PATH_BLOCK
-    assert ss.path_for_n(2000) == ss.PATH_BLOCK
+    assert ss.path_for_n(257) == ss.PATH_GROUP
+    assert ss.path_for_n(2000) == ss.PATH_GROUP
+    assert ss.path_for_n(2055) == ss.PATH_GROUP
+    assert ss.path_for_n(2056) == ss.PATH_STAGE
     assert ss.path_for_n(20000) == ss.PATH_STAGE
 
 
