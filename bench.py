@@ -29,20 +29,19 @@ import ss_inputs  # noqa: E402
 METRIC = "object_frequency_evals_per_second"
 UNIT = "evals/s"
 
-# Algorithmic work per point-eval: fp64 pipe lane-instructions
-# ("slots") the method itself needs in the windowed-moment formulation -- 133 add/mul/fma + 10 div/sqrt
-# at 8 slots each (CV), 85 + 10 (GV) -- reported as FMA-equivalent FLOP (2 per slot) against a peak that
-# counts an FMA as 2.
-SLOTS_PER_POINT_EVAL = {"cv": 213.0, "gv": 165.0}
-FLOP_PER_POINT_EVAL = {m: 2.0 * s for m, s in SLOTS_PER_POINT_EVAL.items()}
-# Algorithmic on-chip traffic per point-eval: scan arrays written once + window-end
-# reads, 8 B each: 15 + 50 (CV), 6 + 30 (GV) -- the second, co-limiting roofline (shared-memory pipe).
+# Algorithmic on-chip traffic per point-eval: prefix arrays written once + window-end
+# reads, 8 B each: 15 + 50 words (CV), 6 + 30 (GV).  The shared-memory / LSU data pipe is the unit that binds the
+# eval kernels (ncu: l1tex__data_pipe_lsu_wavefronts 77-83 % of peak, fp64 pipe 37-44 %), so this is `roofline`.
 SMEM_BYTES_PER_POINT_EVAL = {"cv": 520.0, "gv": 288.0}
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE full-size launch of the heaviest CV kernel, from the
-# ncu --set full capture summarised in profiles/r1e_ncu_warp_kernel_cv.md (39.19 MB + 743.67 MB)
-NCU_TRAFFIC_BYTES = 782.86e6
-NCU_TRAFFIC_NOTE = ("bytes of one launch of warp_kernel<4,3,CV> (1,859 objects x 50,000 frequencies, 328 ms under ncu; "
-                    "profiles/r1e_ncu_warp_kernel_cv.md); algorithmic bytes of that launch: 743.6 MB of periodogram rows")
+# Secondary: fp64 pipe lane-instructions ("slots") per point-eval.  SURVEY.md 8(d) counts 133 add/mul/fma + 10 div/sqrt at
+# 8 slots each (CV), 85 + 10 (GV); the kernels pay less for a division (MUFU seed + 3 DFMA + the multiply = 4 slots) and
+# a square root (MUFU seed + 6 DFMA = 7 slots), reported beside it as "as implemented".
+SLOTS_PER_POINT_EVAL = {"cv": 213.0, "gv": 165.0}
+SLOTS_AS_IMPLEMENTED = {"cv": 133.0 + 10 * 4.0, "gv": 85.0 + 7 * 4.0 + 3 * 7.0}
+FLOP_PER_POINT_EVAL = {m: 2.0 * s for m, s in SLOTS_PER_POINT_EVAL.items()}
+# HBM traffic of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full):
+# read from the committed summary of the capture taken at the commit it names, never a literal here.
+TRAFFIC_JSON = os.path.join(ROOT, "profiles", "r2_traffic.json")
 FP64_LANES_PER_SM = 64          # B200 fp64 pipe: 64 FMA lanes per SM per clock
 N_SM = 148
 
@@ -55,13 +54,9 @@ def parse():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--mode", default="cv", choices=["cv", "gv"])
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5],
-                    help="(sweep) another BASELINE.json config; the bench line proper is config 3")
+                    help="another BASELINE.json config (profiles/r2_bench_configs.md); the bench line proper is config 3")
     ap.add_argument("--objects", type=int, default=None, help="(debug) fewer objects than the config has (configs 3, 4)")
     ap.add_argument("--freqs", type=int, default=None, help="(debug) fewer frequencies than the config has")
-    ap.add_argument("--iper", type=int, default=1, help="(sweep) 2 = periodic windows, PAPER.md:199-200")
-    ap.add_argument("--span", type=float, default=0.0, help="(sweep) > 0 = fixed span, PAPER.md:202-210")
-    ap.add_argument("--path", type=int, default=0, help="(sweep) force a path class: 1 warp, 2 CTA, 3 staging")
-    ap.add_argument("--no-clocks", action="store_true", help="(debug) do not sample nvidia-smi during the run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -254,11 +249,11 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     def step(m=mode, profile=False):
-        o = ss.default_options(profile=1 if profile else 0, iper=args.iper, span=args.span, force_path=args.path)
+        o = ss.default_options(profile=1 if profile else 0)
         ss.ss_periodogram(t, y, e, off, n_obj, cat.f_min, cat.f_max, n_freq, m, pg, bf, bi, o)
 
     sampler = ClockSampler(local)
-    if rank == 0 and not args.no_clocks:
+    if rank == 0:
         sampler.start()
     for _ in range(args.warmup):
         step()
@@ -304,7 +299,7 @@ def run_ours(args):
         hbi = torch.empty(n_obj, dtype=torch.int64).pin_memory()
         def estep():
             ss.ss_periodogram_host(ht, hy, he, hoff, n_obj, cat.f_min, cat.f_max, n_freq, mode, hpg, hbf, hbi,
-                                   ss.default_options(iper=args.iper, span=args.span, force_path=args.path))
+                                   ss.default_options())
         estep()
         barrier()
         t0 = time.perf_counter()
@@ -328,21 +323,29 @@ def run_ours(args):
     peak_tflops = N_SM * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     k_ms = kernel_ms / max(1, kernel_launches)
     k_units = point_evals_per_step * args.steps / max(1, kernel_launches)   # point-evals per launch
-    achieved = FLOP_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "kernel": "eval kernel (fold+sort+smoother+statistic fused)",
-                "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                "traffic": NCU_TRAFFIC_BYTES if (args.config, n_obj, n_freq, args.mode) == (3, 10000, 50000, "cv") else None,
-                "traffic_note": NCU_TRAFFIC_NOTE, "peak_source": f"derived: {N_SM} SM x {FP64_LANES_PER_SM} fp64 FMA lanes x 2 x "
-                f"{sm_max:.0f} MHz ({pk_src} clock); DFMA microbenchmark on this box: {fp64_meas / 1e12:.2f} TFLOP/s, "
-                f"shared memory {smem_meas / 1e12:.2f} TB/s",
-                "flop_per_point_eval": FLOP_PER_POINT_EVAL[args.mode],
+    smem_achieved = SMEM_BYTES_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3)
+    fp64_achieved = FLOP_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / 1e12
+    traffic, traffic_note = None, "no capture for this workload"
+    if os.path.exists(TRAFFIC_JSON):
+        with open(TRAFFIC_JSON) as f:
+            tj = json.load(f)
+        traffic_note = tj.get("note", "")
+        if (args.config, n_obj, n_freq, args.mode) == (tj.get("config"), tj.get("n_objects"), tj.get("n_freq"), tj.get("mode")):
+            traffic = float(tj["dram_bytes_read"]) + float(tj["dram_bytes_write"])
+    roofline = {"bound": "smem", "kernel": "eval kernel (fold+sort+smoother+statistic fused)",
+                "achieved": smem_achieved / 1e12, "peak": smem_meas / 1e12, "unit": "TB/s", "frac": smem_achieved / smem_meas,
+                "traffic": traffic, "traffic_note": traffic_note,
+                "peak_source": "shared-memory read microbenchmark of this run (ss_microbench; 148 SM x 128 B/clk x "
+                               f"{sm_max:.0f} MHz = {N_SM * 128 * sm_max * 1e6 / 1e12:.2f} TB/s nominal)",
+                "bytes_per_point_eval": SMEM_BYTES_PER_POINT_EVAL[args.mode],
                 "point_evals_per_launch": k_units, "kernel_ms_per_launch": k_ms,
                 "kernel_share_of_step": kernel_ms / elapsed_ms,
-                "smem": {"achieved": SMEM_BYTES_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / 1e12,
-                         "peak": smem_meas / 1e12, "unit": "TB/s",
-                         "frac": SMEM_BYTES_PER_POINT_EVAL[args.mode] * k_units / (k_ms * 1e-3) / smem_meas,
-                         "note": "co-limiting roofline: algorithmic shared-memory bytes (SURVEY 8(d)) vs the "
-                                 "shared-memory read microbenchmark measured in this run"},
+                "fp64": {"achieved": fp64_achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": fp64_achieved / peak_tflops,
+                         "frac_as_implemented": fp64_achieved / peak_tflops * SLOTS_AS_IMPLEMENTED[args.mode] / SLOTS_PER_POINT_EVAL[args.mode],
+                         "flop_per_point_eval": FLOP_PER_POINT_EVAL[args.mode],
+                         "note": f"secondary roofline: SURVEY 8(d) slots per point-eval against {N_SM} SM x {FP64_LANES_PER_SM} fp64 "
+                                 f"FMA lanes x 2 x {sm_max:.0f} MHz ({pk_src} clock); DFMA microbenchmark of this run "
+                                 f"{fp64_meas / 1e12:.2f} TFLOP/s; as_implemented prices a division at 4 slots and a square root at 7"},
                 "hbm_gbs_algorithmic": 8.0 * evals_per_step / (ms_per_step * 1e-3) / 1e9}
     cpu = None
     if not args.no_cpu:
@@ -351,9 +354,7 @@ def run_ours(args):
            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": f"config{args.config}: {n_obj} objects ({cat.n_points} points) x {n_freq} "
-                      f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised"
-                      + (f", iper={args.iper}" if args.iper != 1 else "") + (f", span={args.span}" if args.span else "")
-                      + (f", forced path {args.path}" if args.path else ""),
+                      f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised",
                       "objects_per_second": world * n_obj * args.steps / (elapsed_ms * 1e-3),
                       "l2": (f"inputs ({24 * cat.n_points / 1e6:.0f} MB catalog) are re-read per frequency by design; the "
                              f"{8 * evals_per_step / 1e9:.2f} GB periodogram written every step "

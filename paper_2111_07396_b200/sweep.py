@@ -2,11 +2,12 @@
 kernel-cascade study).
 
 For each n a catalog of equal-length light curves is timed through the device entry point on every path
-class that can serve it (SS_PATH_WARP for n <= 256, SS_PATH_BLOCK for n <= 2,055, SS_PATH_STAGE for any
-n), in both modes; the table reports point-evals/s (n x frequencies x objects / second), which is flat
+class that can serve it (SS_PATH_WARP for n <= 256, SS_PATH_GROUP and SS_PATH_BLOCK for n <= 2,055,
+SS_PATH_STAGE for any n), in both modes; the table reports point-evals/s (n x frequencies x objects / second), which is flat
 where a path scales and drops where it stops fitting.  The path the library picks by itself is marked.
 
     python -m paper_2111_07396_b200.sweep [--ns 50,100,...] [--target-ms 150] [--md out.md]
+    python -m paper_2111_07396_b200.sweep --options [--md out.md]     # the listing's options vs the default call
 
 Needs a CUDA device (no CPU fallback).  Inputs are synthetic: times uniform over 30 nights (8 h per
 night), a sinusoid of random period plus Gaussian noise; the arithmetic under test is all in the library.
@@ -36,11 +37,11 @@ def catalog(n: int, n_objects: int, seed: int):
     return t.ravel(), y.ravel(), e.ravel(), off
 
 
-def time_call(torch, dev, arrs, n_objects, n_freq, mode, path, reps=3):
+def time_call(torch, dev, arrs, n_objects, n_freq, mode, path, reps=3, **opts):
     t, y, e, off = arrs
     pg = torch.empty((n_objects, n_freq), dtype=torch.float64, device=dev)
     bi = torch.empty(n_objects, dtype=torch.int64, device=dev)
-    opt = default_options(force_path=path, skip_validation=1)
+    opt = default_options(force_path=path, skip_validation=1, **opts)
 
     def call():
         ss_periodogram(t, y, e, off, n_objects, 0.5, 24.0, n_freq, mode, pg, None, bi, opt)
@@ -58,17 +59,55 @@ def time_call(torch, dev, arrs, n_objects, n_freq, mode, path, reps=3):
     return best
 
 
+def options_table(torch, dev, md):
+    """Listing 1's options, timed on config-3-shaped objects (n ~ U[50, 200]) through the device entry point."""
+    import ss_inputs
+    cat = ss_inputs.config3(n_objects=1000, n_freq=5000)
+    arrs = tuple(torch.as_tensor(a, device=dev) for a in (cat.times, cat.mags, cat.errs, cat.offsets))
+    lines = ["| options | CV evals/s | GV evals/s | CV vs default |", "|---|---|---|---|"]
+    base = None
+    for name, opts in (("default", {}), ("iper=2", dict(iper=2)), ("span=0.2", dict(span=0.2)),
+                       ("iper=2, span=0.2", dict(iper=2, span=0.2)), ("alpha=0", dict(alpha=0.0)), ("alpha=5", dict(alpha=5.0))):
+        row = []
+        for mode in (CROSS_VALIDATION, GENERALIZED_VALIDATION):
+            t, y, e, off = arrs
+            pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev)
+            opt = default_options(skip_validation=1, **opts)
+            best = float("inf")
+            for _ in range(4):
+                ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+                torch.cuda.synchronize()
+                ev[0].record()
+                ss_periodogram(t, y, e, off, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, None, None, opt)
+                ev[1].record()
+                torch.cuda.synchronize()
+                best = min(best, ev[0].elapsed_time(ev[1]))
+            row.append(cat.n_objects * cat.n_freq / (best * 1e-3))
+        base = base or row[0]
+        lines.append(f"| {name} | {row[0]:.4g} | {row[1]:.4g} | {base / row[0]:.2f}x slower |")
+        print(lines[-1], flush=True)
+    if md:
+        with open(md, "w") as f:
+            f.write("\n".join(lines) + "\n")
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--ns", default=",".join(map(str, DEFAULT_NS)))
     ap.add_argument("--target-ms", type=float, default=150.0, help="aim each timed call at about this long")
     ap.add_argument("--md", default=None, help="also write the table as markdown to this file")
+    ap.add_argument("--options", action="store_true",
+                    help="instead of the sweep over n: the listing's options (iper = 2, fixed span; PAPER.md:199-210) "
+                         "against the default call on 1,000 config-3-shaped objects x 5,000 frequencies")
     args = ap.parse_args(argv)
     import torch
     if not torch.cuda.is_available():
         raise SystemExit("sweep needs a CUDA device (the library has no CPU path)")
     load()
     dev = torch.device("cuda")
+    if args.options:
+        return options_table(torch, dev, args.md)
     lines = ["| n | path | auto | objects x frequencies | CV point-evals/s | CV evals/s | GV point-evals/s | GV evals/s |",
              "|---|---|---|---|---|---|---|---|"]
     for n in [int(v) for v in args.ns.split(",")]:
