@@ -57,12 +57,15 @@ typedef enum {
     SS_PATH_WARP = 1,  /* one warp per (object, frequency); n <= SS_WARP_MAX_N; registers + shuffles   */
     SS_PATH_BLOCK = 2, /* one CTA per (object, frequency); per-eval arrays in shared memory            */
     SS_PATH_STAGE = 3, /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
-    SS_PATH_GROUP = 4  /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_MAX_N;
+    SS_PATH_GROUP = 4, /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_MAX_N;
                           points in registers, prefix sums in shared memory, smooths in tensor memory     */
+    SS_PATH_CLUSTER = 5 /* a thread-block cluster of 2..16 CTAs per (object, frequency); SS_GROUP_MAX_N < n <=
+                          SS_CLUSTER_MAX_N; prefix sums in distributed shared memory                      */
 } ss_path_t;
 
 #define SS_WARP_MAX_N 256
 #define SS_GROUP_MAX_N 2055
+#define SS_CLUSTER_MAX_N 40960
 
 typedef struct {
     double alpha;           /* bass enhancement.  Default 9.0.                 */
@@ -161,7 +164,7 @@ size_t ss_workspace_bytes(int64_t n_points_total, int64_t max_n, int64_t n_objec
 double ss_paper_footprint_bytes(int64_t n_t, int64_t n_f);
 int64_t ss_paper_batches(int64_t n_t, int64_t n_f, ss_mode_t mode, double device_gib, double beta);
 
-/* Path class the library picks for an object of n points (SS_PATH_WARP / GROUP / STAGE; SS_PATH_BLOCK serves
+/* Path class the library picks for an object of n points (SS_PATH_WARP / GROUP / CLUSTER / STAGE; SS_PATH_BLOCK serves
  * the listing's options and whatever the other paths hand over). */
 int ss_path_for_n(int64_t n, ss_mode_t mode);
 

@@ -15,7 +15,7 @@ import numpy as np
 
 CROSS_VALIDATION = 0
 GENERALIZED_VALIDATION = 1
-PATH_AUTO, PATH_WARP, PATH_BLOCK, PATH_STAGE, PATH_GROUP = 0, 1, 2, 3, 4
+PATH_AUTO, PATH_WARP, PATH_BLOCK, PATH_STAGE, PATH_GROUP, PATH_CLUSTER = 0, 1, 2, 3, 4, 5
 SS_OK, SS_ERR_INVALID_ARG, SS_ERR_OUT_OF_MEMORY, SS_ERR_CUDA, SS_ERR_UNSUPPORTED = range(5)
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

@@ -39,6 +39,10 @@ def units():
             for gv in (0, 1):
                 for g in (4, 8, 16):
                     u.append((f"{base}_{gv}_{g}.o", src, [f"-DSS_TU_GV={gv}", f"-DSS_TU_G={g}"]))
+        elif base == "ss_cluster_tu":
+            for gv in (0, 1):
+                for c in (3, 4, 5):
+                    u.append((f"{base}_{gv}_{c}.o", src, [f"-DSS_TU_GV={gv}", f"-DSS_TU_C={c}"]))
         elif base == "ss_block_tu":
             for part in range(10):
                 u.append((f"{base}_{part}.o", src, [f"-DSS_TU_PART={part}"]))

@@ -487,11 +487,14 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             // periodic windows and the fixed span live in the generic CTA-per-eval code only
             if ((path == SS_PATH_WARP || path == SS_PATH_GROUP) && has_listing_options(o)) path = SS_PATH_BLOCK;
             if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_GROUP;
-            if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N) path = SS_PATH_STAGE;
+            if (path == SS_PATH_CLUSTER && has_listing_options(o)) path = SS_PATH_STAGE;
+            if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N) path = SS_PATH_CLUSTER;
+            if (path == SS_PATH_CLUSTER && (r.n > SS_CLUSTER_MAX_N || r.n < 2 * 512)) path = SS_PATH_STAGE;
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
             if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
             else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n);
+            else if (path == SS_PATH_CLUSTER) variant = cluster_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
             else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);
             ClassList& c = find(path, variant);
@@ -585,6 +588,9 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         int64_t cpo = std::min<int64_t>(cpo_cap, nk);
         int64_t chunk = (nk + cpo - 1) / cpo;
         if (c.path == SS_PATH_WARP) chunk = (chunk + WARPS_PER_CTA - 1) / WARPS_PER_CTA * WARPS_PER_CTA;
+        // a cluster sets up tensor memory and its window tables per work item: at least 64 evals each while that
+        // still leaves a few hundred items
+        if (c.path == SS_PATH_CLUSTER && chunk < 64 && nk * (int64_t)c.recs.size() >= 64 * 512) chunk = 64;
         cpo = (nk + chunk - 1) / chunk;
         p.chunk = (int32_t)chunk; p.chunks_per_obj = (int32_t)cpo;
         p.chunks_total = (int32_t)cpo_cap; p.chunk_base = 0;
@@ -602,7 +608,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             SS_CUDA(g_pool.event(true, &ev1));
             prof.emplace_back(ev0, ev1);
         }
-        const bool hands_over = c.path == SS_PATH_WARP || c.path == SS_PATH_GROUP;   // one CTA per item, hand-over list
+        const bool hands_over = c.path == SS_PATH_WARP || c.path == SS_PATH_GROUP || c.path == SS_PATH_CLUSTER;   // no work counter, hand-over list
         if (!hands_over) {
             SS_CUDA(cudaMemsetAsync(p.counter, 0, 4, stream));
             next_counter++;
@@ -611,6 +617,9 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         if (c.path == SS_PATH_WARP) {
             ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        } else if (c.path == SS_PATH_CLUSTER) {
+            ss_status_t st = launch_cluster_kernel(p, c.variant, n_items, stream);
+            if (st != SS_OK) return fail(st, "cluster kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (c.path == SS_PATH_GROUP) {
             ss_status_t st = launch_group_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "group kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));

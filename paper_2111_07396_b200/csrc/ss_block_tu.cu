@@ -86,6 +86,21 @@ ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_item
          : g == 8 ? launch_group_tu_0_8(p, c, n_items, stream) : launch_group_tu_0_16(p, c, n_items, stream);
 }
 
+// ---- cluster-kernel translation units (ss_cluster_tu.cu) -----------------------------------------------
+#define SS_DECL(gv, c) ss_status_t launch_cluster_tu_##gv##_##c(const EvalParams&, int, int64_t, cudaStream_t);
+SS_DECL(0, 3) SS_DECL(0, 4) SS_DECL(0, 5) SS_DECL(1, 3) SS_DECL(1, 4) SS_DECL(1, 5)
+#undef SS_DECL
+
+ss_status_t launch_cluster_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
+{
+    const int r = variant / 8, c = variant % 8;
+    if (p.mode == 1)
+        return c == 3 ? launch_cluster_tu_1_3(p, r, n_items, stream)
+             : c == 4 ? launch_cluster_tu_1_4(p, r, n_items, stream) : launch_cluster_tu_1_5(p, r, n_items, stream);
+    return c == 3 ? launch_cluster_tu_0_3(p, r, n_items, stream)
+         : c == 4 ? launch_cluster_tu_0_4(p, r, n_items, stream) : launch_cluster_tu_0_5(p, r, n_items, stream);
+}
+
 // ---- CTA-per-eval kernels ---------------------------------------------------------------------------
 ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int max_n, bool opt, int64_t n_items,
                                 int sm_count, cudaStream_t stream)
@@ -111,7 +126,6 @@ ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int 
 //                                                          a leave-one-out denominator <= 0)
 //   item  : 1 << 63 | record index << 32 | chunk index     a whole work item (the object has duplicated time stamps:
 //                                                          every one of its evals ties)
-constexpr int DEFER_T = 128;
 
 __device__ __forceinline__ unsigned long long sortable_bits(double v)
 {
@@ -120,6 +134,8 @@ __device__ __forceinline__ unsigned long long sortable_bits(double v)
     return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
 }
 
+// STAGE: per-eval arrays in this CTA's slot of the global staging scratch (light curves beyond the shared-memory limit)
+template <int DEFER_T, bool STAGE>
 __global__ void __launch_bounds__(DEFER_T) deferred_eval_kernel(const EvalParams p, double* dval,
                                                                 unsigned long long* dmax)
 {
@@ -130,7 +146,7 @@ __global__ void __launch_bounds__(DEFER_T) deferred_eval_kernel(const EvalParams
     __shared__ int s_flags[4];
     BlockCtx<DEFER_T> cx;
     cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
-    double* S = reinterpret_cast<double*>(smem_raw);
+    double* S = STAGE ? p.stage + (int64_t)blockIdx.x * p.stage_stride : reinterpret_cast<double*>(smem_raw);
     const unsigned cnt = min(p.defer_count[0], p.defer_capacity);
     for (unsigned e = blockIdx.x; e < cnt; e += gridDim.x) {
         const unsigned long long ent = p.defer_entries[e];
@@ -207,10 +223,15 @@ __global__ void deferred_merge_kernel(const EvalParams p, const double* dval, co
 ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, int sm_count,
                                  cudaStream_t stream)
 {
+    if (max_n > BLOCK_MAX_N) {
+        // the staging scratch holds 2 slots per SM (Engine::setup)
+        deferred_eval_kernel<512, true><<<sm_count * 2, 512, 0, stream>>>(p, dval, dmax);
+        return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
+    }
     const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(max_n) * 8;
-    if (cudaFuncSetAttribute(deferred_eval_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    if (cudaFuncSetAttribute(deferred_eval_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return SS_ERR_CUDA;
-    deferred_eval_kernel<<<sm_count * 4, DEFER_T, smem, stream>>>(p, dval, dmax);
+    deferred_eval_kernel<128, false><<<sm_count * 4, 128, smem, stream>>>(p, dval, dmax);
     return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
 }
 

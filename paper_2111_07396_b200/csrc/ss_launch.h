@@ -15,6 +15,9 @@ ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items
 // G-warps-per-eval kernels (ss_group_kernel.cuh); variant = group_variant_for_n(n)
 ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 
+// cluster-per-eval kernels (ss_cluster_kernel.cuh); variant = cluster_variant_for_n(n); n_items clusters
+ss_status_t launch_cluster_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
+
 // CTA-per-eval kernels (ss_block_kernel.cuh): path = SS_PATH_BLOCK (threads = 128 / 256 / 512, per-eval arrays in
 // shared memory sized for max_n) or SS_PATH_STAGE (512 threads, arrays in p.stage); opt = listing options compiled in
 ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int max_n, bool opt, int64_t n_items,

@@ -20,7 +20,18 @@ inline int path_for_n(int64_t n, int /*mode*/)
 {
     if (n <= SS_WARP_MAX_N) return SS_PATH_WARP;
     if (n <= SS_GROUP_MAX_N) return SS_PATH_GROUP;
+    if (n <= SS_CLUSTER_MAX_N) return SS_PATH_CLUSTER;
     return SS_PATH_STAGE;
+}
+
+// Cluster-path kernel variant: R CTAs of 512 threads x C points per thread, the smallest capacity R*512*C >= n
+// (3,072 ... 40,960).  id = R*8 + C.
+inline int cluster_variant_for_n(int n)
+{
+    for (int r = 2; r <= 16; r <<= 1)
+        for (int c = 3; c <= 5; c++)
+            if (r * 512 * c >= n) return r * 8 + c;
+    return 16 * 8 + 5;
 }
 
 // Group-path kernel variant of an object: G warps x C points per thread, the smallest capacity 32*G*C >= n

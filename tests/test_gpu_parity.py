@@ -145,10 +145,14 @@ def test_config4_reduced_and_planner_tiling(ss, mode):
 def test_config5_reduced_global_staging(ss, mode):
     """n = 20,000 (exceeds one SM's shared memory -> SS_PATH_STAGE), 40 frequencies."""
     cat = ss_inputs.make(5).with_grid(n_freq=40)
-    assert ss.path_for_n(20000) == ss.PATH_STAGE
+    assert ss.path_for_n(20000) == ss.PATH_CLUSTER
     res, ref = run_both(ss, cat, mode, oracle.FAST)
     check_parity(cat, res.pgram, ref, mode, label="cfg5")
     check_best(ref, res.best_index, res.best_freq, cat)
+    staged = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                            force_path=ss.PATH_STAGE)
+    check_parity(cat, staged.pgram, ref, mode, label="cfg5/stage")
+    check_best(ref, staged.best_index, staged.best_freq, cat)
     # two evals against the definition oracle (long double direct window sums)
     t, y, e = cat.obj(0)
     for k in (3, 31):
@@ -710,3 +714,33 @@ def test_group_kernel_every_variant(ss, mode):
     res2 = ss.periodogram(times, mags, errs, offs, 0.5, 24.0, 65, mode, force_path=ss.PATH_GROUP)
     check_parity(cat2, res2.pgram, ref2, mode, label="group small")
     check_best(ref2, res2.best_index, res2.best_freq, cat2)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_cluster_kernel_every_cluster_size(ss, mode):
+    """The cluster-per-eval kernels: R = 2, 4, 8, 16 CTAs x C = 3, 4, 5 points per thread, an object at both ends of
+    several capacities (3,072 ... 40,960 points), decade-long nightly sampling, against the oracle (its fp64 variant,
+    held to the long-double one by the pins; the smallest object also against the long-double variant).  One object
+    has two duplicated time stamps: every one of its evals is handed over to the global-staging kernel."""
+    rng = np.random.default_rng(616)
+    ns = [2056, 3072, 3073, 5120, 6000, 10240, 12288, 16385, 20480, 24577, 40960]
+    T, Y, E = [], [], []
+    for i, n in enumerate(ns):
+        assert ss.path_for_n(n) == ss.PATH_CLUSTER
+        t = np.sort(rng.integers(0, 3652, size=n) + rng.uniform(0.0, 0.3, size=n))
+        if n == 6000:
+            t[100] = t[99]; t[4000] = t[3999]
+        P = np.exp(rng.uniform(np.log(0.2), np.log(2.0)))
+        e = rng.uniform(0.01, 0.1, size=n)
+        y = 15 + rng.uniform(0.1, 0.5) * np.sin(2 * np.pi * t / P + i) + rng.normal(0, 1.0, size=n) * e
+        T.append(t); Y.append(y); E.append(e)
+    off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
+    cat = ss_inputs.Catalog("cluster", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
+                            0.01, 20.0, 9, np.full(len(ns), np.nan))
+    res, ref = run_both(ss, cat, mode, oracle.FAST)
+    check_parity(cat, res.pgram, ref, mode, label="cluster variants")
+    check_best(ref, res.best_index, res.best_freq, cat)
+    t, y, e = cat.obj(0)
+    for k in (2, 7):
+        r = oracle.eval_one(t, y, e, oracle.freq(cat.f_min, cat.f_max, cat.n_freq, k), mode=mode, variant=oracle.DEFINITION)
+        assert abs(res.pgram[0, k] - r["P"]) <= _tol(r["P"])

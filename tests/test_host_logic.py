@@ -57,8 +57,10 @@ def test_path_classes():
     assert ss.path_for_n(257) == ss.PATH_GROUP
     assert ss.path_for_n(2000) == ss.PATH_GROUP
     assert ss.path_for_n(2055) == ss.PATH_GROUP
-    assert ss.path_for_n(2056) == ss.PATH_STAGE
-    assert ss.path_for_n(20000) == ss.PATH_STAGE
+    assert ss.path_for_n(2056) == ss.PATH_CLUSTER
+    assert ss.path_for_n(20000) == ss.PATH_CLUSTER
+    assert ss.path_for_n(40960) == ss.PATH_CLUSTER
+    assert ss.path_for_n(40961) == ss.PATH_STAGE
 
 
 @pytest.mark.parametrize("cap_mib", [128, 256, 1024, 16384])
