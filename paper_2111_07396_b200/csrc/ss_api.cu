@@ -588,9 +588,12 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         int64_t cpo = std::min<int64_t>(cpo_cap, nk);
         int64_t chunk = (nk + cpo - 1) / cpo;
         if (c.path == SS_PATH_WARP) chunk = (chunk + WARPS_PER_CTA - 1) / WARPS_PER_CTA * WARPS_PER_CTA;
-        // a cluster sets up tensor memory and its window tables per work item: at least 64 evals each while that
-        // still leaves a few hundred items
-        if (c.path == SS_PATH_CLUSTER && chunk < 64 && nk * (int64_t)c.recs.size() >= 64 * 512) chunk = 64;
+        // a cluster sets up tensor memory and its window tables per work item: up to 64 evals each while that still
+        // leaves a few hundred items
+        if (c.path == SS_PATH_CLUSTER) {
+            const int64_t want = std::max<int64_t>(1, std::min<int64_t>(64, nk * (int64_t)c.recs.size() / 256));
+            if (chunk < want) chunk = want;
+        }
         cpo = (nk + chunk - 1) / chunk;
         p.chunk = (int32_t)chunk; p.chunks_per_obj = (int32_t)cpo;
         p.chunks_total = (int32_t)cpo_cap; p.chunk_base = 0;

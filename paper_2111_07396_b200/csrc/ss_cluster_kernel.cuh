@@ -236,8 +236,24 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const EvalParams p, c
     cluster_sync_all();
 
     // remote access to a pair-prefix array: element `w` = rank << 16 | index
-    auto ldE = [&](uint32_t base, int w) { return ld_cl_d2(mapa_u32(base + ((uint32_t)(w & 0xffff) << 4), (uint32_t)(w >> 16))); };
-    auto ldE8 = [&](uint32_t base, int w) { return ld_cl_d(mapa_u32(base + ((uint32_t)(w & 0xffff) << 3), (uint32_t)(w >> 16))); };
+    // (distributed shared memory moves ~20 B per clock per SM against 128 B for the SM's own: the part of a window that
+    // falls into this CTA's slice -- most tweeter windows, a fifth of the midrange ones -- is read with a plain LDS)
+    auto ldE = [&](uint32_t base, int w) {
+        const int r = w >> 16;
+        const uint32_t a = base + ((uint32_t)(w & 0xffff) << 4);
+        double2 v;
+        if (r == rank) asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a) : "memory");
+        else v = ld_cl_d2(mapa_u32(a, (uint32_t)r));
+        return v;
+    };
+    auto ldE8 = [&](uint32_t base, int w) {
+        const int r = w >> 16;
+        const uint32_t a = base + ((uint32_t)(w & 0xffff) << 3);
+        double v;
+        if (r == rank) asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory");
+        else v = ld_cl_d(mapa_u32(a, (uint32_t)r));
+        return v;
+    };
 
     // Mailbox round: every CTA has published s_mail (tot[0..NS-1], bad; optionally first / last / q); after the cluster
     // barrier warp 0 gathers what this CTA needs: the carry of the CTAs in front of it and the cluster-wide verdict.
@@ -309,6 +325,15 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const EvalParams p, c
             xa += a[i]; xb += b[i];
         }
         if (tid == NT - 1) E[NT] = make_double2(xa, xb);      // used only in the last CTA (the grand total)
+    };
+    // one stream, plain doubles (CV keeps wxy alone: 8-byte window ends); carry in s_carry[which].x
+    auto finish_one = [&](const PairScan& s, const double (&a)[C], int which, double* E) {
+        double ca = s_carry[which].x;
+        for (int q = 0; q < warp; q++) ca += s_tot[which][q].x;
+        double xa = ca + (s.ia - s.ra);
+#pragma unroll
+        for (int i = 0; i < C; i++) { E[i * ROW + tid] = xa; xa += a[i]; }
+        if (tid == NT - 1) E[NT] = xa;
     };
     auto hand_over = [&](int64_t k) {
         if (rank == 0 && tid == 0) {
@@ -445,7 +470,8 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const EvalParams p, c
         if (!skip) {
             finish_pair(ps0, ma, mb, 0, E01);
             finish_pair(ps1, mc_, md, 1, E23);
-            finish_pair(ps2, me, mf, 2, E45);
+            if (GV) finish_pair(ps2, me, mf, 2, E45);
+            else finish_one(ps2, me, 2, reinterpret_cast<double*>(E45));
             const double vsmlsq = s_vs;
             cluster_sync_all();
             double chi2 = 0.0;
@@ -491,9 +517,9 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const EvalParams p, c
                     for (int s = 0; s < C; s++) {
                         const int a_ = wi[s], b_ = wi[C + s];
                         const double2 l0 = ldE(a_E01, a_), h0 = ldE(a_E01, b_), l1 = ldE(a_E23, a_), h1 = ldE(a_E23, b_);
-                        const double2 l2 = ldE(a_E45, a_), h2 = ldE(a_E45, b_);
+                        const double lxy = ldE8(a_E45, a_), hxy = ldE8(a_E45, b_);
                         const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                        const double Sxy = h2.x - l2.x;
+                        const double Sxy = hxy - lxy;
                         const double isw = rcp64(Sw), xb = Swx * isw;
                         const double sxx = Swxx - xb * Swx;
                         const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
