@@ -36,7 +36,7 @@
 extern "C" {
 #endif
 
-#define SS_VERSION 100 /* 0.1.0 */
+#define SS_VERSION 200 /* 0.2.0 */
 
 typedef enum {
     SS_MODE_CROSS_VALIDATION = 0,      /* Listing 1, PAPER.md:127-297 (paper: SSO-*)            */
@@ -131,6 +131,36 @@ ss_status_t ss_periodogram_host(const double *times, const double *mags, const d
                                 double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
                                 double *pgram_out, double *best_freq_out, int64_t *best_index_out,
                                 const ss_options_t *opt);
+
+/* ------------------------------------------------------------------ top-k peaks */
+
+#define SS_MAX_PEAKS 32
+
+/*
+ * The n_peaks highest PEAKS of every periodogram row.  Algorithm 1 returns only the argmax, but the
+ * daily cadence of ground-based surveys aliases the true period into several comparable maxima (Fig. 1),
+ * so a caller usually wants the leading candidates.  A peak is a local maximum of the row:
+ *     P[k] > P[k-1]  and  P[k] >= P[k+1]
+ * (a neighbour outside the grid does not disqualify; of a flat top the first index counts; NaN never qualifies).
+ * Per object the peaks are ordered by falling power, equal powers by rising index; rows with fewer than n_peaks
+ * peaks are padded with index -1, power NaN, frequency NaN.  peak 0 of a row is its argmax whenever the argmax is
+ * unique.
+ *   pgram          : const double[n_objects][row_stride], row-major, columns 0 .. n_freq-1 used (what ss_periodogram*
+ *                    wrote: row_stride = n_freq, or k_count for a grid sub-range -- then pass the sub-range's own
+ *                    f_min + k_begin*df as f_min and its end as f_max)
+ *   peak_index_out : int64_t[n_objects][n_peaks]   column index k
+ *   peak_power_out : double [n_objects][n_peaks]   P[k]                       (may be NULL)
+ *   peak_freq_out  : double [n_objects][n_peaks]   f_min + k*(f_max-f_min)/n_freq   (may be NULL)
+ * ss_periodogram_peaks: DEVICE pointers, work enqueued on `stream` (cudaStream_t; NULL = default stream), returns
+ * after it completed.  ss_periodogram_peaks_host: HOST pointers; rows go through the device in slabs.
+ * 1 <= n_peaks <= SS_MAX_PEAKS, n_freq >= 1, row_stride >= n_freq, else SS_ERR_INVALID_ARG.
+ */
+ss_status_t ss_periodogram_peaks(const double *pgram, int64_t n_objects, int64_t n_freq, int64_t row_stride,
+                                 double f_min, double f_max, int n_peaks, int64_t *peak_index_out,
+                                 double *peak_power_out, double *peak_freq_out, void *stream);
+ss_status_t ss_periodogram_peaks_host(const double *pgram, int64_t n_objects, int64_t n_freq, int64_t row_stride,
+                                      double f_min, double f_max, int n_peaks, int64_t *peak_index_out,
+                                      double *peak_power_out, double *peak_freq_out);
 
 /* ------------------------------------------------------------------ batch planner (host only) */
 

@@ -146,3 +146,24 @@ def periodogram(times, mags, errs, offsets, f_min, f_max, n_freq, *, mode=CV, va
 
 def max_threads():
     return min(lib().sso_max_threads(), os.cpu_count() or 1)
+
+
+def peaks(row, n_peaks):
+    """The n_peaks highest PEAKS of one periodogram row, written out (include/ss_periodogram.h, ss_periodogram_peaks;
+    motivation PAPER.md:67, Fig. 1): k is a peak if P[k] > P[k-1] and P[k] >= P[k+1], a neighbour outside the grid
+    does not disqualify, NaN never qualifies; ordered by falling power, equal powers by rising index; padded with
+    index -1 / power NaN.  Plain Python loop: test infrastructure."""
+    row = np.asarray(row, dtype=np.float64)
+    n = len(row)
+    found = []
+    for k in range(n):
+        left = row[k - 1] if k > 0 else -np.inf
+        right = row[k + 1] if k + 1 < n else -np.inf
+        if row[k] > left and row[k] >= right:
+            found.append((-row[k], k))
+    found.sort()
+    idx = np.full(n_peaks, -1, dtype=np.int64)
+    val = np.full(n_peaks, np.nan)
+    for j, (nv, k) in enumerate(found[:n_peaks]):
+        idx[j], val[j] = k, -nv
+    return idx, val

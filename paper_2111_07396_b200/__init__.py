@@ -24,7 +24,7 @@ LIB_PATH = os.path.join(_HERE, "libss_b200.so")
 EXPORTS = ["ss_default_options", "ss_periodogram", "ss_periodogram_ex", "ss_periodogram_host",
            "ss_plan", "ss_workspace_bytes", "ss_paper_footprint_bytes", "ss_paper_batches",
            "ss_path_for_n", "ss_debug_eval", "ss_microbench", "ss_last_launch_count", "ss_last_kernel_ms", "ss_last_kernel_count",
-           "ss_last_error", "ss_version", "ss_release_workspace"]
+           "ss_last_error", "ss_version", "ss_release_workspace", "ss_periodogram_peaks", "ss_periodogram_peaks_host"]
 
 
 class SSError(RuntimeError):
@@ -86,6 +86,9 @@ def load():
     L.ss_last_error.restype = C.c_char_p
     L.ss_version.restype = C.c_int
     L.ss_release_workspace.restype = None
+    peaks = [vp, i64, i64, i64, d, d, C.c_int, vp, vp, vp]
+    L.ss_periodogram_peaks.argtypes = peaks + [vp]
+    L.ss_periodogram_peaks_host.argtypes = peaks
     _lib = L
     return L
 
@@ -239,6 +242,33 @@ def periodogram(times, mags, errs, offsets, f_min, f_max, n_freq, mode=CROSS_VAL
     ss_periodogram_host(times, mags, errs, offsets, n_obj, f_min, f_max, n_freq, mode, pg, bf, bi,
                         default_options(**opts))
     return Result(pg, bf, bi)
+
+
+def ss_periodogram_peaks(pgram, n_objects, n_freq, row_stride, f_min, f_max, n_peaks, peak_index_out,
+                         peak_power_out=None, peak_freq_out=None):
+    """Device-tensor call (include/ss_periodogram.h: ss_periodogram_peaks); enqueued on torch's current stream."""
+    torch = _torch()
+    _check(load().ss_periodogram_peaks(_dev_ptr(pgram, torch.float64, "pgram"), int(n_objects), int(n_freq), int(row_stride),
+                                       float(f_min), float(f_max), int(n_peaks),
+                                       _dev_ptr(peak_index_out, torch.int64, "peak_index_out"),
+                                       _dev_ptr(peak_power_out, torch.float64, "peak_power_out"),
+                                       _dev_ptr(peak_freq_out, torch.float64, "peak_freq_out"),
+                                       C.c_void_p(torch.cuda.current_stream().cuda_stream)))
+
+
+def peaks(pgram, f_min, f_max, n_peaks):
+    """Convenience wrapper: numpy periodogram [n_objects, n_freq] in, (index, power, freq) [n_objects, n_peaks] out,
+    through ss_periodogram_peaks_host."""
+    _torch()
+    pgram = np.ascontiguousarray(pgram, dtype=np.float64)
+    n_obj, n_freq = pgram.shape
+    pi = np.empty((n_obj, n_peaks), dtype=np.int64)
+    pv = np.empty((n_obj, n_peaks))
+    pf = np.empty((n_obj, n_peaks))
+    _check(load().ss_periodogram_peaks_host(_host_ptr(pgram, np.float64, "pgram"), n_obj, n_freq, n_freq, float(f_min),
+                                            float(f_max), int(n_peaks), _host_ptr(pi, np.int64, "pi"),
+                                            _host_ptr(pv, np.float64, "pv"), _host_ptr(pf, np.float64, "pf")))
+    return pi, pv, pf
 
 
 def debug_eval(times, mags, errs, freq, mode=CROSS_VALIDATION, **opts):

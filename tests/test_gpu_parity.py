@@ -744,3 +744,54 @@ def test_cluster_kernel_every_cluster_size(ss, mode):
     for k in (2, 7):
         r = oracle.eval_one(t, y, e, oracle.freq(cat.f_min, cat.f_max, cat.n_freq, k), mode=mode, variant=oracle.DEFINITION)
         assert abs(res.pgram[0, k] - r["P"]) <= _tol(r["P"])
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_top_k_peaks(ss, mode):
+    """ss_periodogram_peaks: on the library's OWN periodogram the peak indices must be bit-identical to
+    the definition written out (oracle.peaks, a plain Python loop); against the oracle's periodogram they agree
+    wherever the oracle's row separates its peaks by more than the parity tolerance.  Covers rows with fewer peaks
+    than asked for, NaN rows (n < 5), a constant row (all zeros: one flat top at index 0), n_peaks = 1 = the argmax,
+    a one-column grid, and both entry points."""
+    import torch
+    cat = ss_inputs.config3(n_objects=24, n_freq=2000)
+    # add a degenerate object (NaN row) and a constant one (row of zeros)
+    times = np.concatenate([cat.times, [0.0, 1.0, 2.5], np.linspace(0, 20, 30)])
+    mags = np.concatenate([cat.mags, [15.0, 15.1, 15.2], np.full(30, 15.5)])
+    errs = np.concatenate([cat.errs, [0.1, 0.1, 0.1], np.full(30, 0.05)])
+    off = np.concatenate([cat.offsets, [cat.offsets[-1] + 3, cat.offsets[-1] + 33]])
+    res = ss.periodogram(times, mags, errs, off, cat.f_min, cat.f_max, cat.n_freq, mode)
+    ref, _, _ = oracle.periodogram(times, mags, errs, off, cat.f_min, cat.f_max, cat.n_freq, mode=mode, variant=oracle.FAST)
+    n_obj = len(off) - 1
+    for k in (1, 3, 8, 13, 32):
+        pi, pv, pf = ss.peaks(res.pgram, cat.f_min, cat.f_max, k)
+        for o in range(n_obj):
+            ei, ev = oracle.peaks(res.pgram[o], k)
+            assert np.array_equal(pi[o], ei), (k, o)
+            assert np.array_equal(pv[o], ev, equal_nan=True)
+            ok = ei >= 0
+            assert np.array_equal(pf[o][ok], [oracle.freq(cat.f_min, cat.f_max, cat.n_freq, int(j)) for j in ei[ok]])
+            assert np.all(np.isnan(pf[o][~ok]))
+            # against the oracle's own row: same peaks where its leading peaks are separated by more than the tolerance
+            ri, rv = oracle.peaks(ref[o], k + 1)
+            gaps = np.abs(np.diff(rv[~np.isnan(rv)]))
+            if len(gaps) == k and np.all(gaps > 1e-6):
+                assert np.array_equal(pi[o], ri[:k]), (k, o)
+        assert np.all(pi[n_obj - 2] == -1) and np.all(np.isnan(pv[n_obj - 2]))            # NaN row
+        assert pi[n_obj - 1][0] == 0 and np.all(pi[n_obj - 1][1:] == -1)                   # row of zeros: one flat top
+        if k == 1:
+            real = res.best_index >= 0
+            assert np.array_equal(pi[real, 0], res.best_index[real])
+    # device entry point, strided rows, a sub-range of the columns
+    dev = torch.device("cuda")
+    pg = torch.as_tensor(res.pgram, device=dev)
+    di = torch.empty((n_obj, 5), dtype=torch.int64, device=dev)
+    dv = torch.empty((n_obj, 5), dtype=torch.float64, device=dev)
+    ss.ss_periodogram_peaks(pg, n_obj, 700, cat.n_freq, cat.f_min, cat.f_min + 700 * cat.df, 5, di, dv, None)
+    for o in range(n_obj):
+        ei, ev = oracle.peaks(res.pgram[o, :700], 5)
+        assert np.array_equal(di[o].cpu().numpy(), ei) and np.array_equal(dv[o].cpu().numpy(), ev, equal_nan=True)
+    one_i, one_v, _ = ss.peaks(res.pgram[:3, :1], cat.f_min, cat.f_max, 2)
+    assert np.all(one_i[:, 0] == 0) and np.all(one_i[:, 1] == -1)
+    with pytest.raises(ss.SSError):
+        ss.peaks(res.pgram, cat.f_min, cat.f_max, 33)

@@ -22,7 +22,7 @@ def test_library_exports_every_declared_symbol():
     for name in sorted(declared):
         assert hasattr(lib, name), name
     assert declared == set(ss.EXPORTS)
-    assert ss.version() == 100
+    assert ss.version() == 200
 
 
 def test_paper_footprint_fixture():
