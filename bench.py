@@ -57,6 +57,8 @@ def parse():
                     help="another BASELINE.json config (profiles/r2_bench_configs.md); the bench line proper is config 3")
     ap.add_argument("--objects", type=int, default=None, help="(debug) fewer objects than the config has (configs 3, 4)")
     ap.add_argument("--freqs", type=int, default=None, help="(debug) fewer frequencies than the config has")
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="mixed = the paper's FP32 switch as built here (fp32 smoother for 256 < n <= 2,055; never the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()
@@ -249,7 +251,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
 
     def step(m=mode, profile=False):
-        o = ss.default_options(profile=1 if profile else 0)
+        o = ss.default_options(profile=1 if profile else 0, precision=1 if args.precision == "mixed" else 0)
         ss.ss_periodogram(t, y, e, off, n_obj, cat.f_min, cat.f_max, n_freq, m, pg, bf, bi, o)
 
     sampler = ClockSampler(local)
@@ -299,7 +301,7 @@ def run_ours(args):
         hbi = torch.empty(n_obj, dtype=torch.int64).pin_memory()
         def estep():
             ss.ss_periodogram_host(ht, hy, he, hoff, n_obj, cat.f_min, cat.f_max, n_freq, mode, hpg, hbf, hbi,
-                                   ss.default_options())
+                                   ss.default_options(precision=1 if args.precision == "mixed" else 0))
         estep()
         barrier()
         t0 = time.perf_counter()
@@ -352,9 +354,10 @@ def run_ours(args):
         cpu, _, _ = cpu_baseline(cat, args.mode)
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "vs_baseline": None, "dtype": "f64" if args.precision == "f64" else "f32", "data": "synthetic",
            "config": {"workload": f"config{args.config}: {n_obj} objects ({cat.n_points} points) x {n_freq} "
-                      f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised",
+                      f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised"
+                      + (", precision=mixed (fp32 smoother on the group path; fp64 fold, sort and prefix accumulation)" if args.precision == "mixed" else ""),
                       "objects_per_second": world * n_obj * args.steps / (elapsed_ms * 1e-3),
                       "l2": (f"inputs ({24 * cat.n_points / 1e6:.0f} MB catalog) are re-read per frequency by design; the "
                              f"{8 * evals_per_step / 1e9:.2f} GB periodogram written every step "

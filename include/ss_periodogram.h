@@ -51,6 +51,8 @@ typedef enum {
     SS_ERR_UNSUPPORTED = 4    /* an object above 2^24 points, or more work items than one tile can index  */
 } ss_status_t;
 
+typedef enum { SS_PRECISION_F64 = 0, SS_PRECISION_MIXED = 1 } ss_precision_t;
+
 /* Which kernel family serves an object (chosen by its number of points n). */
 typedef enum {
     SS_PATH_AUTO = 0,
@@ -89,6 +91,13 @@ typedef struct {
                                columns (column 0 = index k_begin), best_index stays an index into the whole
                                grid.  k_count = 0: up to the end of the grid.  For splitting one object's
                                frequency range across GPUs.                           */
+    int precision;          /* ss_precision_t.  SS_PRECISION_F64 (default): everything in fp64.  SS_PRECISION_MIXED
+                               (the paper's FP32 switch): for objects of SS_WARP_MAX_N < n <=
+                               SS_GROUP_MAX_N points the smoother runs in fp32 -- prefix arrays stored and window fits,
+                               residuals, span selection and interpolation computed in float -- while the fold, the
+                               sort, the centring and the accumulation of the prefix sums stay in fp64 (the
+                               permutation is therefore the fp64 one).  Shorter and longer light curves are served in
+                               fp64.  Periodogram values then agree with the fp64 result to about 1e-4 absolute.       */
     unsigned int defer_capacity; /* test hook: entries of the list through which the warp-per-eval kernels hand
                                tied / undecidable evals to the generic kernel, per tile (0 = 2^20).  When it
                                overflows the call repeats itself on the CTA-per-eval kernels; results never

@@ -16,6 +16,7 @@ import numpy as np
 CROSS_VALIDATION = 0
 GENERALIZED_VALIDATION = 1
 PATH_AUTO, PATH_WARP, PATH_BLOCK, PATH_STAGE, PATH_GROUP, PATH_CLUSTER = 0, 1, 2, 3, 4, 5
+PRECISION_F64, PRECISION_MIXED = 0, 1
 SS_OK, SS_ERR_INVALID_ARG, SS_ERR_OUT_OF_MEMORY, SS_ERR_CUDA, SS_ERR_UNSUPPORTED = range(5)
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -37,7 +38,7 @@ class Options(C.Structure):
     _fields_ = [("alpha", C.c_double), ("span", C.c_double), ("iper", C.c_int),
                 ("force_path", C.c_int), ("stream", C.c_void_p), ("workspace_cap", C.c_size_t),
                 ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int),
-                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("defer_capacity", C.c_uint)]
+                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("precision", C.c_int), ("defer_capacity", C.c_uint)]
 
 
 class Plan(C.Structure):

@@ -409,6 +409,8 @@ static ss_status_t validate_scalars(int64_t n_objects, double f_min, double f_ma
     if (!(o.span >= 0.0) || !(o.span <= 1.0)) return fail(SS_ERR_INVALID_ARG, "span must be 0 (variable) or in (0, 1]");
     if (o.iper != 1 && o.iper != 2) return fail(SS_ERR_INVALID_ARG, "iper = %d (1 = non-periodic, 2 = periodic)", o.iper);
     if (!std::isfinite(o.alpha)) return fail(SS_ERR_INVALID_ARG, "alpha is not finite");
+    if (o.precision != SS_PRECISION_F64 && o.precision != SS_PRECISION_MIXED)
+        return fail(SS_ERR_INVALID_ARG, "precision = %d (0 = fp64, 1 = mixed)", o.precision);
     if (o.k_begin < 0 || o.k_count < 0 || o.k_begin >= n_freq || o.k_begin + o.k_count > n_freq)
         return fail(SS_ERR_INVALID_ARG, "k_begin/k_count outside the grid");
     return SS_OK;
@@ -493,7 +495,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
             if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
-            else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n);
+            else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? GROUP_VARIANT_F32 : 0);
             else if (path == SS_PATH_CLUSTER) variant = cluster_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
             else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);

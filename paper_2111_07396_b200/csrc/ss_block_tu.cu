@@ -75,10 +75,22 @@ ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items
 #define SS_DECL(gv, g) ss_status_t launch_group_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
 SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
 #undef SS_DECL
+#define SS_DECL(gv, g) ss_status_t launch_group_f32_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
+SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
+#undef SS_DECL
 
 ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
 {
+    const bool f32 = variant >= GROUP_VARIANT_F32;
+    if (f32) variant -= GROUP_VARIANT_F32;
     const int g = variant / 8, c = variant % 8;
+    if (f32) {
+        if (p.mode == 1)
+            return g == 4 ? launch_group_f32_tu_1_4(p, c, n_items, stream)
+                 : g == 8 ? launch_group_f32_tu_1_8(p, c, n_items, stream) : launch_group_f32_tu_1_16(p, c, n_items, stream);
+        return g == 4 ? launch_group_f32_tu_0_4(p, c, n_items, stream)
+             : g == 8 ? launch_group_f32_tu_0_8(p, c, n_items, stream) : launch_group_f32_tu_0_16(p, c, n_items, stream);
+    }
     if (p.mode == 1)
         return g == 4 ? launch_group_tu_1_4(p, c, n_items, stream)
              : g == 8 ? launch_group_tu_1_8(p, c, n_items, stream) : launch_group_tu_1_16(p, c, n_items, stream);

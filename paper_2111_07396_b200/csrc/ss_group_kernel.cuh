@@ -15,20 +15,106 @@
 // Evals this path cannot decide exactly (tied phases, a bucket that one adjacent swap does not settle, a
 // leave-one-out denominator <= 0) are handed to the generic CTA-per-eval kernel through the same list the warp path
 // uses, so results never depend on which path ran.
+//
+// The kernel is templated on the smoother's scalar T ("toggle between using FP32 or FP64").
+// T = double is the library's default.  T = float is the MIXED mode (ss_options_t::precision): the fold, the sort, the
+// centring of x and y and the ACCUMULATION of every prefix sum stay in fp64 (a window sum is the difference of two
+// prefixes of magnitude ~n/K times its own: rounding the accumulation to fp32 would leave no digits), the prefix
+// arrays are stored, and every window fit, residual, span pick and interpolation is computed, in fp32.
 #pragma once
 #include "ss_warp_kernel.cuh"
 
 namespace ss {
 
-template <int G, int C> struct GroupCfg {
+template <typename T> struct Real;
+template <> struct Real<double> {
+    using vec2 = double2;
+    static constexpr int WORDS = 2;             // 32-bit tensor-memory columns per value
+    static constexpr int TINY = 0x00100000;     // high word of the smallest normal
+    static __device__ __forceinline__ double2 make2(double a, double b) { return make_double2(a, b); }
+    static __device__ __forceinline__ double rcp(double x) { return rcp64(x); }
+    static __device__ __forceinline__ double sqrt0(double x) { return sqrt64(x); }
+    static __device__ __forceinline__ double wpad() { return W_PAD; }
+    static __device__ __forceinline__ int hi_word(double a) { return __double2hiint(a); }
+};
+template <> struct Real<float> {
+    using vec2 = float2;
+    static constexpr int WORDS = 1;
+    static constexpr int TINY = 0x00800000;
+    static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
+    static __device__ __forceinline__ float rcp(float x) { return __frcp_rn(x); }
+    static __device__ __forceinline__ float sqrt0(float x) { return x > 0.0f ? sqrtf(x) : 0.0f; }
+    static __device__ __forceinline__ float wpad() { return 1.0e-30f; }
+    static __device__ __forceinline__ int hi_word(float a) { return __float_as_int(a); }
+};
+
+// parked values in tensor memory: doubles take two columns, floats one (arrays padded to an even number of columns)
+template <typename T, int N> struct TmemArr;
+template <int N> struct TmemArr<double, N> {
+    static constexpr uint32_t COLS = 2 * N;
+    static __device__ __forceinline__ void park(uint32_t a, const double (&v)[N]) { tmem_park<N>(a, v); }
+    static __device__ __forceinline__ void fetch(uint32_t a, double (&v)[N]) { tmem_fetch<N>(a, v); }
+};
+template <int N> struct TmemArr<float, N> {
+    static constexpr int NE = (N + 1) & ~1;
+    static constexpr uint32_t COLS = NE;
+    static __device__ __forceinline__ void park(uint32_t a, const float (&v)[N])
+    {
+        int w[N];
+#pragma unroll
+        for (int i = 0; i < N; i++) w[i] = __float_as_int(v[i]);
+        tmem_park_words<N>(a, w);
+    }
+    static __device__ __forceinline__ void fetch(uint32_t a, float (&v)[N])
+    {
+        int w[NE];
+        tmem_fetch_words<NE>(a, w);
+#pragma unroll
+        for (int i = 0; i < N; i++) v[i] = __int_as_float(w[i]);
+    }
+};
+
+// Listing 1 lines 63-77, loop-invariant tests hoisted (cf. pick_span_w), any scalar
+template <typename T>
+__device__ __forceinline__ T pick_span_t(T v0, T v1, T v2, int bass, double bexp)
+{
+    T resmin = v0, sp = (T)SPAN0;
+    if (v1 < resmin) { resmin = v1; sp = (T)SPAN1; }
+    if (v2 < resmin) { resmin = v2; sp = (T)SPAN2; }
+    if (bass != 0 && resmin < v2 && resmin > (T)0) {
+        T tmp = resmin * Real<T>::rcp(v2);
+        if (tmp < (T)1.e-7) tmp = (T)1.e-7;
+        const T pw = bass == 1 ? tmp : (T)pow((double)tmp, bexp);
+        sp += ((T)SPAN2 - sp) * pw;
+    }
+    return sp;
+}
+// Listing 1 lines 83-95 (R10), any scalar
+template <typename T>
+__device__ __forceinline__ T interp_spans_t(T sps, T A0, T A1, T A2)
+{
+    if (sps <= (T)SPAN0) sps = (T)SPAN0;
+    if (sps >= (T)SPAN2) sps = (T)SPAN2;
+    T f = sps - (T)SPAN1;
+    constexpr double G0 = 1.0 / (SPAN0 - SPAN1), G2 = 1.0 / (SPAN2 - SPAN1);
+    if (f < (T)0) {
+        f *= (T)G0;
+        return ((T)1 - f) * A1 + f * A0;
+    }
+    f *= (T)G2;
+    return ((T)1 - f) * A1 + f * A2;
+}
+
+template <int G, int C, typename T = double> struct GroupCfg {
     static constexpr int NT = 32 * G;               // threads
     static constexpr int NP = NT * C;               // capacity in points
     static constexpr int ROW = NT + 1;              // row of a transposed prefix array: NT threads + the total
     static constexpr int MINB = G == 4 ? 4 : (G == 8 ? 2 : 1);      // 16 warps per SM at 128 registers
     static constexpr int IDX_BITS = NP <= 512 ? 9 : (NP <= 1024 ? 10 : (NP <= 2048 ? 11 : 12));
     static constexpr unsigned IDX_MASK = (1u << IDX_BITS) - 1u;
-    // tensor memory per warp: 14C columns of parked doubles (A0, A1, A2, tweeter isw / xbar / g, y) + 6C window indices
-    static constexpr uint32_t TCOLS_WARP = 20 * C;
+    // tensor memory per warp: 7 parked arrays (A0, A1, A2, tweeter isw / xbar / g, y) + 6C window indices
+    static constexpr uint32_t PCOLS = TmemArr<T, C>::COLS;
+    static constexpr uint32_t TCOLS_WARP = 7 * PCOLS + 6 * C;
     static constexpr uint32_t TCOLS_NEED = TCOLS_WARP * (G / 4);
     static constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
     static_assert(TCOLS * MINB <= 512, "tensor memory over-subscribed");
@@ -65,70 +151,75 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                     "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
 }
 
-template <int G, int C, bool GV>
+template <int G, int C, bool GV, typename T = double>
 inline size_t group_smem_bytes()
 {
-    using Cfg = GroupCfg<G, C>;
-    // object arrays (3 x NP doubles) + 3 pair-prefix arrays of C*ROW double2 (the sort's exchange buffers overlay them)
-    return (size_t)3 * Cfg::NP * 8 + (size_t)3 * C * Cfg::ROW * 16;
+    using Cfg = GroupCfg<G, C, T>;
+    // object arrays (3 x NP doubles) + 3 pair-prefix arrays of C*ROW vec2 (the sort's exchange buffers, 2 x NT*C words,
+    // overlay the first of them: C*ROW*sizeof(vec2) >= 8*NT*C also for float2)
+    return (size_t)3 * Cfg::NP * 8 + (size_t)3 * C * Cfg::ROW * sizeof(typename Real<T>::vec2);
 }
 
 // Exclusive prefix sums of two streams over the whole CTA (C values per thread, blocked), stored interleaved and
 // transposed: E[(j % C)*ROW + j/C] = (sum_{i<j} a_i, sum_{i<j} b_i).  Phase 1 (before the barrier): lane-local sums,
 // Kogge-Stone over the warp, the warp's totals to `tot`; phase 2 (after it): the carry of the warps in front.
 struct PairScan { double ra, rb, ia, ib; };
-template <int C>
-__device__ __forceinline__ PairScan pair_scan_begin(const double (&a)[C], const double (&b)[C], double2* tot, int warp,
+template <int C, typename T>
+__device__ __forceinline__ PairScan pair_scan_begin(const T (&a)[C], const T (&b)[C], double2* tot, int warp,
                                                     int lane, const ScanMask& mk)
 {
+    // the thread's own C values are summed in T (C terms: no accuracy at stake), everything across threads in fp64:
+    // a float kernel then converts twice per thread and stream, not per element
     PairScan s;
-    s.ra = a[0]; s.rb = b[0];
+    T ra = a[0], rb = b[0];
 #pragma unroll
-    for (int i = 1; i < C; i++) { s.ra += a[i]; s.rb += b[i]; }
+    for (int i = 1; i < C; i++) { ra += a[i]; rb += b[i]; }
+    s.ra = (double)ra; s.rb = (double)rb;
     s.ia = s.ra; s.ib = s.rb;
 #pragma unroll
     for (int i = 0; i < 5; i++) { scan_step(s.ia, i, mk); scan_step(s.ib, i, mk); }
     if (lane == 31) tot[warp] = make_double2(s.ia, s.ib);
     return s;
 }
-template <int G, int C>
-__device__ __forceinline__ void pair_scan_finish(const PairScan& s, const double (&a)[C], const double (&b)[C],
-                                                 const double2* tot, double2* E, int warp, int tid)
+template <int G, int C, typename T>
+__device__ __forceinline__ void pair_scan_finish(const PairScan& s, const T (&a)[C], const T (&b)[C],
+                                                 const double2* tot, typename Real<T>::vec2* E, int warp, int tid)
 {
     constexpr int ROW = GroupCfg<G, C>::ROW;
     double ca = 0.0, cb = 0.0;
     for (int q = 0; q < warp; q++) { const double2 t = tot[q]; ca += t.x; cb += t.y; }      // warp-uniform: broadcast loads
-    double xa = ca + (s.ia - s.ra), xb = cb + (s.ib - s.rb);
+    T xa = (T)(ca + (s.ia - s.ra)), xb = (T)(cb + (s.ib - s.rb));
 #pragma unroll
     for (int i = 0; i < C; i++) {
-        E[i * ROW + tid] = make_double2(xa, xb);
+        E[i * ROW + tid] = Real<T>::make2(xa, xb);
         xa += a[i]; xb += b[i];
     }
-    if (tid == 32 * G - 1) E[32 * G] = make_double2(xa, xb);       // position NP lives at row 0, column NT
+    if (tid == 32 * G - 1) E[32 * G] = Real<T>::make2(xa, xb);       // position NP lives at row 0, column NT
 }
 // one stream, plain doubles (row length ROW doubles)
 struct OneScan { double ra, ia; };
-template <int C>
-__device__ __forceinline__ OneScan one_scan_begin(const double (&a)[C], double* tot, int warp, int lane, const ScanMask& mk)
+template <int C, typename T>
+__device__ __forceinline__ OneScan one_scan_begin(const T (&a)[C], double* tot, int warp, int lane, const ScanMask& mk)
 {
     OneScan s;
-    s.ra = a[0];
+    T ra = a[0];
 #pragma unroll
-    for (int i = 1; i < C; i++) s.ra += a[i];
+    for (int i = 1; i < C; i++) ra += a[i];
+    s.ra = (double)ra;
     s.ia = s.ra;
 #pragma unroll
     for (int i = 0; i < 5; i++) scan_step(s.ia, i, mk);
     if (lane == 31) tot[warp] = s.ia;
     return s;
 }
-template <int G, int C>
-__device__ __forceinline__ void one_scan_finish(const OneScan& s, const double (&a)[C], const double* tot, double* E,
+template <int G, int C, typename T>
+__device__ __forceinline__ void one_scan_finish(const OneScan& s, const T (&a)[C], const double* tot, T* E,
                                                 int warp, int tid)
 {
     constexpr int ROW = GroupCfg<G, C>::ROW;
     double ca = 0.0;
     for (int q = 0; q < warp; q++) ca += tot[q];
-    double xa = ca + (s.ia - s.ra);
+    T xa = (T)(ca + (s.ia - s.ra));
 #pragma unroll
     for (int i = 0; i < C; i++) { E[i * ROW + tid] = xa; xa += a[i]; }
     if (tid == 32 * G - 1) E[32 * G] = xa;
@@ -196,10 +287,13 @@ struct GroupConst {
 // ------------------------------------------------------------------------------------------------
 // Kernel: one CTA = one work item (object, chunk of frequencies), evals one after the other.
 // ------------------------------------------------------------------------------------------------
-template <int G, int C, bool GV>
-__global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) group_kernel(const EvalParams p)
+template <int G, int C, bool GV, typename T = double>
+__global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB) group_kernel(const EvalParams p)
 {
-    using Cfg = GroupCfg<G, C>;
+    using Cfg = GroupCfg<G, C, T>;
+    using RT = Real<T>;
+    using T2 = typename RT::vec2;
+    using TA = TmemArr<T, C>;
     constexpr int NT = Cfg::NT, NP = Cfg::NP, ROW = Cfg::ROW, ASZ = C * ROW;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ __align__(16) double2 s_tot[3][G];          // warp totals of up to three pair scans
@@ -232,9 +326,9 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
     double* o_tt = reinterpret_cast<double*>(smem_raw);
     double* o_y = o_tt + NP;
     double* o_w = o_y + NP;
-    double2* E01 = reinterpret_cast<double2*>(smem_raw + (size_t)3 * NP * 8);      // (w, wx)      | residual 0 | spans
-    double2* E23 = E01 + ASZ;                                                      // (wxx, wy)    | residual 1 | final
-    double2* E45 = E23 + ASZ;                                                      // (wxy[, wyy]) | residual 2
+    T2* E01 = reinterpret_cast<T2*>(smem_raw + (size_t)3 * NP * 8);                // (w, wx)      | residual 0 | spans
+    T2* E23 = E01 + ASZ;                                                           // (wxx, wy)    | residual 1 | final
+    T2* E45 = E23 + ASZ;                                                           // (wxy[, wyy]) | residual 2
     unsigned* kbuf = reinterpret_cast<unsigned*>(E01);                             // sort exchange (2 x NT*C words)
 
     // ---- stage the object once per work item: three bulk copies, one mbarrier
@@ -272,14 +366,13 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
     K.kc = s_kc;
     K.bexp = 10.0 - p.alpha;
     K.bass = (p.alpha > 0.0 && p.alpha <= 10.0) ? (K.bexp == 1.0 ? 1 : 2) : 0;
-    EvalConst KW;      // what pick_span_w reads
-    KW.bass = K.bass; KW.bexp = K.bexp;
 
     const ScanMask mk = make_scan_mask(lane);
     const uint32_t tmem = s_tmem + ((uint32_t)(warp & 3) << 21) + (uint32_t)(warp >> 2) * Cfg::TCOLS_WARP;
     // tensor-memory columns (32-bit words) of this warp
-    constexpr uint32_t T_A0 = 0, T_A1 = 2 * C, T_A2 = 4 * C, T_ISW = 6 * C, T_XB = 8 * C, T_G0 = 10 * C, T_Y = 12 * C;
-    constexpr uint32_t T_W0 = 14 * C, T_W1 = 16 * C, T_W2 = 18 * C;      // window indices (lo[C], hi[C]) per span
+    constexpr uint32_t PC = Cfg::PCOLS;
+    constexpr uint32_t T_A0 = 0, T_A1 = PC, T_A2 = 2 * PC, T_ISW = 3 * PC, T_XB = 4 * PC, T_G0 = 5 * PC, T_Y = 6 * PC;
+    constexpr uint32_t T_W0 = 7 * PC, T_W1 = T_W0 + 2 * C, T_W2 = T_W0 + 4 * C;      // window indices (lo[C], hi[C]) per span
     {
         int w0[2 * C], w1[2 * C], w2[2 * C];
 #pragma unroll
@@ -363,11 +456,11 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
             if (tid * C + s + 1 < n && phi[s + 1] <= phi[s]) bad = true;                   // tie, or a bucket of three
 
         // ---- gather; x centred by 0.5, padded slots carry x = 0, y = 0, w = W_PAD
-        double x[C], y[C], w[C];
+        T x[C], y[C], w[C];
 #pragma unroll
         for (int s = 0; s < C; s++) {
-            if (tid * C + s < n) { x[s] = phi[s] - 0.5; y[s] = o_y[idx[s]]; w[s] = o_w[idx[s]]; }
-            else { x[s] = 0.0; y[s] = 0.0; w[s] = W_PAD; }
+            if (tid * C + s < n) { x[s] = (T)(phi[s] - 0.5); y[s] = (T)o_y[idx[s]]; w[s] = (T)o_w[idx[s]]; }
+            else { x[s] = (T)0; y[s] = (T)0; w[s] = RT::wpad(); }
         }
         // quartile phases for vsmlsq
         if (tid == K.q1t) {
@@ -380,7 +473,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
         }
 
         // ---- prefix sums of the weighted moments
-        double ma[C], mb[C], mc[C], md[C], me[C];
+        T ma[C], mb[C], mc[C], md[C], me[C];
 #pragma unroll
         for (int s = 0; s < C; s++) {
             ma[s] = w[s]; mb[s] = w[s] * x[s]; mc[s] = mb[s] * x[s]; md[s] = w[s] * y[s]; me[s] = mb[s] * y[s];
@@ -388,7 +481,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
         const PairScan ps0 = pair_scan_begin<C>(ma, mb, s_tot[0], warp, lane, mk);
         const PairScan ps1 = pair_scan_begin<C>(mc, md, s_tot[1], warp, lane, mk);
         PairScan ps2; OneScan os2;
-        double mf[C];
+        T mf[C];
         if (GV) {
 #pragma unroll
             for (int s = 0; s < C; s++) mf[s] = md[s] * y[s];
@@ -408,17 +501,17 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
         }
         double P = 0.0;
         if (!bad) {
-            pair_scan_finish<G, C>(ps0, ma, mb, s_tot[0], E01, warp, tid);
-            pair_scan_finish<G, C>(ps1, mc, md, s_tot[1], E23, warp, tid);
-            if (GV) pair_scan_finish<G, C>(ps2, me, mf, s_tot[2], E45, warp, tid);
-            else one_scan_finish<G, C>(os2, me, reinterpret_cast<const double*>(s_tot[2]), reinterpret_cast<double*>(E45), warp, tid);
+            pair_scan_finish<G, C, T>(ps0, ma, mb, s_tot[0], E01, warp, tid);
+            pair_scan_finish<G, C, T>(ps1, mc, md, s_tot[1], E23, warp, tid);
+            if (GV) pair_scan_finish<G, C, T>(ps2, me, mf, s_tot[2], E45, warp, tid);
+            else one_scan_finish<G, C, T>(os2, me, reinterpret_cast<const double*>(s_tot[2]), reinterpret_cast<T*>(E45), warp, tid);
             const double scale = s_q[1] - s_q[0];
-            const double vsmlsq = 1.e-6 * scale * scale;
+            const T vsmlsq = (T)(1.e-6 * scale * scale);
             __syncthreads();                                                                // BAR 3
-            double chi2 = 0.0;
+            T chi2 = (T)0;
             if (GV) {
                 // ---- O6: three windows, scores, pick, interpolate
-                double A[3][C], Gs[3][C];
+                T A[3][C], Gs[3][C];
 #pragma unroll
                 for (int i = 0; i < 3; i++) {
                     int wi[2 * C];
@@ -426,64 +519,64 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
 #pragma unroll
                     for (int s = 0; s < C; s++) {
                         const int a_ = wi[s], b_ = wi[C + s];
-                        const double2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_], l2 = E45[a_], h2 = E45[b_];
-                        const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                        const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
-                        const double isw = rcp64(Sw), xb = Swx * isw;
-                        const double sxx = Swxx - xb * Swx;
-                        const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                        const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
+                        const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_], l2 = E45[a_], h2 = E45[b_];
+                        const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                        const T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                        const T isw = RT::rcp(Sw), xb = Swx * isw;
+                        const T sxx = Swxx - xb * Swx;
+                        const T isxx = sxx > vsmlsq ? RT::rcp(sxx) : (T)0;
+                        const T yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
                         A[i][s] = yb + b * (x[s] - xb);
-                        const double rss = (Syy - yb * Sy) - b * sxy;
-                        Gs[i][s] = sqrt64(rss * isw) * (isxx != 0.0 ? K.kc[2 * i + 1] : K.kc[2 * i]);
+                        const T rss = (Syy - yb * Sy) - b * sxy;
+                        Gs[i][s] = RT::sqrt0(rss * isw) * (isxx != (T)0 ? (T)K.kc[2 * i + 1] : (T)K.kc[2 * i]);
                     }
                 }
 #pragma unroll
                 for (int s = 0; s < C; s++) {
-                    const double sp = pick_span_w(Gs[0][s], Gs[1][s], Gs[2][s], KW);
-                    const double smo = interp_spans(sp, A[0][s], A[1][s], A[2][s]);
-                    const double r = y[s] - smo;
+                    const T sp = pick_span_t<T>(Gs[0][s], Gs[1][s], Gs[2][s], K.bass, K.bexp);
+                    const T smo = interp_spans_t<T>(sp, A[0][s], A[1][s], A[2][s]);
+                    const T r = y[s] - smo;
                     chi2 += w[s] * r * r;
                 }
             } else {
                 // ---- CV pass 1: one span at a time; smooths parked in tensor memory
-                double r0[C], r1[C], r2[C];
-                double m_isw[C], m_xb[C], m_g[C];
-                const double* E4 = reinterpret_cast<const double*>(E45);
+                T r0[C], r1[C], r2[C];
+                T m_isw[C], m_xb[C], m_g[C];
+                const T* E4 = reinterpret_cast<const T*>(E45);
                 int amin = 0x7fffffff;
 #pragma unroll
                 for (int i = 0; i < 3; i++) {
                     int wi[2 * C];
                     tmem_fetch_words<2 * C>(tmem + T_W0 + 2 * C * i, wi);
-                    double Ai[C], q_isw[C], q_xb[C], q_g[C];
+                    T Ai[C], q_isw[C], q_xb[C], q_g[C];
 #pragma unroll
                     for (int s = 0; s < C; s++) {
                         const int a_ = wi[s], b_ = wi[C + s];
-                        const double2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_];
-                        const double lxy = E4[a_], hxy = E4[b_];
-                        const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                        const double Sxy = hxy - lxy;
-                        const double isw = rcp64(Sw), xb = Swx * isw;
-                        const double sxx = Swxx - xb * Swx;
-                        const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                        const double dx = x[s] - xb, g = isxx * dx;
+                        const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_];
+                        const T lxy = E4[a_], hxy = E4[b_];
+                        const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                        const T Sxy = hxy - lxy;
+                        const T isw = RT::rcp(Sw), xb = Swx * isw;
+                        const T sxx = Swxx - xb * Swx;
+                        const T isxx = sxx > vsmlsq ? RT::rcp(sxx) : (T)0;
+                        const T dx = x[s] - xb, g = isxx * dx;
                         q_isw[s] = isw; q_xb[s] = xb; q_g[s] = g;
                         Ai[s] = Sy * isw + (Sxy - xb * Sy) * g;
-                        const double a = 1.0 - w[s] * (isw + dx * g);
-                        const double r = fabs(y[s] - Ai[s]) * rcp64(a);
+                        const T a = (T)1 - w[s] * (isw + dx * g);
+                        const T r = (T)fabs(y[s] - Ai[s]) * RT::rcp(a);
                         if (i == 0) r0[s] = r; else if (i == 1) r1[s] = r; else r2[s] = r;
-                        amin = min(amin, __double2hiint(a));
+                        amin = min(amin, RT::hi_word(a));
                     }
-                    tmem_park<C>(tmem + T_A0 + 2 * C * i, Ai);
-                    if (i == 0) { tmem_park<C>(tmem + T_ISW, q_isw); tmem_park<C>(tmem + T_XB, q_xb); tmem_park<C>(tmem + T_G0, q_g); }
+                    TA::park(tmem + T_A0 + PC * i, Ai);
+                    if (i == 0) { TA::park(tmem + T_ISW, q_isw); TA::park(tmem + T_XB, q_xb); TA::park(tmem + T_G0, q_g); }
                     if (i == 1) {
 #pragma unroll
                         for (int s = 0; s < C; s++) { m_isw[s] = q_isw[s]; m_xb[s] = q_xb[s]; m_g[s] = q_g[s]; }
                     }
                 }
-                tmem_park<C>(tmem + T_Y, y);
+                TA::park(tmem + T_Y, y);
                 // ---- pass 2: the three residuals smoothed at the midrange span
-                double za[C], zb[C], zc[C], zd[C], ze[C], zf[C];
+                T za[C], zb[C], zc[C], zd[C], ze[C], zf[C];
 #pragma unroll
                 for (int s = 0; s < C; s++) {
                     za[s] = w[s] * r0[s]; zb[s] = za[s] * x[s];
@@ -494,7 +587,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
                 const PairScan qs1 = pair_scan_begin<C>(zc, zd, s_tot[1], warp, lane, mk);
                 const PairScan qs2 = pair_scan_begin<C>(ze, zf, s_tot[2], warp, lane, mk);
                 // a <= 0 (or below the smallest normal): the residual carries (R23) -> generic path
-                const bool carry = __syncthreads_or(amin < 0x00100000);                    // BAR 4 (primary arrays dead)
+                const bool carry = __syncthreads_or(amin < RT::TINY);                    // BAR 4 (primary arrays dead)
                 if (carry) {
                     if (tid == 0) {
                         const unsigned pos = atomicAdd(p.defer_count, 1u);
@@ -505,69 +598,70 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
                     }
                     bad = true;
                 } else {
-                    pair_scan_finish<G, C>(qs0, za, zb, s_tot[0], E01, warp, tid);
-                    pair_scan_finish<G, C>(qs1, zc, zd, s_tot[1], E23, warp, tid);
-                    pair_scan_finish<G, C>(qs2, ze, zf, s_tot[2], E45, warp, tid);
+                    pair_scan_finish<G, C, T>(qs0, za, zb, s_tot[0], E01, warp, tid);
+                    pair_scan_finish<G, C, T>(qs1, zc, zd, s_tot[1], E23, warp, tid);
+                    pair_scan_finish<G, C, T>(qs2, ze, zf, s_tot[2], E45, warp, tid);
                     __syncthreads();                                                        // BAR 5
                     int w1i[2 * C];
                     tmem_fetch_words<2 * C>(tmem + T_W1, w1i);
-                    auto mid_load = [&](const double2* Ez, double (&out)[C]) {
+                    auto mid_load = [&](const T2* Ez, T (&out)[C]) {
 #pragma unroll
                         for (int s = 0; s < C; s++) {
-                            const double2 l = Ez[w1i[s]], h = Ez[w1i[C + s]];
-                            const double Sz = h.x - l.x, Sxz = h.y - l.y;
+                            const T2 l = Ez[w1i[s]], h = Ez[w1i[C + s]];
+                            const T Sz = h.x - l.x, Sxz = h.y - l.y;
                             out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
                         }
                     };
-                    double sp[C];
+                    T sp[C];
                     {
-                        double R0[C], R1[C], R2[C];
+                        T R0[C], R1[C], R2[C];
                         mid_load(E01, R0); mid_load(E23, R1); mid_load(E45, R2);
 #pragma unroll
-                        for (int s = 0; s < C; s++) sp[s] = pick_span_w(R0[s], R1[s], R2[s], KW);
+                        for (int s = 0; s < C; s++) sp[s] = pick_span_t<T>(R0[s], R1[s], R2[s], K.bass, K.bexp);
                     }
                     // ---- the spans smoothed at midrange
 #pragma unroll
                     for (int s = 0; s < C; s++) { za[s] = w[s] * sp[s]; zb[s] = za[s] * x[s]; }
                     const PairScan ss0 = pair_scan_begin<C>(za, zb, s_tot[0], warp, lane, mk);
                     __syncthreads();                                                        // BAR 6 (residual arrays dead)
-                    pair_scan_finish<G, C>(ss0, za, zb, s_tot[0], E01, warp, tid);
+                    pair_scan_finish<G, C, T>(ss0, za, zb, s_tot[0], E01, warp, tid);
                     __syncthreads();                                                        // BAR 7
-                    double B[C];
+                    T B[C];
                     mid_load(E01, B);
                     tmem_wait_st();
                     {
-                        double a0[C], a1[C], a2[C];
-                        tmem_fetch<C>(tmem + T_A0, a0); tmem_fetch<C>(tmem + T_A1, a1); tmem_fetch<C>(tmem + T_A2, a2);
+                        T a0[C], a1[C], a2[C];
+                        TA::fetch(tmem + T_A0, a0); TA::fetch(tmem + T_A1, a1); TA::fetch(tmem + T_A2, a2);
 #pragma unroll
-                        for (int s = 0; s < C; s++) B[s] = interp_spans(B[s], a0[s], a1[s], a2[s]);
+                        for (int s = 0; s < C; s++) B[s] = interp_spans_t<T>(B[s], a0[s], a1[s], a2[s]);
                     }
                     // ---- final tweeter smooth
 #pragma unroll
                     for (int s = 0; s < C; s++) { zc[s] = w[s] * B[s]; zd[s] = zc[s] * x[s]; }
                     const PairScan fs0 = pair_scan_begin<C>(zc, zd, s_tot[1], warp, lane, mk);
                     __syncthreads();                                                        // BAR 8
-                    pair_scan_finish<G, C>(fs0, zc, zd, s_tot[1], E23, warp, tid);
+                    pair_scan_finish<G, C, T>(fs0, zc, zd, s_tot[1], E23, warp, tid);
                     __syncthreads();                                                        // BAR 9
                     int w0i[2 * C];
                     tmem_fetch_words<2 * C>(tmem + T_W0, w0i);
-                    double t_isw[C], t_xb[C], t_g[C], yy[C];
-                    tmem_fetch<C>(tmem + T_ISW, t_isw); tmem_fetch<C>(tmem + T_XB, t_xb); tmem_fetch<C>(tmem + T_G0, t_g);
-                    tmem_fetch<C>(tmem + T_Y, yy);
+                    T t_isw[C], t_xb[C], t_g[C], yy[C];
+                    TA::fetch(tmem + T_ISW, t_isw); TA::fetch(tmem + T_XB, t_xb); TA::fetch(tmem + T_G0, t_g);
+                    TA::fetch(tmem + T_Y, yy);
 #pragma unroll
                     for (int s = 0; s < C; s++) {
-                        const double2 l = E23[w0i[s]], h = E23[w0i[C + s]];
-                        const double Sz = h.x - l.x, Sxz = h.y - l.y;
-                        const double smo = Sz * t_isw[s] + (Sxz - t_xb[s] * Sz) * t_g[s];
-                        const double r = yy[s] - smo;
+                        const T2 l = E23[w0i[s]], h = E23[w0i[C + s]];
+                        const T Sz = h.x - l.x, Sxz = h.y - l.y;
+                        const T smo = Sz * t_isw[s] + (Sxz - t_xb[s] * Sz) * t_g[s];
+                        const T r = yy[s] - smo;
                         chi2 += w[s] * r * r;
                     }
                 }
             }
             if (!bad) {
+                double chi2d = (double)chi2;
 #pragma unroll
-                for (int d = 16; d > 0; d >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, d);
-                if (lane == 0) s_red[warp] = chi2;
+                for (int d = 16; d > 0; d >>= 1) chi2d += __shfl_xor_sync(0xffffffffu, chi2d, d);
+                if (lane == 0) s_red[warp] = chi2d;
                 __syncthreads();                                                            // BAR 10
                 double c2 = 0.0;
 #pragma unroll
@@ -595,13 +689,13 @@ __global__ void __launch_bounds__(GroupCfg<G, C>::NT, GroupCfg<G, C>::MINB) grou
     }
 }
 
-template <int G, int C, bool GV>
+template <int G, int C, bool GV, typename T = double>
 inline ss_status_t launch_group_variant(const EvalParams& p, int64_t n_items, cudaStream_t stream)
 {
-    const size_t smem = group_smem_bytes<G, C, GV>();
-    if (cudaFuncSetAttribute(group_kernel<G, C, GV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    const size_t smem = group_smem_bytes<G, C, GV, T>();
+    if (cudaFuncSetAttribute(group_kernel<G, C, GV, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return SS_ERR_CUDA;
-    group_kernel<G, C, GV><<<(unsigned)n_items, GroupCfg<G, C>::NT, smem, stream>>>(p);
+    group_kernel<G, C, GV, T><<<(unsigned)n_items, GroupCfg<G, C, T>::NT, smem, stream>>>(p);
     return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
 }
 

@@ -1,25 +1,32 @@
-// ss_group_tu.cu -- instantiations of the G-warps-per-eval kernel (ss_group_kernel.cuh).  Compiled six times by
-// _build.py: -DSS_TU_GV=0|1 x -DSS_TU_G=4|8|16, three kernels each (C = 3, 4, 5 points per thread).
+// ss_group_tu.cu -- instantiations of the G-warps-per-eval kernel (ss_group_kernel.cuh).  Compiled twelve times by
+// _build.py: -DSS_TU_GV=0|1 x -DSS_TU_G=4|8|16 x -DSS_TU_F32=0|1 (smoother scalar double / float), three kernels each
+// (C = 3, 4, 5 points per thread).
 #include "ss_group_kernel.cuh"
 #include "ss_launch.h"
 
 #ifndef SS_TU_GV
-#error "compile with -DSS_TU_GV=0|1 -DSS_TU_G=4|8|16"
+#error "compile with -DSS_TU_GV=0|1 -DSS_TU_G=4|8|16 -DSS_TU_F32=0|1"
 #endif
 
 namespace ss {
 
 #define SS_CAT2(a, b, c, d) a##b##c##d
 #define SS_CAT(a, b, c, d) SS_CAT2(a, b, c, d)
+#if SS_TU_F32
+#define SS_TU_FN SS_CAT(launch_group_f32_tu_, SS_TU_GV, _, SS_TU_G)
+typedef float tu_real;
+#else
 #define SS_TU_FN SS_CAT(launch_group_tu_, SS_TU_GV, _, SS_TU_G)
+typedef double tu_real;
+#endif
 
 ss_status_t SS_TU_FN(const EvalParams& p, int c, int64_t n_items, cudaStream_t stream)
 {
     constexpr bool GV = SS_TU_GV != 0;
     switch (c) {
-        case 3: return launch_group_variant<SS_TU_G, 3, GV>(p, n_items, stream);
-        case 4: return launch_group_variant<SS_TU_G, 4, GV>(p, n_items, stream);
-        case 5: return launch_group_variant<SS_TU_G, 5, GV>(p, n_items, stream);
+        case 3: return launch_group_variant<SS_TU_G, 3, GV, tu_real>(p, n_items, stream);
+        case 4: return launch_group_variant<SS_TU_G, 4, GV, tu_real>(p, n_items, stream);
+        case 5: return launch_group_variant<SS_TU_G, 5, GV, tu_real>(p, n_items, stream);
         default: return SS_ERR_UNSUPPORTED;
     }
 }

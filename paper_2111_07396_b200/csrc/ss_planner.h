@@ -24,6 +24,8 @@ inline int path_for_n(int64_t n, int /*mode*/)
     return SS_PATH_STAGE;
 }
 
+constexpr int GROUP_VARIANT_F32 = 1000;   // added to the group variant id: smoother scalar float (mixed precision)
+
 // Cluster-path kernel variant: R CTAs of 512 threads x C points per thread, the smallest capacity R*512*C >= n
 // (3,072 ... 40,960).  id = R*8 + C.
 inline int cluster_variant_for_n(int n)
