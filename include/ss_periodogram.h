@@ -98,6 +98,12 @@ typedef struct {
                                sort, the centring and the accumulation of the prefix sums stay in fp64 (the
                                permutation is therefore the fp64 one).  Shorter and longer light curves are served in
                                fp64.  Periodogram values then agree with the fp64 result to about 1e-4 absolute.       */
+    int shared_times;       /* 1 = every object of the catalog has the SAME time stamps in the same order (one field
+                               observed together).  The fold and the sort are then done once per
+                               frequency for 4 objects at a time (objects of n <= SS_WARP_MAX_N; longer ones are
+                               served as usual).  Checked on the device unless skip_validation is set: a catalog
+                               whose time arrays differ is SS_ERR_INVALID_ARG.  Results equal those of
+                               shared_times = 0 to rounding (same arithmetic, same order).                   */
     unsigned int defer_capacity; /* test hook: entries of the list through which the warp-per-eval kernels hand
                                tied / undecidable evals to the generic kernel, per tile (0 = 2^20).  When it
                                overflows the call repeats itself on the CTA-per-eval kernels; results never

@@ -38,7 +38,7 @@ class Options(C.Structure):
     _fields_ = [("alpha", C.c_double), ("span", C.c_double), ("iper", C.c_int),
                 ("force_path", C.c_int), ("stream", C.c_void_p), ("workspace_cap", C.c_size_t),
                 ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int),
-                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("precision", C.c_int), ("defer_capacity", C.c_uint)]
+                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("precision", C.c_int), ("shared_times", C.c_int), ("defer_capacity", C.c_uint)]
 
 
 class Plan(C.Structure):

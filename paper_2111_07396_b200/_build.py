@@ -34,7 +34,9 @@ def units():
         if base == "ss_warp_tu":
             for gv in (0, 1):
                 for grp in (0, 1, 2):
-                    u.append((f"{base}_{gv}_{grp}.o", src, [f"-DSS_TU_GV={gv}", f"-DSS_TU_GROUP={grp}"]))
+                    for sh in (0, 1):
+                        u.append((f"{base}_{gv}_{grp}_{sh}.o", src,
+                                  [f"-DSS_TU_GV={gv}", f"-DSS_TU_GROUP={grp}", f"-DSS_TU_SHARED={sh}"]))
         elif base == "ss_group_tu":
             for gv in (0, 1):
                 for g in (4, 8, 16):

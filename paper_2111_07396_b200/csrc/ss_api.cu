@@ -219,6 +219,19 @@ __global__ void __launch_bounds__(PREP_T) prep_kernel(const double* __restrict__
     }
 }
 
+// shared_times = 1: every object must carry the time stamps of the first one (flag |= 2 otherwise)
+__global__ void shared_times_check_kernel(const double* __restrict__ times, const ObjRec* recs,
+                                          const int64_t* __restrict__ raw_off, int n_recs, int* flag)
+{
+    const int ri = blockIdx.x + 1;
+    if (ri >= n_recs) return;
+    const int n = recs[ri].n;
+    const int64_t a = raw_off[0], b = raw_off[ri];
+    int bad = recs[0].n != n;
+    for (int j = threadIdx.x; j < n && !bad; j += blockDim.x) bad |= times[a + j] != times[b + j];
+    if (bad) atomicOr(flag, 2);
+}
+
 // Fold one tile's partial maxima into the running best of each object (O8: first maximum wins).
 __global__ void fold_best_kernel(const ObjRec* recs, const int32_t* list, int n_list, int chunks,
                                  int chunks_total, int chunk_base, const double* part_val,
@@ -564,10 +577,16 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         g_launches++;
         SS_CUDA(cudaGetLastError());
     }
+    if (o.shared_times && !o.skip_validation && recs.size() > 1) {
+        if (recs.size() != (size_t)n_obj) return fail(SS_ERR_INVALID_ARG, "shared_times: every object needs the same number of points");
+        shared_times_check_kernel<<<(unsigned)recs.size() - 1, 256, 0, stream>>>(times, d_recs, d_raw_off, (int)recs.size(), flag);
+        g_launches++;
+    }
     if (!o.skip_validation) {
         int h_flag = 0;
         SS_CUDA(cudaMemcpyAsync(&h_flag, flag, sizeof(int), cudaMemcpyDeviceToHost, stream));
         SS_CUDA(cudaStreamSynchronize(stream));
+        if (h_flag & 2) return fail(SS_ERR_INVALID_ARG, "shared_times is set but the objects' time stamps differ");
         if (h_flag) return fail(SS_ERR_INVALID_ARG, "non-finite time/magnitude/error or error <= 0 in the catalog");
     }
     return SS_OK;
@@ -605,7 +624,8 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         p.counter = counters + (next_counter % n_counters);
         p.stage = stage; p.stage_stride = stage_stride;
         p.defer_entries = defer_entries; p.defer_count = defer_count; p.defer_capacity = defer_capacity;
-        const int64_t n_items = (int64_t)p.n_list * cpo;
+        const bool shared = opt.shared_times && c.path == SS_PATH_WARP;      // one fold + sort per group of objects
+        const int64_t n_items = (shared ? ((int64_t)p.n_list + SHARED_TIMES_M - 1) / SHARED_TIMES_M : (int64_t)p.n_list) * cpo;
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (opt.profile) {
@@ -620,7 +640,8 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         }
         if (ev0) SS_CUDA(cudaEventRecord(ev0, stream));
         if (c.path == SS_PATH_WARP) {
-            ss_status_t st = launch_warp_kernel(p, c.variant, n_items, stream);
+            ss_status_t st = shared ? launch_warp_shared_kernel(p, c.variant, n_items, stream)
+                                    : launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (c.path == SS_PATH_CLUSTER) {
             ss_status_t st = launch_cluster_kernel(p, c.variant, n_items, stream);

@@ -71,6 +71,20 @@ ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items
          : g == 1 ? launch_warp_tu_0_1(p, variant, n_items, stream) : launch_warp_tu_0_2(p, variant, n_items, stream);
 }
 
+#define SS_DECL(gv, g) ss_status_t launch_warp_shared_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
+SS_DECL(0, 0) SS_DECL(0, 1) SS_DECL(0, 2) SS_DECL(1, 0) SS_DECL(1, 1) SS_DECL(1, 2)
+#undef SS_DECL
+
+ss_status_t launch_warp_shared_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
+{
+    const int c = variant / 8, g = c <= 4 ? 0 : (c <= 6 ? 1 : 2);
+    if (p.mode == 1)
+        return g == 0 ? launch_warp_shared_tu_1_0(p, variant, n_items, stream)
+             : g == 1 ? launch_warp_shared_tu_1_1(p, variant, n_items, stream) : launch_warp_shared_tu_1_2(p, variant, n_items, stream);
+    return g == 0 ? launch_warp_shared_tu_0_0(p, variant, n_items, stream)
+         : g == 1 ? launch_warp_shared_tu_0_1(p, variant, n_items, stream) : launch_warp_shared_tu_0_2(p, variant, n_items, stream);
+}
+
 // ---- group-kernel translation units (ss_group_tu.cu) -------------------------------------------------
 #define SS_DECL(gv, g) ss_status_t launch_group_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
 SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)

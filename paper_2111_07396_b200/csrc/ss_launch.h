@@ -12,6 +12,9 @@ namespace ss {
 // warp-per-eval kernels (ss_warp_kernel.cuh); variant = warp_variant_for_n(n)
 ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 
+// the same for a catalog with one shared time sampling (ss_warp_shared.cuh): n_items = groups of SHARED_M objects x chunks
+ss_status_t launch_warp_shared_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
+
 // G-warps-per-eval kernels (ss_group_kernel.cuh); variant = group_variant_for_n(n)
 ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 

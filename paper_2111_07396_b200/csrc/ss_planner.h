@@ -24,6 +24,7 @@ inline int path_for_n(int64_t n, int /*mode*/)
     return SS_PATH_STAGE;
 }
 
+constexpr int SHARED_TIMES_M = 4;          // objects per work item of the shared-time-sampling warp kernel
 constexpr int GROUP_VARIANT_F32 = 1000;   // added to the group variant id: smoother scalar float (mixed precision)
 
 // Cluster-path kernel variant: R CTAs of 512 threads x C points per thread, the smallest capacity R*512*C >= n

@@ -1,36 +1,44 @@
-// ss_warp_tu.cu -- instantiations of the warp-per-eval kernel.  Compiled six times by _build.py:
+// ss_warp_tu.cu -- instantiations of the warp-per-eval kernel.  Compiled twelve times by _build.py:
 //   -DSS_TU_GV=0|1 (cross-validation / generalized validation)  x  -DSS_TU_GROUP=0|1|2 (C = 2..4 / 5..6 / 7..8)
-// so that the 20 kernels build in parallel.
+//   x -DSS_TU_SHARED=0|1 (warp_kernel / warp_shared_kernel, the shared-time-sampling variant)
+// so that the 40 kernels build in parallel.
 #include "ss_launch.h"
 #include "ss_warp_kernel.cuh"
+#include "ss_warp_shared.cuh"
 
 #ifndef SS_TU_GV
-#error "compile with -DSS_TU_GV=0|1 -DSS_TU_GROUP=0|1|2"
+#error "compile with -DSS_TU_GV=0|1 -DSS_TU_GROUP=0|1|2 -DSS_TU_SHARED=0|1"
 #endif
 
 namespace ss {
 
 #define SS_CAT2(a, b, c, d) a##b##c##d
 #define SS_CAT(a, b, c, d) SS_CAT2(a, b, c, d)
+#if SS_TU_SHARED
+#define SS_TU_FN SS_CAT(launch_warp_shared_tu_, SS_TU_GV, _, SS_TU_GROUP)
+#define SS_TU_LAUNCH launch_warp_shared_variant
+#else
 #define SS_TU_FN SS_CAT(launch_warp_tu_, SS_TU_GV, _, SS_TU_GROUP)
+#define SS_TU_LAUNCH launch_warp_variant
+#endif
 
 ss_status_t SS_TU_FN(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
 {
     constexpr bool GV = SS_TU_GV != 0;
     switch (variant) {
 #if SS_TU_GROUP == 0
-        case 2 * 8 + 2: return launch_warp_variant<2, 2, GV>(p, n_items, stream);
-        case 3 * 8 + 2: return launch_warp_variant<3, 2, GV>(p, n_items, stream);
-        case 4 * 8 + 2: return launch_warp_variant<4, 2, GV>(p, n_items, stream);
-        case 4 * 8 + 3: return launch_warp_variant<4, 3, GV>(p, n_items, stream);
+        case 2 * 8 + 2: return SS_TU_LAUNCH<2, 2, GV>(p, n_items, stream);
+        case 3 * 8 + 2: return SS_TU_LAUNCH<3, 2, GV>(p, n_items, stream);
+        case 4 * 8 + 2: return SS_TU_LAUNCH<4, 2, GV>(p, n_items, stream);
+        case 4 * 8 + 3: return SS_TU_LAUNCH<4, 3, GV>(p, n_items, stream);
 #elif SS_TU_GROUP == 1
-        case 5 * 8 + 3: return launch_warp_variant<5, 3, GV>(p, n_items, stream);
-        case 5 * 8 + 4: return launch_warp_variant<5, 4, GV>(p, n_items, stream);
-        case 6 * 8 + 4: return launch_warp_variant<6, 4, GV>(p, n_items, stream);
-        case 6 * 8 + 5: return launch_warp_variant<6, 5, GV>(p, n_items, stream);
+        case 5 * 8 + 3: return SS_TU_LAUNCH<5, 3, GV>(p, n_items, stream);
+        case 5 * 8 + 4: return SS_TU_LAUNCH<5, 4, GV>(p, n_items, stream);
+        case 6 * 8 + 4: return SS_TU_LAUNCH<6, 4, GV>(p, n_items, stream);
+        case 6 * 8 + 5: return SS_TU_LAUNCH<6, 5, GV>(p, n_items, stream);
 #else
-        case 7 * 8 + 5: return launch_warp_variant<7, 5, GV>(p, n_items, stream);
-        case 8 * 8 + 6: return launch_warp_variant<8, 6, GV>(p, n_items, stream);
+        case 7 * 8 + 5: return SS_TU_LAUNCH<7, 5, GV>(p, n_items, stream);
+        case 8 * 8 + 6: return SS_TU_LAUNCH<8, 6, GV>(p, n_items, stream);
 #endif
         default: return SS_ERR_UNSUPPORTED;
     }

@@ -846,3 +846,57 @@ def test_mixed_precision_mode(ss, mode):
     assert np.abs(mix2.pgram - ref2).max() <= MIXED_ATOL, np.abs(mix2.pgram - ref2).max()
     with pytest.raises(ss.SSError):
         ss.periodogram(t2, y2, e2, off2, 0.01, 10.0, 61, mode, precision=7)
+
+
+# ------------------------------------------------------------------ shared time sampling
+def _shared_times_catalog(n_objects, n, seed, dup=False):
+    rng = np.random.default_rng(seed)
+    t = np.sort(rng.integers(0, 30, size=n) + rng.uniform(0.0, 0.33, size=n))
+    if dup:
+        t[7] = t[6]
+    T, Y, E = [], [], []
+    for i in range(n_objects):
+        P = np.exp(rng.uniform(np.log(0.1), np.log(2.0)))
+        e = rng.uniform(0.02, 0.1, size=n)
+        T.append(t); E.append(e)
+        Y.append(15 + rng.uniform(0.1, 1.0) * np.sin(2 * np.pi * t / P + i) + rng.normal(0, 1.0, size=n) * e)
+    off = np.arange(n_objects + 1, dtype=np.int64) * n
+    return np.concatenate(T), np.concatenate(Y), np.concatenate(E), off
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+def test_shared_time_sampling_reuses_the_sort(ss, mode):
+    """shared_times = 1: one fold + sort per frequency for 4 objects at a time.  Equal to the ordinary call (to rounding),
+    parity with the oracle, for group sizes that do not divide the catalog, every points-per-lane variant, a shared
+    sampling with a duplicated time stamp (every eval handed over) and tied phases at f = 1 / d on integer times;
+    a catalog whose time stamps differ is refused."""
+    for n_objects, n, dup in ((37, 150, False), (9, 64, False), (6, 200, False), (5, 256, False), (7, 90, True)):
+        t, y, e, off = _shared_times_catalog(n_objects, n, seed=n, dup=dup)
+        plain = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode)
+        shared = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode, shared_times=1)
+        # the same arithmetic in the same order; the compiler is free to contract a*b+c differently in the two kernels
+        # (seen: 4e-16 on P for the 8-points-per-lane variant), so equality is to rounding, not to the bit
+        assert np.allclose(shared.pgram, plain.pgram, rtol=1e-13, atol=1e-14), (n_objects, n)
+        assert np.array_equal(shared.best_index, plain.best_index) and np.array_equal(shared.best_freq, plain.best_freq)
+        if n_objects == 9:
+            cat = ss_inputs.Catalog("shared", t, y, e, off, 0.5, 24.0, 131, np.full(n_objects, np.nan))
+            ref, _, _ = oracle.periodogram(t, y, e, off, 0.5, 24.0, 131, mode=mode, variant=oracle.DEFINITION)
+            check_parity(cat, shared.pgram, ref, mode, label="shared times")
+            check_best(ref, shared.best_index, shared.best_freq, cat)
+    # integer-day times: at f = 1 every phase ties (handed over for the whole group)
+    n = 40
+    t1 = np.arange(n, dtype=np.float64) + 0.25 * (np.arange(n) % 3 == 0)
+    rng = np.random.default_rng(3)
+    T = np.tile(t1, 5); Y = 15 + rng.normal(0, 0.1, size=5 * n); E = np.full(5 * n, 0.05)
+    off = np.arange(6, dtype=np.int64) * n
+    plain = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode)
+    shared = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode, shared_times=1)
+    assert np.allclose(shared.pgram, plain.pgram, rtol=1e-13, atol=1e-14) and np.array_equal(shared.best_index, plain.best_index)
+    # not actually shared
+    T2 = T.copy(); T2[3 * n + 5] += 1e-9
+    with pytest.raises(ss.SSError) as ei:
+        ss.periodogram(T2, Y, E, off, 0.25, 1.25, 4, mode, shared_times=1)
+    assert ei.value.status == ss.SS_ERR_INVALID_ARG
+    ragged = np.array([0, n, 2 * n, 3 * n, 4 * n, 5 * n - 1], dtype=np.int64)
+    with pytest.raises(ss.SSError):
+        ss.periodogram(T[:5 * n - 1], Y[:5 * n - 1], E[:5 * n - 1], ragged, 0.25, 1.25, 4, mode, shared_times=1)
