@@ -22,8 +22,8 @@
  * best_index = -1.  chi0 == 0 (constant magnitudes) gives a row of zeros and best_index = 0.
  * Argmax ties resolve to the lowest index.
  *
- * Errors: every entry point returns SS_OK or an error code; on error the outputs are unspecified
- * (never partially trusted) and ss_last_error() (thread-local) describes the failure.  The library
+ * Errors: every entry point returns SS_OK or an error code.  Argument errors are found before any output is
+ * touched (outputs untouched); on SS_ERR_CUDA / SS_ERR_OUT_OF_MEMORY the outputs are unspecified and ss_last_error() (thread-local) describes the failure.  The library
  * never frees or retains caller memory.
  */
 #ifndef SS_PERIODOGRAM_H
@@ -104,6 +104,17 @@ typedef struct {
                                served as usual).  Checked on the device unless skip_validation is set: a catalog
                                whose time arrays differ is SS_ERR_INVALID_ARG.  Results equal those of
                                shared_times = 0 to rounding (same arithmetic, same order).                   */
+    void *workspace;        /* device entry points: a DEVICE buffer of workspace_bytes bytes (256-byte aligned) the library
+                               carves its workspace from instead of allocating; ss_workspace_bytes() is an upper bound
+                               of the need.  NULL = the library allocates (and keeps the buffer for the next call).     */
+    size_t workspace_bytes;
+    const int64_t *offsets_host; /* device entry points: a HOST copy of `offsets`.  The batch planner needs the objects'
+                               sizes on the host; without this copy the call reads `offsets` back and waits for it.    */
+    int async_mode;         /* ss_periodogram_ex only.  1 = enqueue everything on opt->stream and return without waiting;
+                               needs skip_validation = 1 and offsets_host (nothing is then read back).  The call is
+                               completed -- status, profile counters, the hand-over overflow fallback, release of the
+                               workspace -- by ss_synchronize(), or implicitly by this thread's next library call.
+                               Inputs, outputs and a caller-supplied workspace must stay valid until then.               */
     unsigned int defer_capacity; /* test hook: entries of the list through which the warp-per-eval kernels hand
                                tied / undecidable evals to the generic kernel, per tile (0 = 2^20).  When it
                                overflows the call repeats itself on the CTA-per-eval kernels; results never
@@ -127,7 +138,8 @@ ss_status_t ss_periodogram(const double *times, const double *mags, const double
                            double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
                            double *pgram_out, double *best_freq_out, int64_t *best_index_out);
 
-/* Same with options; enqueues on opt->stream and returns after that stream's work has completed. */
+/* Same with options; enqueues on opt->stream and returns after that stream's work has completed -- unless
+ * opt->async_mode is set (see ss_options_t), in which case it returns as soon as the work is enqueued. */
 ss_status_t ss_periodogram_ex(const double *times, const double *mags, const double *errs,
                               const int64_t *offsets, int64_t n_objects,
                               double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
@@ -146,6 +158,11 @@ ss_status_t ss_periodogram_host(const double *times, const double *mags, const d
                                 double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
                                 double *pgram_out, double *best_freq_out, int64_t *best_index_out,
                                 const ss_options_t *opt);
+
+/* Completes this thread's pending asynchronous ss_periodogram_ex call (opt->async_mode): waits for its stream, repeats
+ * the call on the CTA-per-eval kernels if the hand-over list overflowed, releases the workspace and returns the call's
+ * final status.  SS_OK when nothing is pending. */
+ss_status_t ss_synchronize(void);
 
 /* ------------------------------------------------------------------ top-k peaks */
 

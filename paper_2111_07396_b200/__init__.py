@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "libss_b200.so")
 EXPORTS = ["ss_default_options", "ss_periodogram", "ss_periodogram_ex", "ss_periodogram_host",
            "ss_plan", "ss_workspace_bytes", "ss_paper_footprint_bytes", "ss_paper_batches",
            "ss_path_for_n", "ss_debug_eval", "ss_microbench", "ss_last_launch_count", "ss_last_kernel_ms", "ss_last_kernel_count",
-           "ss_last_error", "ss_version", "ss_release_workspace", "ss_periodogram_peaks", "ss_periodogram_peaks_host"]
+           "ss_last_error", "ss_version", "ss_release_workspace", "ss_periodogram_peaks", "ss_periodogram_peaks_host", "ss_synchronize"]
 
 
 class SSError(RuntimeError):
@@ -38,7 +38,8 @@ class Options(C.Structure):
     _fields_ = [("alpha", C.c_double), ("span", C.c_double), ("iper", C.c_int),
                 ("force_path", C.c_int), ("stream", C.c_void_p), ("workspace_cap", C.c_size_t),
                 ("freq_tile", C.c_int64), ("skip_validation", C.c_int), ("profile", C.c_int),
-                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("precision", C.c_int), ("shared_times", C.c_int), ("defer_capacity", C.c_uint)]
+                ("k_begin", C.c_int64), ("k_count", C.c_int64), ("precision", C.c_int), ("shared_times", C.c_int), ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+                ("offsets_host", C.c_void_p), ("async_mode", C.c_int), ("defer_capacity", C.c_uint)]
 
 
 class Plan(C.Structure):
@@ -107,6 +108,11 @@ def default_options(**kw) -> Options:
             raise TypeError(f"unknown option {k}")
         setattr(o, k, v)
     return o
+
+
+def synchronize() -> None:
+    """Complete this thread's pending asynchronous call (ss_synchronize)."""
+    _check(load().ss_synchronize())
 
 
 def release_workspace() -> None:

@@ -5,6 +5,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <memory>
 #include <string>
 #include <vector>
 
@@ -130,6 +131,7 @@ struct DevicePool {
     }
 };
 static thread_local DevicePool g_pool;
+static_assert(sizeof(ObjRec) == OBJREC_BYTES, "planner's record size");
 
 // ------------------------------------------------------------------------------------------------
 // P0 prep: tt = t - min t, w = e^-2, ybar_w, chi0; yc = y - ybar_w.
@@ -354,6 +356,7 @@ struct Engine {
     // device workspace
     char* ws = nullptr;
     size_t ws_bytes = 0;
+    bool ws_owned = true;              // false: the caller's buffer (opt.workspace)
     double *tt = nullptr, *yc = nullptr, *w = nullptr;
     ObjRec* d_recs = nullptr;
     int32_t* d_list = nullptr;
@@ -384,7 +387,7 @@ struct Engine {
         // pooled buffers must be idle when they go back (already true unless the call is failing)
         if (ws) cudaStreamSynchronize(stream);
         for (auto& e : prof) { g_pool.event_back(true, e.first); g_pool.event_back(true, e.second); }
-        g_pool.release(ws, ws_bytes);
+        if (ws_owned) g_pool.release(ws, ws_bytes);
     }
     // After the stream is synchronised: did the deferred list overflow?
     bool defer_overflowed()
@@ -427,6 +430,17 @@ static ss_status_t validate_scalars(int64_t n_objects, double f_min, double f_ma
     if (o.k_begin < 0 || o.k_count < 0 || o.k_begin >= n_freq || o.k_begin + o.k_count > n_freq)
         return fail(SS_ERR_INVALID_ARG, "k_begin/k_count outside the grid");
     return SS_OK;
+}
+
+// SM count of the current device; the B200's when no device is visible (planner queries on a CPU-only box)
+static int device_sm_count()
+{
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+        cudaGetLastError();
+        return DEFAULT_SM_COUNT;
+    }
+    return sms;
 }
 
 static bool has_listing_options(const ss_options_t& o) { return o.iper == 2 || o.span > 0.0; }
@@ -479,7 +493,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         SS_CUDA(cudaMemGetInfo(&fr, &tot));
         cap = (size_t)(0.75 * (double)fr);   // the paper's beta
     }
-    PlanInput pin{total, max_n, n_obj, k_n, md, cap, host_tiles ? 1 : 0, want_pgram ? 1 : 0, o.freq_tile};
+    PlanInput pin{total, max_n, n_obj, k_n, md, cap, host_tiles ? 1 : 0, want_pgram ? 1 : 0, o.freq_tile, sm_count, defer_capacity};
     ss_status_t st = make_plan(pin, &plan);
     if (st != SS_OK) return fail(st, "workspace cap %zu B too small for the smallest tile", cap);
 
@@ -525,41 +539,41 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
         tiles[t] = std::move(cls);
     }
 
-    // ---- workspace
+    // ---- workspace: one buffer, carved by the planner's layout function with this catalog's actual counts
     const bool need_stage = max_n > BLOCK_MAX_N || o.force_path == SS_PATH_STAGE;
-    stage_stride = need_stage ? BLOCK_SLOTS * block_slot_len(max_n) : 0;
-    const int stage_ctas = sm_count * 2;
     const int64_t cpo = chunks_per_object(plan.objects_per_tile, plan.freq_per_tile);
-    n_counters = 64;
-    size_t b = 0;
-    auto carve = [&](size_t bytes) { size_t o_ = b; b += align_up(bytes); return o_; };
-    size_t o_tt = carve(8 * (size_t)padded_total), o_yc = carve(8 * (size_t)padded_total), o_w = carve(8 * (size_t)padded_total);
-    size_t o_recs = carve(sizeof(ObjRec) * std::max<size_t>(recs.size(), 1));
-    size_t o_raw = carve(8 * std::max<size_t>(recs.size(), 1));
-    size_t o_list = carve(4 * std::max<size_t>(all_lists.size(), 1));
-    size_t o_deg = carve(8 * std::max<size_t>(degenerate.size(), 1));
-    size_t o_bv = carve(8 * (size_t)std::max<int64_t>(n_obj, 1)), o_bi = carve(8 * (size_t)std::max<int64_t>(n_obj, 1));
-    size_t o_pv = carve(8 * std::max<size_t>(recs.size(), 1) * (size_t)cpo), o_pi = carve(8 * std::max<size_t>(recs.size(), 1) * (size_t)cpo);
-    size_t o_cnt = carve(4 * (size_t)n_counters), o_flag = carve(64);
-    size_t o_stage = carve(need_stage ? 8 * (size_t)stage_stride * (size_t)stage_ctas : 0);
-    size_t o_de = carve(8 * (size_t)defer_capacity), o_dv = carve(8 * (size_t)defer_capacity), o_dc = carve(64);
-    size_t o_dmax = carve(8 * (size_t)std::max<int64_t>(n_obj, 1)), o_dmin = carve(8 * (size_t)std::max<int64_t>(n_obj, 1));
-    size_t o_extra = carve(extra_bytes);
-    ws_bytes = b;
-    if (ws_bytes > cap + (64 << 20))
+    WsCounts wc;
+    wc.padded_points = padded_total; wc.n_recs = (int64_t)recs.size(); wc.n_list = (int64_t)all_lists.size();
+    wc.n_degenerate = (int64_t)degenerate.size(); wc.n_objects = n_obj;
+    wc.partial_slots = (int64_t)std::max<size_t>(recs.size(), 1) * cpo;
+    wc.max_n = max_n; wc.stage = need_stage ? 1 : 0; wc.sm_count = sm_count; wc.defer_capacity = defer_capacity;
+    const WsLayout L = ws_layout(wc);
+    stage_stride = L.stage_stride;
+    n_counters = WS_COUNTERS;
+    ws_bytes = L.bytes + ws_align(extra_bytes);
+    if (ws_bytes > cap)
         return fail(SS_ERR_OUT_OF_MEMORY, "workspace %zu B exceeds the cap %zu B", ws_bytes, cap);
-    SS_CUDA(g_pool.acquire(ws_bytes, &ws));
-    tt = (double*)(ws + o_tt); yc = (double*)(ws + o_yc); w = (double*)(ws + o_w);
-    d_raw_off = (int64_t*)(ws + o_raw);
-    d_recs = (ObjRec*)(ws + o_recs); d_list = (int32_t*)(ws + o_list); d_degen = (int64_t*)(ws + o_deg);
-    best_val = (double*)(ws + o_bv); best_idx = (int64_t*)(ws + o_bi);
-    part_val = (double*)(ws + o_pv); part_idx = (int64_t*)(ws + o_pi);
-    counters = (unsigned int*)(ws + o_cnt); flag = (int*)(ws + o_flag);
-    stage = need_stage ? (double*)(ws + o_stage) : nullptr;
-    defer_entries = (unsigned long long*)(ws + o_de); defer_val = (double*)(ws + o_dv);
-    defer_count = (unsigned int*)(ws + o_dc);
-    dmax = (unsigned long long*)(ws + o_dmax); dmin = (unsigned long long*)(ws + o_dmin);
-    extra = ws + o_extra;
+    if (o.workspace) {
+        // caller-supplied device workspace (ss_workspace_bytes() is an upper bound of the need)
+        if (o.workspace_bytes < ws_bytes)
+            return fail(SS_ERR_OUT_OF_MEMORY, "caller workspace of %zu B is smaller than the %zu B this call needs", o.workspace_bytes, ws_bytes);
+        if (((uintptr_t)o.workspace & 255) != 0) return fail(SS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+        ws = (char*)o.workspace;
+        ws_owned = false;
+    } else {
+        SS_CUDA(g_pool.acquire(ws_bytes, &ws));
+    }
+    tt = (double*)(ws + L.tt); yc = (double*)(ws + L.yc); w = (double*)(ws + L.w);
+    d_raw_off = (int64_t*)(ws + L.raw);
+    d_recs = (ObjRec*)(ws + L.recs); d_list = (int32_t*)(ws + L.list); d_degen = (int64_t*)(ws + L.degen);
+    best_val = (double*)(ws + L.best_val); best_idx = (int64_t*)(ws + L.best_idx);
+    part_val = (double*)(ws + L.part_val); part_idx = (int64_t*)(ws + L.part_idx);
+    counters = (unsigned int*)(ws + L.counters); flag = (int*)(ws + L.flag);
+    stage = need_stage ? (double*)(ws + L.stage) : nullptr;
+    defer_entries = (unsigned long long*)(ws + L.defer_entries); defer_val = (double*)(ws + L.defer_val);
+    defer_count = (unsigned int*)(ws + L.defer_count);
+    dmax = (unsigned long long*)(ws + L.dmax); dmin = (unsigned long long*)(ws + L.dmin);
+    extra = ws + L.bytes;
 
     if (!recs.empty()) SS_CUDA(cudaMemcpyAsync(d_recs, recs.data(), sizeof(ObjRec) * recs.size(), cudaMemcpyHostToDevice, stream));
     if (!recs.empty()) SS_CUDA(cudaMemcpyAsync(d_raw_off, raw_off.data(), 8 * raw_off.size(), cudaMemcpyHostToDevice, stream));
@@ -726,7 +740,7 @@ void ss_default_options(ss_options_t* opt)
 }
 
 const char* ss_last_error(void) { return g_err.c_str(); }
-void ss_release_workspace(void) { g_pool.release_all(); }
+void ss_release_workspace(void) { ss_synchronize(); g_pool.release_all(); }
 int ss_version(void) { return SS_VERSION; }
 int64_t ss_last_launch_count(void) { return g_launches; }
 double ss_last_kernel_ms(void) { return g_kernel_ms; }
@@ -744,7 +758,7 @@ ss_status_t ss_plan(int64_t n_points_total, int64_t max_n, int64_t n_objects, in
     if (!plan_out) return fail(SS_ERR_INVALID_ARG, "plan_out is null");
     if (n_points_total < 0 || max_n < 0 || n_objects < 0 || n_freq < 1)
         return fail(SS_ERR_INVALID_ARG, "negative size");
-    PlanInput in{n_points_total, max_n, n_objects, n_freq, (int)mode, cap_bytes, host_tiles, want_pgram, 0};
+    PlanInput in{n_points_total, max_n, n_objects, n_freq, (int)mode, cap_bytes, host_tiles, want_pgram, 0, device_sm_count()};
     ss_status_t st = make_plan(in, plan_out);
     if (st != SS_OK) return fail(st, "cap %zu B too small", cap_bytes);
     return SS_OK;
@@ -754,17 +768,19 @@ size_t ss_workspace_bytes(int64_t n_points_total, int64_t max_n, int64_t n_objec
                           ss_mode_t mode)
 {
     ss_plan_t pl{};
-    PlanInput in{n_points_total, max_n, n_objects, n_freq, (int)mode, (size_t)-1, 0, 0, 0};
+    PlanInput in{n_points_total, max_n, n_objects, n_freq, (int)mode, (size_t)-1, 0, 0, 0, device_sm_count()};
     if (make_plan(in, &pl) != SS_OK) return 0;
     return pl.total_bytes;
 }
 
 // One pass over the catalog with DEVICE pointers.  *overflow: the warp path's hand-over list was too short (the
 // outputs are then incomplete; the caller repeats the pass on the CTA path once this pass's buffers are back in the pool).
+// pending != null (asynchronous call): the engine is handed back still running instead of being waited for.
 static ss_status_t periodogram_device(const double* times, const double* mags, const double* errs,
                                       const int64_t* offsets, int64_t n_objects, double f_min, double f_max,
                                       int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
-                                      int64_t* best_index_out, const ss_options_t& o, bool* overflow)
+                                      int64_t* best_index_out, const ss_options_t& o, bool* overflow,
+                                      std::unique_ptr<Engine>* pending)
 {
     *overflow = false;
     ss_status_t st = validate_scalars(n_objects, f_min, f_max, n_freq, (int)mode, o);
@@ -772,29 +788,73 @@ static ss_status_t periodogram_device(const double* times, const double* mags, c
     if (!offsets) return fail(SS_ERR_INVALID_ARG, "offsets is null");
     if (n_objects == 0) return SS_OK;
     cudaStream_t stream = (cudaStream_t)o.stream;
-    std::vector<int64_t> off((size_t)n_objects + 1);
-    SS_CUDA(cudaMemcpyAsync(off.data(), offsets, 8 * ((size_t)n_objects + 1), cudaMemcpyDeviceToHost, stream));
-    SS_CUDA(cudaStreamSynchronize(stream));
+    std::vector<int64_t> off_copy;
+    const int64_t* off = o.offsets_host;
+    if (!off) {
+        off_copy.resize((size_t)n_objects + 1);
+        SS_CUDA(cudaMemcpyAsync(off_copy.data(), offsets, 8 * ((size_t)n_objects + 1), cudaMemcpyDeviceToHost, stream));
+        SS_CUDA(cudaStreamSynchronize(stream));
+        off = off_copy.data();
+    }
     if (off[n_objects] > 0 && (!times || !mags || !errs)) return fail(SS_ERR_INVALID_ARG, "times/mags/errs is null");
-    Engine eng;
-    st = eng.setup(times, mags, errs, off.data(), n_objects, f_min, f_max, n_freq, (int)mode, o, false,
-                   pgram_out != nullptr, 0);
+    std::unique_ptr<Engine> eng(new Engine);
+    st = eng->setup(times, mags, errs, off, n_objects, f_min, f_max, n_freq, (int)mode, o, false,
+                    pgram_out != nullptr, 0);
     if (st != SS_OK) return st;
     // device output: the caller's array is written directly; frequency tiles only bound the
     // partial-argmax rows
-    for (int ot = 0; ot < (int)eng.tiles.size(); ot++) {
-        for (int64_t ft = 0; ft < eng.plan.n_freq_tiles; ft++) {
-            int64_t k0 = eng.k_lo + ft * eng.plan.freq_per_tile, k1 = std::min(eng.k_lo + eng.k_n, k0 + eng.plan.freq_per_tile);
-            st = eng.run_tile(ot, k0, k1, (int)ft, pgram_out, eng.k_n, 0, eng.k_lo);
+    for (int ot = 0; ot < (int)eng->tiles.size(); ot++) {
+        for (int64_t ft = 0; ft < eng->plan.n_freq_tiles; ft++) {
+            int64_t k0 = eng->k_lo + ft * eng->plan.freq_per_tile, k1 = std::min(eng->k_lo + eng->k_n, k0 + eng->plan.freq_per_tile);
+            st = eng->run_tile(ot, k0, k1, (int)ft, pgram_out, eng->k_n, 0, eng->k_lo);
             if (st != SS_OK) return st;
         }
     }
-    st = eng.finish(best_freq_out, best_index_out);
+    st = eng->finish(best_freq_out, best_index_out);
     if (st != SS_OK) return st;
+    if (pending) {
+        *pending = std::move(eng);
+        return SS_OK;
+    }
     SS_CUDA(cudaStreamSynchronize(stream));
-    eng.collect_profile();
-    *overflow = eng.defer_overflowed();
+    eng->collect_profile();
+    *overflow = eng->defer_overflowed();
     return SS_OK;
+}
+
+// this thread's asynchronous call in flight (ss_options_t::async_mode)
+struct PendingCall {
+    std::unique_ptr<Engine> eng;
+    const double *times, *mags, *errs;
+    const int64_t* offsets;
+    std::vector<int64_t> offsets_host;
+    int64_t n_objects, n_freq;
+    double f_min, f_max;
+    ss_mode_t mode;
+    double *pgram_out, *best_freq_out;
+    int64_t* best_index_out;
+    ss_options_t o;
+};
+static thread_local std::unique_ptr<PendingCall> g_pending;
+
+ss_status_t ss_synchronize(void)
+{
+    if (!g_pending) return SS_OK;
+    std::unique_ptr<PendingCall> pc = std::move(g_pending);
+    if (cudaStreamSynchronize((cudaStream_t)pc->o.stream) != cudaSuccess) {
+        pc->eng.reset();
+        return fail(SS_ERR_CUDA, "asynchronous call failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    pc->eng->collect_profile();
+    const bool overflow = pc->eng->defer_overflowed();
+    pc->eng.reset();                                  // workspace back to the pool
+    if (!overflow) return SS_OK;
+    if (pc->o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "hand-over list overflow on the CTA path");
+    ss_options_t o = pc->o;
+    o.force_path = SS_PATH_BLOCK; o.async_mode = 0; o.offsets_host = pc->offsets_host.data();
+    bool again = false;
+    return periodogram_device(pc->times, pc->mags, pc->errs, pc->offsets, pc->n_objects, pc->f_min, pc->f_max, pc->n_freq,
+                              pc->mode, pc->pgram_out, pc->best_freq_out, pc->best_index_out, o, &again, nullptr);
 }
 
 ss_status_t ss_periodogram_ex(const double* times, const double* mags, const double* errs,
@@ -802,19 +862,35 @@ ss_status_t ss_periodogram_ex(const double* times, const double* mags, const dou
                               int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
                               int64_t* best_index_out, const ss_options_t* opt_in)
 {
+    ss_status_t st = ss_synchronize();
+    if (st != SS_OK) return st;
     g_launches = 0;
     ss_options_t o;
     if (opt_in) o = *opt_in; else ss_default_options(&o);
     bool overflow = false;
-    ss_status_t st = periodogram_device(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
-                                        best_freq_out, best_index_out, o, &overflow);
+    if (o.async_mode) {
+        if (!o.skip_validation || !o.offsets_host)
+            return fail(SS_ERR_INVALID_ARG, "async_mode needs skip_validation = 1 and offsets_host");
+        std::unique_ptr<PendingCall> pc(new PendingCall);
+        st = periodogram_device(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                                best_freq_out, best_index_out, o, &overflow, &pc->eng);
+        if (st != SS_OK || !pc->eng) return st;
+        pc->times = times; pc->mags = mags; pc->errs = errs; pc->offsets = offsets;
+        pc->offsets_host.assign(o.offsets_host, o.offsets_host + n_objects + 1);
+        pc->n_objects = n_objects; pc->n_freq = n_freq; pc->f_min = f_min; pc->f_max = f_max; pc->mode = mode;
+        pc->pgram_out = pgram_out; pc->best_freq_out = best_freq_out; pc->best_index_out = best_index_out; pc->o = o;
+        g_pending = std::move(pc);
+        return SS_OK;
+    }
+    st = periodogram_device(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+                            best_freq_out, best_index_out, o, &overflow, nullptr);
     if (st == SS_OK && overflow) {
         // more ties than the hand-over list holds (e.g. integer time stamps at a commensurate frequency in every
         // object): serve everything with the generic kernel instead.  The first pass's buffers are already released.
         if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "hand-over list overflow on the CTA path");
         o.force_path = SS_PATH_BLOCK;
         st = periodogram_device(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
-                                best_freq_out, best_index_out, o, &overflow);
+                                best_freq_out, best_index_out, o, &overflow, nullptr);
     }
     return st;
 }
@@ -923,11 +999,14 @@ ss_status_t ss_periodogram_host(const double* times, const double* mags, const d
                                 int64_t n_freq, ss_mode_t mode, double* pgram_out, double* best_freq_out,
                                 int64_t* best_index_out, const ss_options_t* opt_in)
 {
+    ss_status_t st = ss_synchronize();
+    if (st != SS_OK) return st;
     g_launches = 0;
     ss_options_t o;
     if (opt_in) o = *opt_in; else ss_default_options(&o);
+    if (o.async_mode) return fail(SS_ERR_INVALID_ARG, "async_mode applies to ss_periodogram_ex only");
     bool overflow = false;
-    ss_status_t st = periodogram_host(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
+    st = periodogram_host(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out,
                                       best_freq_out, best_index_out, o, &overflow);
     if (st == SS_OK && overflow) {
         if (o.force_path == SS_PATH_BLOCK) return fail(SS_ERR_CUDA, "hand-over list overflow on the CTA path");

@@ -88,7 +88,7 @@ inline int64_t paper_batches(int64_t n_t, int64_t n_f, int mode, double device_g
 }
 
 constexpr unsigned int DEFER_CAPACITY = 1u << 20;   // evals the warp path may defer per tile
-constexpr int STAGE_CTAS = 148 * 2;      // persistent CTAs of the STAGE path (2 per SM)
+constexpr int DEFAULT_SM_COUNT = 148;    // B200; the planner queries take the device's own count when there is one
 constexpr int64_t MIN_CHUNK = 1;          // smallest frequency chunk a work item may cover
 
 // Work items are (object, frequency chunk).  Launches are per path class (about a tenth of a ragged catalog
@@ -116,7 +116,57 @@ struct PlanInput {
     int host_tiles;    // output tiles are device buffers copied back (x2, double buffered)
     int want_pgram;
     int64_t force_freq_tile;
+    int sm_count = DEFAULT_SM_COUNT;
+    unsigned int defer_capacity = DEFER_CAPACITY;
 };
+
+// ---- the one workspace buffer of a call, carved: the SAME function sizes it for the planner queries (worst-case
+// counts: every object kept, every object padded by one element) and for the engine (actual counts), so what
+// ss_workspace_bytes() reports is an upper bound of what a call allocates or takes from the caller.
+inline size_t ws_align(size_t x) { return (x + 255) / 256 * 256; }
+struct WsCounts {
+    int64_t padded_points = 0;   // elements of tt / yc / w (objects padded to an even length)
+    int64_t n_recs = 0;          // objects with n >= 5
+    int64_t n_list = 0;          // entries of the class lists
+    int64_t n_degenerate = 0;    // objects with n < 5
+    int64_t n_objects = 0;
+    int64_t partial_slots = 0;   // (object, chunk) partial-argmax slots of one tile
+    int64_t max_n = 0;
+    int stage = 0;               // the global staging scratch is needed
+    int sm_count = DEFAULT_SM_COUNT;
+    unsigned int defer_capacity = DEFER_CAPACITY;
+};
+struct WsLayout {
+    size_t tt, yc, w, recs, raw, list, degen, best_val, best_idx, part_val, part_idx, counters, flag, stage, defer_entries,
+        defer_val, defer_count, dmax, dmin, bytes;
+    int64_t stage_stride;
+    int stage_ctas;
+};
+constexpr int WS_COUNTERS = 64;
+constexpr size_t OBJREC_BYTES = 64;
+inline WsLayout ws_layout(const WsCounts& c)
+{
+    WsLayout L{};
+    size_t b = 0;
+    auto carve = [&](size_t bytes) { size_t o = b; b += ws_align(bytes); return o; };
+    auto atl1 = [](int64_t v) { return (size_t)(v > 1 ? v : 1); };
+    L.tt = carve(8 * (size_t)c.padded_points); L.yc = carve(8 * (size_t)c.padded_points); L.w = carve(8 * (size_t)c.padded_points);
+    L.recs = carve(OBJREC_BYTES * atl1(c.n_recs));
+    L.raw = carve(8 * atl1(c.n_recs));
+    L.list = carve(4 * atl1(c.n_list));
+    L.degen = carve(8 * atl1(c.n_degenerate));
+    L.best_val = carve(8 * atl1(c.n_objects)); L.best_idx = carve(8 * atl1(c.n_objects));
+    L.part_val = carve(8 * atl1(c.partial_slots)); L.part_idx = carve(8 * atl1(c.partial_slots));
+    L.counters = carve(4 * (size_t)WS_COUNTERS); L.flag = carve(64);
+    L.stage_ctas = c.sm_count * 2;
+    L.stage_stride = c.stage ? 14 * ((((int64_t)c.max_n + 2)) & ~(int64_t)1) : 0;     // BLOCK_SLOTS * block_slot_len(max_n)
+    L.stage = carve(c.stage ? 8 * (size_t)L.stage_stride * (size_t)L.stage_ctas : 0);
+    L.defer_entries = carve(8 * (size_t)c.defer_capacity); L.defer_val = carve(8 * (size_t)c.defer_capacity);
+    L.defer_count = carve(64);
+    L.dmax = carve(8 * atl1(c.n_objects)); L.dmin = carve(8 * atl1(c.n_objects));
+    L.bytes = b;
+    return L;
+}
 
 // New footprint model: nothing is materialised at N_t*N_f.  Fixed = catalog copy (tt, yc, w) +
 // records + lists + partial argmax rows; stage = scratch of the STAGE path; tiles = periodogram
@@ -125,16 +175,19 @@ inline ss_status_t make_plan(const PlanInput& in, ss_plan_t* out)
 {
     ss_plan_t p{};
     const int64_t nobj = in.n_objects > 0 ? in.n_objects : 0;
-    // tt, yc, w (+ the raw catalog copy when the caller's arrays live on the host), records, lists,
-    // running best (value, index), offsets, scheduler counters
-    p.fixed_bytes = (size_t)((in.host_tiles ? 6 : 3) * 8 * in.n_points_total)
-                  + (size_t)(nobj * (64 + 4 + 8 + 8 + 8 + 16 + 24 + 8)) + 8192   // + even-length padding of tt/yc/w, raw offsets
-                  + (size_t)DEFER_CAPACITY * 16;   // warp-path hand-over list (entries + values)
-    if (in.max_n > BLOCK_MAX_N)
-        p.stage_bytes = (size_t)STAGE_CTAS * (size_t)(14 * 8 * (((in.max_n + 2) + 1) & ~(int64_t)1));
+    // worst-case counts of the workspace (every object kept and padded by one element), partial rows added below;
+    // + the raw catalog copy and the best-frequency outputs when the caller's arrays live on the host
+    WsCounts wc;
+    wc.padded_points = in.n_points_total + nobj; wc.n_recs = nobj; wc.n_list = nobj; wc.n_degenerate = nobj;
+    wc.n_objects = nobj; wc.partial_slots = 0; wc.max_n = in.max_n; wc.stage = in.max_n > BLOCK_MAX_N;
+    wc.sm_count = in.sm_count > 0 ? in.sm_count : DEFAULT_SM_COUNT; wc.defer_capacity = in.defer_capacity;
+    const WsLayout wl = ws_layout(wc);
+    p.stage_bytes = wc.stage ? ws_align(8 * (size_t)wl.stage_stride * (size_t)wl.stage_ctas) : 0;
+    p.fixed_bytes = wl.bytes - p.stage_bytes - 2 * ws_align(8)      // the two empty partial arrays come back with partials()
+                  + (in.host_tiles ? 3 * ws_align(8 * (size_t)in.n_points_total) + 2 * ws_align(8 * (size_t)(nobj > 1 ? nobj : 1)) + 256 : 0);
     // partial argmax rows of ONE tile: 16 B per (object, chunk); folded into the running best per
     // object after every tile, so they never scale with the number of tiles
-    auto partials = [&](int64_t f, int64_t o) { return (size_t)16 * (size_t)o * (size_t)chunks_per_object(o, f); };
+    auto partials = [&](int64_t f, int64_t o) { return 2 * ws_align((size_t)8 * (size_t)(nobj > 1 ? nobj : 1) * (size_t)chunks_per_object(o, f)); };
     const size_t base = p.fixed_bytes + p.stage_bytes;
     int64_t fpt = in.n_freq, opt = nobj > 0 ? nobj : 1;
     if (in.force_freq_tile > 0 && in.force_freq_tile < fpt) fpt = in.force_freq_tile;

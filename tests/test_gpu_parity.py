@@ -900,3 +900,58 @@ def test_shared_time_sampling_reuses_the_sort(ss, mode):
     ragged = np.array([0, n, 2 * n, 3 * n, 4 * n, 5 * n - 1], dtype=np.int64)
     with pytest.raises(ss.SSError):
         ss.periodogram(T[:5 * n - 1], Y[:5 * n - 1], E[:5 * n - 1], ragged, 0.25, 1.25, 4, mode, shared_times=1)
+
+
+# ------------------------------------------------------------------ boundary: asynchronous call, caller workspace
+def test_async_call_and_caller_workspace(ss):
+    """ss_periodogram_ex with async_mode = 1 (skip_validation + offsets_host: nothing is read back) returns before the
+    work is done and ss_synchronize() completes it; a caller-supplied device workspace of ss_workspace_bytes() bytes
+    is enough for the call (and nothing is allocated), a smaller one is refused; both give the bits of the plain call."""
+    import torch
+    a = ss_inputs.config3(n_objects=300, n_freq=2000)
+    b = ss_inputs.config4(n_objects=3, n_freq=2000)
+    times = np.concatenate([a.times, b.times]); mags = np.concatenate([a.mags, b.mags]); errs = np.concatenate([a.errs, b.errs])
+    offsets = np.concatenate([a.offsets, a.offsets[-1] + b.offsets[1:]])
+    n_obj, n_freq = len(offsets) - 1, 2000
+    dev = torch.device("cuda")
+    t = torch.as_tensor(times, device=dev); y = torch.as_tensor(mags, device=dev)
+    e = torch.as_tensor(errs, device=dev); off = torch.as_tensor(offsets, device=dev)
+    ref_pg = torch.empty((n_obj, n_freq), dtype=torch.float64, device=dev)
+    ref_bi = torch.empty(n_obj, dtype=torch.int64, device=dev)
+    ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, ref_pg, None, ref_bi)
+    # asynchronous on a side stream
+    s = torch.cuda.Stream()
+    pg = torch.zeros((n_obj, n_freq), dtype=torch.float64, device=dev)
+    bi = torch.zeros(n_obj, dtype=torch.int64, device=dev)
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        o = ss.default_options(async_mode=1, skip_validation=1, offsets_host=offsets.ctypes.data)
+        ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, pg, None, bi, o)
+        returned_early = not s.query()          # ~0.1 s of kernels are still running when the call is back
+    ss.synchronize()
+    assert s.query()
+    assert torch.equal(pg, ref_pg) and torch.equal(bi, ref_bi)
+    assert returned_early
+    with pytest.raises(ss.SSError):             # async needs skip_validation and offsets_host
+        ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, pg, None, bi, ss.default_options(async_mode=1))
+    # the next call completes a pending one implicitly
+    pg.zero_()
+    ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, pg, None, bi,
+                      ss.default_options(async_mode=1, skip_validation=1, offsets_host=offsets.ctypes.data))
+    res = ss.periodogram(times[:a.offsets[5]], mags[:a.offsets[5]], errs[:a.offsets[5]], a.offsets[:6], 0.5, 24.0, 50, CV)
+    assert res.pgram.shape == (5, 50) and torch.equal(pg, ref_pg)
+    # caller-supplied workspace
+    need = ss.workspace_bytes(len(times), int(np.diff(offsets).max()), n_obj, n_freq, CV)
+    ws = torch.empty(need, dtype=torch.uint8, device=dev)
+    assert ws.data_ptr() % 256 == 0
+    ss.release_workspace()
+    free0 = torch.cuda.mem_get_info()[0]
+    pg.zero_()
+    ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, pg, None, bi,
+                      ss.default_options(workspace=ws.data_ptr(), workspace_bytes=need))
+    assert torch.equal(pg, ref_pg) and torch.equal(bi, ref_bi)
+    assert torch.cuda.mem_get_info()[0] == free0            # the library allocated nothing
+    with pytest.raises(ss.SSError) as ei:
+        ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, pg, None, bi,
+                          ss.default_options(workspace=ws.data_ptr(), workspace_bytes=1 << 20))
+    assert ei.value.status == ss.SS_ERR_OUT_OF_MEMORY
