@@ -60,8 +60,12 @@ def _deps():
                   + [os.path.abspath(__file__)])
 
 
+EXTRA = os.environ.get("SS_EXTRA_NVCC_FLAGS", "").split()      # experiments (-D switches); part of the source hash
+
+
 def source_hash() -> str:
     h = hashlib.sha256()
+    h.update(" ".join(EXTRA).encode())
     for d in _deps():
         h.update(os.path.basename(d).encode())
         with open(d, "rb") as f:
@@ -87,7 +91,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         obj, src, defs = u
         out = os.path.join(OBJ, obj)
         t0 = time.time()
-        r = subprocess.run([NVCC] + FLAGS + extra + defs + ["-c", "-o", out, src], capture_output=True, text=True)
+        r = subprocess.run([NVCC] + FLAGS + EXTRA + extra + defs + ["-c", "-o", out, src], capture_output=True, text=True)
         if os.environ.get("SS_BUILD_TIMES"):
             sys.stderr.write(f"{obj}: {time.time() - t0:.1f} s\n")
         return out, r

@@ -27,6 +27,9 @@ ss_status_t SS_TU_FN(const EvalParams& p, int c, int64_t n_items, cudaStream_t s
         case 3: return launch_group_variant<SS_TU_G, 3, GV, tu_real>(p, n_items, stream);
         case 4: return launch_group_variant<SS_TU_G, 4, GV, tu_real>(p, n_items, stream);
         case 5: return launch_group_variant<SS_TU_G, 5, GV, tu_real>(p, n_items, stream);
+#if SS_TU_G != 16
+        case 6: return launch_group_variant<SS_TU_G, 6, GV, tu_real>(p, n_items, stream);
+#endif
         default: return SS_ERR_UNSUPPORTED;
     }
 }

@@ -37,14 +37,17 @@ inline int cluster_variant_for_n(int n)
     return 16 * 8 + 5;
 }
 
-// Group-path kernel variant of an object: G warps x C points per thread, the smallest capacity 32*G*C >= n
-// (384, 512, 640, 768, 1024, 1280, 1536, 2048, 2560).  id = G*8 + C.
+// Group-path kernel variant of an object: G warps x C points per thread, the smallest capacity 32*G*C >= n among
+// (4,3) 384, (4,4) 512, (4,5) 640, (4,6) 768, (8,4) 1,024, (8,5) 1,280, (8,6) 1,536, (16,4) 2,048, (16,5) 2,560.  More
+// points per thread beat more warps per eval (measured: (8,6) 2.37e10 point-evals/s at n = 1,400 where (16,3) gave
+// 1.85e10; (4,6) 2.49e10 at n = 700 where (8,3) gave 2.23e10); C = 6 is what tensor memory allows at 16 warps per SM
+// (20C columns per warp <= 128).  id = G*8 + C.
 inline int group_variant_for_n(int n)
 {
     const int gs[3] = {4, 8, 16};
     for (int gi = 0; gi < 3; gi++)
-        for (int c = 3; c <= 5; c++)
-            if (32 * gs[gi] * c >= n) return gs[gi] * 8 + c;
+        for (int c = 3; c <= (gs[gi] == 16 ? 5 : 6); c++)
+            if (32 * gs[gi] * c >= n && !(gs[gi] > 4 && c == 3)) return gs[gi] * 8 + c;
     return 16 * 8 + 5;
 }
 

@@ -24,9 +24,11 @@ namespace ss {
 template <int C, bool GV> struct WarpCfg {
     // each shape chosen by measurement on config 3:
     //   GV: C <= 4: 4 warps x 5 CTAs (20 warps/SM,  96 registers);  C >= 5: 4 x 3 (12 warps, 168)
-    //   CV: C <= 6: 8 warps x 2 CTAs (16 warps/SM, 128 registers);  C = 7: 4 x 3 (12 warps, 168);  C = 8: 8 x 1 (255)
-    static constexpr int WPC = GV ? 4 : (C == 7 ? 4 : 8);
-    static constexpr int MINB = GV ? (C <= 4 ? 5 : 3) : (C <= 6 ? 2 : (C == 7 ? 3 : 1));
+    //   CV: C <= 3: 4 x 5 (20 warps/SM, 96 registers: +2.6 % over 16 warps, round 2);  C = 4..6: 8 warps x 2 CTAs (16 warps/SM,
+    //       128 registers; tensor memory -- 18C columns per warp -- allows no more for C >= 4);  C = 7: 4 x 3 (12 warps, 168);
+    //       C = 8: 8 x 1 (255)
+    static constexpr int WPC = GV ? 4 : ((C == 7 || C <= 3) ? 4 : 8);
+    static constexpr int MINB = GV ? (C <= 4 ? 5 : 3) : (C <= 3 ? 5 : (C <= 6 ? 2 : (C == 7 ? 3 : 1)));
 };
 constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lanes + the total)
 constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0

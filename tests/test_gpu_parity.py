@@ -684,10 +684,10 @@ def test_config4_full_size_sampled(ss, mode):
 @pytest.mark.parametrize("mode", [CV, GV])
 def test_group_kernel_every_variant(ss, mode):
     """The G-warps-per-eval kernels, one object per (G, C) variant at both ends of its range of n (capacities 384,
-    512, 640, 768, 1,024, 1,280, 1,536, 2,048, 2,560 points; the path ends at n = 2,055), heteroscedastic errors,
+    512, 640, 768 = 4 warps x 6 points, 1,024, 1,280, 1,536 = 8 x 6, 2,048, 2,560 points; the path ends at n = 2,055), heteroscedastic errors,
     config-4 time sampling; against the definition oracle, best index included."""
     rng = np.random.default_rng(515)
-    ns = [257, 384, 385, 512, 513, 640, 641, 768, 769, 1024, 1025, 1280, 1281, 1536, 1537, 2048, 2049, 2055]
+    ns = [257, 384, 385, 512, 513, 640, 641, 700, 768, 769, 1024, 1025, 1280, 1281, 1400, 1536, 1537, 2048, 2049, 2055]
     T, Y, E = [], [], []
     for i, n in enumerate(ns):
         assert ss.path_for_n(n) == ss.PATH_GROUP
@@ -832,7 +832,7 @@ def test_mixed_precision_mode(ss, mode):
     assert match.mean() >= 0.93, match.mean()
     # every (G, C) variant of the float kernel
     rng = np.random.default_rng(717)
-    ns = [257, 384, 500, 640, 768, 1000, 1280, 1536, 2048, 2055]
+    ns = [257, 384, 500, 640, 700, 768, 1000, 1280, 1400, 1536, 2048, 2055]
     T, Y, E = [], [], []
     for i, n in enumerate(ns):
         t = np.sort(rng.integers(0, 1200, size=n) + rng.uniform(0.0, 0.3, size=n))
