@@ -112,9 +112,12 @@ template <int G, int C, typename T = double> struct GroupCfg {
     static constexpr int MINB = G == 4 ? 4 : (G == 8 ? 2 : 1);      // 16 warps per SM at 128 registers
     static constexpr int IDX_BITS = NP <= 512 ? 9 : (NP <= 1024 ? 10 : (NP <= 2048 ? 11 : 12));
     static constexpr unsigned IDX_MASK = (1u << IDX_BITS) - 1u;
-    // tensor memory per warp: 7 parked arrays (A0, A1, A2, tweeter isw / xbar / g, y) + 6C window indices
+    // tensor memory per warp: 7 parked arrays (A0, A1, A2, tweeter isw / xbar / g, y) + per span C words of window
+    // ends, two 16-bit element indices each (padded to an even count)
     static constexpr uint32_t PCOLS = TmemArr<T, C>::COLS;
-    static constexpr uint32_t TCOLS_WARP = 7 * PCOLS + 6 * C;
+    static constexpr int CE = (C + 1) & ~1;
+    static constexpr uint32_t TCOLS_WARP = 7 * PCOLS + 3 * CE;
+    static_assert(C * (NT + 1) < 65536, "window-end indices are packed two to a word");
     static constexpr uint32_t TCOLS_NEED = TCOLS_WARP * (G / 4);
     static constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
     static_assert(TCOLS * MINB <= 512, "tensor memory over-subscribed");
@@ -287,8 +290,13 @@ struct GroupConst {
 // ------------------------------------------------------------------------------------------------
 // Kernel: one CTA = one work item (object, chunk of frequencies), evals one after the other.
 // ------------------------------------------------------------------------------------------------
+// Resident CTAs per SM: 16 warps at 128 registers, except 4-warp CTAs with 6 or 7 points per thread, which spill less and
+// run faster at 12 warps / 168 registers (measured, CV: +11..13 % at C = 7, +2..3 % at C = 6; GV: C = 7 only)
+template <int G, int C, bool GV, typename T>
+constexpr int group_minb() { return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 : GroupCfg<G, C, T>::MINB; }
+
 template <int G, int C, bool GV, typename T = double>
-__global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB) group_kernel(const EvalParams p)
+__global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>()) group_kernel(const EvalParams p)
 {
     using Cfg = GroupCfg<G, C, T>;
     using RT = Real<T>;
@@ -372,20 +380,22 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB
     // tensor-memory columns (32-bit words) of this warp
     constexpr uint32_t PC = Cfg::PCOLS;
     constexpr uint32_t T_A0 = 0, T_A1 = PC, T_A2 = 2 * PC, T_ISW = 3 * PC, T_XB = 4 * PC, T_G0 = 5 * PC, T_Y = 6 * PC;
-    constexpr uint32_t T_W0 = 7 * PC, T_W1 = T_W0 + 2 * C, T_W2 = T_W0 + 4 * C;      // window indices (lo[C], hi[C]) per span
+    constexpr int CE = Cfg::CE;
+    constexpr uint32_t T_W0 = 7 * PC, T_W1 = T_W0 + CE, T_W2 = T_W0 + 2 * CE;      // window ends per span: lo | hi << 16
     {
-        int w0[2 * C], w1[2 * C], w2[2 * C];
+        int w0[C], w1[C], w2[C];
+        auto at = [&](int pos) { return (pos % C) * ROW + pos / C; };
 #pragma unroll
         for (int s = 0; s < C; s++) {
             const int j = tid * C + s;
             const int l0 = window_lo(j, ibw0, K0, n), l1 = window_lo(j, ibw1, K1, n), l2 = window_lo(j, ibw2, K2, n);
-            w0[s] = ((l0 % C) * ROW + l0 / C); w0[C + s] = (((l0 + K0) % C) * ROW + (l0 + K0) / C);
-            w1[s] = ((l1 % C) * ROW + l1 / C); w1[C + s] = (((l1 + K1) % C) * ROW + (l1 + K1) / C);
-            w2[s] = ((l2 % C) * ROW + l2 / C); w2[C + s] = (((l2 + K2) % C) * ROW + (l2 + K2) / C);
+            w0[s] = at(l0) | (at(l0 + K0) << 16);
+            w1[s] = at(l1) | (at(l1 + K1) << 16);
+            w2[s] = at(l2) | (at(l2 + K2) << 16);
         }
-        tmem_park_words<2 * C>(tmem + T_W0, w0);
-        tmem_park_words<2 * C>(tmem + T_W1, w1);
-        tmem_park_words<2 * C>(tmem + T_W2, w2);
+        tmem_park_words<C>(tmem + T_W0, w0);
+        tmem_park_words<C>(tmem + T_W1, w1);
+        tmem_park_words<C>(tmem + T_W2, w2);
         tmem_wait_st();
     }
     mbar_wait(&s_bar, 0);
@@ -514,11 +524,11 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB
                 T A[3][C], Gs[3][C];
 #pragma unroll
                 for (int i = 0; i < 3; i++) {
-                    int wi[2 * C];
-                    tmem_fetch_words<2 * C>(tmem + T_W0 + 2 * C * i, wi);
+                    int wi[CE];
+                    tmem_fetch_words<CE>(tmem + T_W0 + CE * i, wi);
 #pragma unroll
                     for (int s = 0; s < C; s++) {
-                        const int a_ = wi[s], b_ = wi[C + s];
+                        const int a_ = wi[s] & 0xffff, b_ = (int)((unsigned)wi[s] >> 16);
                         const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_], l2 = E45[a_], h2 = E45[b_];
                         const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                         const T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
@@ -546,12 +556,12 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB
                 int amin = 0x7fffffff;
 #pragma unroll
                 for (int i = 0; i < 3; i++) {
-                    int wi[2 * C];
-                    tmem_fetch_words<2 * C>(tmem + T_W0 + 2 * C * i, wi);
+                    int wi[CE];
+                    tmem_fetch_words<CE>(tmem + T_W0 + CE * i, wi);
                     T Ai[C], q_isw[C], q_xb[C], q_g[C];
 #pragma unroll
                     for (int s = 0; s < C; s++) {
-                        const int a_ = wi[s], b_ = wi[C + s];
+                        const int a_ = wi[s] & 0xffff, b_ = (int)((unsigned)wi[s] >> 16);
                         const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_];
                         const T lxy = E4[a_], hxy = E4[b_];
                         const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
@@ -602,12 +612,12 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB
                     pair_scan_finish<G, C, T>(qs1, zc, zd, s_tot[1], E23, warp, tid);
                     pair_scan_finish<G, C, T>(qs2, ze, zf, s_tot[2], E45, warp, tid);
                     __syncthreads();                                                        // BAR 5
-                    int w1i[2 * C];
-                    tmem_fetch_words<2 * C>(tmem + T_W1, w1i);
+                    int w1i[CE];
+                    tmem_fetch_words<CE>(tmem + T_W1, w1i);
                     auto mid_load = [&](const T2* Ez, T (&out)[C]) {
 #pragma unroll
                         for (int s = 0; s < C; s++) {
-                            const T2 l = Ez[w1i[s]], h = Ez[w1i[C + s]];
+                            const T2 l = Ez[w1i[s] & 0xffff], h = Ez[(unsigned)w1i[s] >> 16];
                             const T Sz = h.x - l.x, Sxz = h.y - l.y;
                             out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
                         }
@@ -642,14 +652,14 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, GroupCfg<G, C, T>::MINB
                     __syncthreads();                                                        // BAR 8
                     pair_scan_finish<G, C, T>(fs0, zc, zd, s_tot[1], E23, warp, tid);
                     __syncthreads();                                                        // BAR 9
-                    int w0i[2 * C];
-                    tmem_fetch_words<2 * C>(tmem + T_W0, w0i);
+                    int w0i[CE];
+                    tmem_fetch_words<CE>(tmem + T_W0, w0i);
                     T t_isw[C], t_xb[C], t_g[C], yy[C];
                     TA::fetch(tmem + T_ISW, t_isw); TA::fetch(tmem + T_XB, t_xb); TA::fetch(tmem + T_G0, t_g);
                     TA::fetch(tmem + T_Y, yy);
 #pragma unroll
                     for (int s = 0; s < C; s++) {
-                        const T2 l = E23[w0i[s]], h = E23[w0i[C + s]];
+                        const T2 l = E23[w0i[s] & 0xffff], h = E23[(unsigned)w0i[s] >> 16];
                         const T Sz = h.x - l.x, Sxz = h.y - l.y;
                         const T smo = Sz * t_isw[s] + (Sxz - t_xb[s] * Sz) * t_g[s];
                         const T r = yy[s] - smo;

@@ -29,6 +29,7 @@ ss_status_t SS_TU_FN(const EvalParams& p, int c, int64_t n_items, cudaStream_t s
         case 5: return launch_group_variant<SS_TU_G, 5, GV, tu_real>(p, n_items, stream);
 #if SS_TU_G != 16
         case 6: return launch_group_variant<SS_TU_G, 6, GV, tu_real>(p, n_items, stream);
+        case 7: return launch_group_variant<SS_TU_G, 7, GV, tu_real>(p, n_items, stream);
 #endif
         default: return SS_ERR_UNSUPPORTED;
     }

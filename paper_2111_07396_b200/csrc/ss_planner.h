@@ -46,7 +46,7 @@ inline int group_variant_for_n(int n)
 {
     const int gs[3] = {4, 8, 16};
     for (int gi = 0; gi < 3; gi++)
-        for (int c = 3; c <= (gs[gi] == 16 ? 5 : 6); c++)
+        for (int c = 3; c <= (gs[gi] == 16 ? 5 : 7); c++)
             if (32 * gs[gi] * c >= n && !(gs[gi] > 4 && c == 3)) return gs[gi] * 8 + c;
     return 16 * 8 + 5;
 }
