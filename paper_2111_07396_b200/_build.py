@@ -34,7 +34,7 @@ def units():
         if base == "ss_warp_tu":
             for gv in (0, 1):
                 for grp in (0, 1, 2):
-                    for sh in (0, 1):
+                    for sh in (0, 1, 2):
                         u.append((f"{base}_{gv}_{grp}_{sh}.o", src,
                                   [f"-DSS_TU_GV={gv}", f"-DSS_TU_GROUP={grp}", f"-DSS_TU_SHARED={sh}"]))
         elif base == "ss_group_tu":
@@ -47,7 +47,7 @@ def units():
                 for c in (3, 4, 5):
                     u.append((f"{base}_{gv}_{c}.o", src, [f"-DSS_TU_GV={gv}", f"-DSS_TU_C={c}"]))
         elif base == "ss_block_tu":
-            for part in range(10):
+            for part in range(14):
                 u.append((f"{base}_{part}.o", src, [f"-DSS_TU_PART={part}"]))
         else:
             u.append((base + ".o", src, []))

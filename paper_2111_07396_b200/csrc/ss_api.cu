@@ -514,14 +514,16 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (r.obj < o0 || r.obj >= o1) continue;
             int path = o.force_path != SS_PATH_AUTO ? o.force_path : path_for_n(r.n, md);
             // periodic windows and the fixed span live in the generic CTA-per-eval code only
-            if ((path == SS_PATH_WARP || path == SS_PATH_GROUP) && has_listing_options(o)) path = SS_PATH_BLOCK;
+            // periodic windows and the fixed span: the warp path has its own kernel for them, longer light curves
+            // go to the generic CTA-per-eval code
+            if (path == SS_PATH_GROUP && has_listing_options(o)) path = SS_PATH_BLOCK;
             if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_GROUP;
             if (path == SS_PATH_CLUSTER && has_listing_options(o)) path = SS_PATH_STAGE;
             if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N) path = SS_PATH_CLUSTER;
             if (path == SS_PATH_CLUSTER && (r.n > SS_CLUSTER_MAX_N || r.n < 2 * 512)) path = SS_PATH_STAGE;
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
-            if (path == SS_PATH_WARP) variant = warp_variant_for_n(r.n);
+            if (path == SS_PATH_WARP) variant = has_listing_options(o) ? WARP_VARIANT_OPT + std::max(2, (r.n + 31) / 32) : warp_variant_for_n(r.n);
             else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? GROUP_VARIANT_F32 : 0);
             else if (path == SS_PATH_CLUSTER) variant = cluster_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
@@ -638,7 +640,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         p.counter = counters + (next_counter % n_counters);
         p.stage = stage; p.stage_stride = stage_stride;
         p.defer_entries = defer_entries; p.defer_count = defer_count; p.defer_capacity = defer_capacity;
-        const bool shared = opt.shared_times && c.path == SS_PATH_WARP;      // one fold + sort per group of objects
+        const bool shared = opt.shared_times && c.path == SS_PATH_WARP && c.variant < WARP_VARIANT_OPT;      // one fold + sort per group of objects
         const int64_t n_items = (shared ? ((int64_t)p.n_list + SHARED_TIMES_M - 1) / SHARED_TIMES_M : (int64_t)p.n_list) * cpo;
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -654,8 +656,10 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         }
         if (ev0) SS_CUDA(cudaEventRecord(ev0, stream));
         if (c.path == SS_PATH_WARP) {
-            ss_status_t st = shared ? launch_warp_shared_kernel(p, c.variant, n_items, stream)
-                                    : launch_warp_kernel(p, c.variant, n_items, stream);
+            ss_status_t st = c.variant >= WARP_VARIANT_OPT
+                                 ? launch_warp_opt_kernel(p, c.variant - WARP_VARIANT_OPT, opt.span > 0.0 ? 2 : mode, n_items, stream)
+                                 : shared ? launch_warp_shared_kernel(p, c.variant, n_items, stream)
+                                          : launch_warp_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "warp kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (c.path == SS_PATH_CLUSTER) {
             ss_status_t st = launch_cluster_kernel(p, c.variant, n_items, stream);
@@ -676,7 +680,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             // write their partial-argmax slot (hence before the fold below), single evals fold into the running best
             SS_CUDA(cudaMemsetAsync(dmax, 0, 8 * (size_t)n_objects, stream));
             SS_CUDA(cudaMemsetAsync(dmin, 0xff, 8 * (size_t)n_objects, stream));
-            ss_status_t st = launch_deferred_eval(p, defer_val, dmax, c.max_n, sm_count, stream);
+            ss_status_t st = launch_deferred_eval(p, defer_val, dmax, c.max_n, has_listing_options(opt), sm_count, stream);
             if (st != SS_OK) return fail(st, "deferred kernel launch failed");
             g_launches++;
         }

@@ -1,23 +1,116 @@
 // ss_block_tu.cu -- instantiations and launchers of the CTA-per-eval kernels (ss_block_kernel.cuh), the kernels
 // that recompute what the warp path hands over, and the dispatcher over the warp-kernel translation units.
-// Compiled ten times by _build.py, -DSS_TU_PART=0..9, so the instantiations build in parallel:
-//   part 0       dispatchers and the hand-over (deferred) kernels
-//   part 1       the debug kernel
-//   parts 2..9   one block_kernel<T, STAGE, OPT> each
+// Compiled fourteen times by _build.py, -DSS_TU_PART=0..13, so the instantiations build in parallel:
+//   part 0         dispatchers and the small hand-over kernels
+//   part 1         the debug kernel
+//   parts 2..9     one block_kernel<T, STAGE, OPT> each
+//   parts 10..13   one deferred_eval_kernel<T, STAGE, OPT> each (what the warp / group / cluster paths hand over)
 #include "ss_block_kernel.cuh"
 #include "ss_launch.h"
 #include "ss_planner.h"
 
 #ifndef SS_TU_PART
-#error "compile with -DSS_TU_PART=0..9"
+#error "compile with -DSS_TU_PART=0..13"
 #endif
 
 namespace ss {
 
 template <int T, bool STAGE, bool OPT>
 ss_status_t launch_block_variant(const EvalParams& p, size_t smem, int grid, cudaStream_t stream);
+template <int T, bool STAGE, bool OPT>
+ss_status_t launch_deferred_variant(const EvalParams& p, double* dval, unsigned long long* dmax, size_t smem, int grid,
+                                    cudaStream_t stream);
 
-#if SS_TU_PART >= 2
+#if SS_TU_PART >= 10
+// ---- what the warp path hands over: recomputed exactly by the generic CTA-per-eval code ------------------
+// Entry formats (EvalParams::defer_entries):
+//   eval  : record index << 32 | (k - k_begin)             one (object, frequency) pair (tied or misordered phases,
+//                                                          a leave-one-out denominator <= 0)
+//   item  : 1 << 63 | record index << 32 | chunk index     a whole work item (the object has duplicated time stamps:
+//                                                          every one of its evals ties)
+
+__device__ __forceinline__ unsigned long long sortable_bits(double v)
+{
+    if (v != v) return 0ull;      // NaN sorts below everything: it can never hide a valid maximum
+    unsigned long long u = (unsigned long long)__double_as_longlong(v);
+    return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
+}
+
+// STAGE: per-eval arrays in this CTA's slot of the global staging scratch (light curves beyond the shared-memory limit)
+template <int DEFER_T, bool STAGE, bool OPT>
+__global__ void __launch_bounds__(DEFER_T) deferred_eval_kernel(const EvalParams p, double* dval,
+                                                                unsigned long long* dmax)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NW = DEFER_T / 32;
+    __shared__ double s_wsum[6][NW];
+    __shared__ double s_red[NW];
+    __shared__ int s_flags[4];
+    BlockCtx<DEFER_T> cx;
+    cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
+    double* S = STAGE ? p.stage + (int64_t)blockIdx.x * p.stage_stride : reinterpret_cast<double*>(smem_raw);
+    const unsigned cnt = min(p.defer_count[0], p.defer_capacity);
+    for (unsigned e = blockIdx.x; e < cnt; e += gridDim.x) {
+        const unsigned long long ent = p.defer_entries[e];
+        const int ri = (int)((ent & ~DEFER_ITEM) >> 32);
+        const ObjRec rec = p.recs[ri];
+        const int64_t sl = block_slot_len(rec.n);
+        double* prow = p.pgram ? p.pgram + (rec.obj - p.pgram_row0) * p.pgram_row_stride - p.pgram_k0 : nullptr;
+        if (ent & DEFER_ITEM) {
+            const int ch = (int)(ent & 0xffffffffull);
+            const int64_t k0 = p.k_begin + (int64_t)ch * p.chunk;
+            const int64_t k1 = min(k0 + (int64_t)p.chunk, p.k_end);
+            double best = -INFINITY;
+            int64_t best_k = k0;
+            for (int64_t k = k0; k < k1; k++) {
+                __syncthreads();
+                const double P = block_eval<DEFER_T, OPT>(p, rec, freq_of(p.f_min, p.df, k), S, sl, cx, nullptr, nullptr);
+                if (threadIdx.x == 0) {
+                    if (prow) prow[k] = P;
+                    if (P > best) { best = P; best_k = k; }
+                }
+            }
+            if (threadIdx.x == 0) {
+                const int64_t slot = (int64_t)ri * p.chunks_total + p.chunk_base + ch;
+                p.part_val[slot] = best;
+                p.part_idx[slot] = best_k;
+                dval[e] = nan("");
+            }
+            continue;
+        }
+        const int64_t k = p.k_begin + (int64_t)(ent & 0xffffffffull);
+        __syncthreads();
+        const double P = block_eval<DEFER_T, OPT>(p, rec, freq_of(p.f_min, p.df, k), S, sl, cx, nullptr, nullptr);
+        if (threadIdx.x == 0) {
+            if (prow) prow[k] = P;
+            dval[e] = P;
+            atomicMax(&dmax[rec.obj], sortable_bits(P));
+        }
+    }
+}
+
+
+template <int T, bool STAGE, bool OPT>
+ss_status_t launch_deferred_variant(const EvalParams& p, double* dval, unsigned long long* dmax, size_t smem, int grid,
+                                    cudaStream_t stream)
+{
+    auto kern = deferred_eval_kernel<T, STAGE, OPT>;
+    if (smem > 0 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+        return SS_ERR_CUDA;
+    kern<<<grid, T, smem, stream>>>(p, dval, dmax);
+    return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
+}
+#if SS_TU_PART == 10
+template ss_status_t launch_deferred_variant<128, false, false>(const EvalParams&, double*, unsigned long long*, size_t, int, cudaStream_t);
+#elif SS_TU_PART == 11
+template ss_status_t launch_deferred_variant<128, false, true>(const EvalParams&, double*, unsigned long long*, size_t, int, cudaStream_t);
+#elif SS_TU_PART == 12
+template ss_status_t launch_deferred_variant<512, true, false>(const EvalParams&, double*, unsigned long long*, size_t, int, cudaStream_t);
+#else
+template ss_status_t launch_deferred_variant<512, true, true>(const EvalParams&, double*, unsigned long long*, size_t, int, cudaStream_t);
+#endif
+
+#elif SS_TU_PART >= 2
 template <int T, bool STAGE, bool OPT>
 ss_status_t launch_block_variant(const EvalParams& p, size_t smem, int grid, cudaStream_t stream)
 {
@@ -85,6 +178,20 @@ ss_status_t launch_warp_shared_kernel(const EvalParams& p, int variant, int64_t 
          : g == 1 ? launch_warp_shared_tu_0_1(p, variant, n_items, stream) : launch_warp_shared_tu_0_2(p, variant, n_items, stream);
 }
 
+#define SS_DECL(gv, g) ss_status_t launch_warp_opt_tu_##gv##_##g(const EvalParams&, int, int, int64_t, cudaStream_t);
+SS_DECL(0, 0) SS_DECL(0, 1) SS_DECL(0, 2) SS_DECL(1, 0) SS_DECL(1, 1) SS_DECL(1, 2)
+#undef SS_DECL
+
+ss_status_t launch_warp_opt_kernel(const EvalParams& p, int c, int mode, int64_t n_items, cudaStream_t stream)
+{
+    const int g = c <= 4 ? 0 : (c <= 6 ? 1 : 2);
+    if (mode == 1)
+        return g == 0 ? launch_warp_opt_tu_1_0(p, c, mode, n_items, stream)
+             : g == 1 ? launch_warp_opt_tu_1_1(p, c, mode, n_items, stream) : launch_warp_opt_tu_1_2(p, c, mode, n_items, stream);
+    return g == 0 ? launch_warp_opt_tu_0_0(p, c, mode, n_items, stream)
+         : g == 1 ? launch_warp_opt_tu_0_1(p, c, mode, n_items, stream) : launch_warp_opt_tu_0_2(p, c, mode, n_items, stream);
+}
+
 // ---- group-kernel translation units (ss_group_tu.cu) -------------------------------------------------
 #define SS_DECL(gv, g) ss_status_t launch_group_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
 SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
@@ -146,73 +253,13 @@ ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int 
                : launch_block_variant<256, false, false>(p, smem, grid_of(2), stream);
 }
 
-// ---- what the warp path hands over: recomputed exactly by the generic CTA-per-eval code ------------------
-// Entry formats (EvalParams::defer_entries):
-//   eval  : record index << 32 | (k - k_begin)             one (object, frequency) pair (tied or misordered phases,
-//                                                          a leave-one-out denominator <= 0)
-//   item  : 1 << 63 | record index << 32 | chunk index     a whole work item (the object has duplicated time stamps:
-//                                                          every one of its evals ties)
-
+// (the hand-over eval kernels are instantiated in parts 10..13)
 __device__ __forceinline__ unsigned long long sortable_bits(double v)
 {
     if (v != v) return 0ull;      // NaN sorts below everything: it can never hide a valid maximum
     unsigned long long u = (unsigned long long)__double_as_longlong(v);
     return (u >> 63) ? ~u : (u | 0x8000000000000000ull);
 }
-
-// STAGE: per-eval arrays in this CTA's slot of the global staging scratch (light curves beyond the shared-memory limit)
-template <int DEFER_T, bool STAGE>
-__global__ void __launch_bounds__(DEFER_T) deferred_eval_kernel(const EvalParams p, double* dval,
-                                                                unsigned long long* dmax)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    constexpr int NW = DEFER_T / 32;
-    __shared__ double s_wsum[6][NW];
-    __shared__ double s_red[NW];
-    __shared__ int s_flags[4];
-    BlockCtx<DEFER_T> cx;
-    cx.wsum = s_wsum; cx.red = s_red; cx.flags = s_flags;
-    double* S = STAGE ? p.stage + (int64_t)blockIdx.x * p.stage_stride : reinterpret_cast<double*>(smem_raw);
-    const unsigned cnt = min(p.defer_count[0], p.defer_capacity);
-    for (unsigned e = blockIdx.x; e < cnt; e += gridDim.x) {
-        const unsigned long long ent = p.defer_entries[e];
-        const int ri = (int)((ent & ~DEFER_ITEM) >> 32);
-        const ObjRec rec = p.recs[ri];
-        const int64_t sl = block_slot_len(rec.n);
-        double* prow = p.pgram ? p.pgram + (rec.obj - p.pgram_row0) * p.pgram_row_stride - p.pgram_k0 : nullptr;
-        if (ent & DEFER_ITEM) {
-            const int ch = (int)(ent & 0xffffffffull);
-            const int64_t k0 = p.k_begin + (int64_t)ch * p.chunk;
-            const int64_t k1 = min(k0 + (int64_t)p.chunk, p.k_end);
-            double best = -INFINITY;
-            int64_t best_k = k0;
-            for (int64_t k = k0; k < k1; k++) {
-                __syncthreads();
-                const double P = block_eval<DEFER_T, false>(p, rec, freq_of(p.f_min, p.df, k), S, sl, cx, nullptr, nullptr);
-                if (threadIdx.x == 0) {
-                    if (prow) prow[k] = P;
-                    if (P > best) { best = P; best_k = k; }
-                }
-            }
-            if (threadIdx.x == 0) {
-                const int64_t slot = (int64_t)ri * p.chunks_total + p.chunk_base + ch;
-                p.part_val[slot] = best;
-                p.part_idx[slot] = best_k;
-                dval[e] = nan("");
-            }
-            continue;
-        }
-        const int64_t k = p.k_begin + (int64_t)(ent & 0xffffffffull);
-        __syncthreads();
-        const double P = block_eval<DEFER_T, false>(p, rec, freq_of(p.f_min, p.df, k), S, sl, cx, nullptr, nullptr);
-        if (threadIdx.x == 0) {
-            if (prow) prow[k] = P;
-            dval[e] = P;
-            atomicMax(&dmax[rec.obj], sortable_bits(P));
-        }
-    }
-}
-
 __global__ void deferred_min_kernel(const EvalParams p, const double* dval, const unsigned long long* dmax,
                                     unsigned long long* dmin)
 {
@@ -246,19 +293,15 @@ __global__ void deferred_merge_kernel(const EvalParams p, const double* dval, co
     }
 }
 
-ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, int sm_count,
-                                 cudaStream_t stream)
+ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, bool opt,
+                                 int sm_count, cudaStream_t stream)
 {
-    if (max_n > BLOCK_MAX_N) {
-        // the staging scratch holds 2 slots per SM (Engine::setup)
-        deferred_eval_kernel<512, true><<<sm_count * 2, 512, 0, stream>>>(p, dval, dmax);
-        return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
-    }
+    if (max_n > BLOCK_MAX_N)      // the staging scratch holds 2 slots per SM (Engine::setup)
+        return opt ? launch_deferred_variant<512, true, true>(p, dval, dmax, 0, sm_count * 2, stream)
+                   : launch_deferred_variant<512, true, false>(p, dval, dmax, 0, sm_count * 2, stream);
     const size_t smem = (size_t)BLOCK_SLOTS * (size_t)block_slot_len(max_n) * 8;
-    if (cudaFuncSetAttribute(deferred_eval_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-        return SS_ERR_CUDA;
-    deferred_eval_kernel<128, false><<<sm_count * 4, 128, smem, stream>>>(p, dval, dmax);
-    return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
+    return opt ? launch_deferred_variant<128, false, true>(p, dval, dmax, smem, sm_count * 4, stream)
+               : launch_deferred_variant<128, false, false>(p, dval, dmax, smem, sm_count * 4, stream);
 }
 
 ss_status_t launch_deferred_merge(const EvalParams& p, const double* dval, const unsigned long long* dmax,

@@ -15,6 +15,9 @@ ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items
 // the same for a catalog with one shared time sampling (ss_warp_shared.cuh): n_items = groups of SHARED_M objects x chunks
 ss_status_t launch_warp_shared_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 
+// the listing's options on the warp path (ss_warp_opt.cuh): c = points per lane, mode 0 = CV, 1 = GV, 2 = fixed span
+ss_status_t launch_warp_opt_kernel(const EvalParams& p, int c, int mode, int64_t n_items, cudaStream_t stream);
+
 // G-warps-per-eval kernels (ss_group_kernel.cuh); variant = group_variant_for_n(n)
 ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 
@@ -28,8 +31,8 @@ ss_status_t launch_block_kernel(const EvalParams& p, int path, int threads, int 
 
 // evals / whole work items the warp path handed over (p.defer_entries): recompute with the generic code, patch the
 // periodogram and the item's partial-argmax slot (item entries) or fold into best_val / best_idx (eval entries)
-ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, int sm_count,
-                                 cudaStream_t stream);
+ss_status_t launch_deferred_eval(const EvalParams& p, double* dval, unsigned long long* dmax, int max_n, bool opt,
+                                 int sm_count, cudaStream_t stream);
 ss_status_t launch_deferred_merge(const EvalParams& p, const double* dval, const unsigned long long* dmax,
                                   unsigned long long* dmin, double* best_val, int64_t* best_idx, int sm_count,
                                   cudaStream_t stream);

@@ -357,6 +357,18 @@ __device__ __forceinline__ void tmem_fetch_words(uint32_t taddr, int (&v)[N])
     else asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6), SS_T(7) :: "memory");
 #undef SS_T
 }
+// N words, N odd or even: an odd count reads one column more (the caller's tables leave it allocated)
+template <int N>
+__device__ __forceinline__ void tmem_fetch_words_any(uint32_t taddr, int (&v)[N])
+{
+    if constexpr (N % 2 == 0) tmem_fetch_words<N>(taddr, v);
+    else {
+        int t[N + 1];
+        tmem_fetch_words<N + 1>(taddr, t);
+#pragma unroll
+        for (int i = 0; i < N; i++) v[i] = t[i];
+    }
+}
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // Per-warp view of the shared memory.

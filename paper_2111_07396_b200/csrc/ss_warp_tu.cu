@@ -1,9 +1,11 @@
 // ss_warp_tu.cu -- instantiations of the warp-per-eval kernel.  Compiled twelve times by _build.py:
 //   -DSS_TU_GV=0|1 (cross-validation / generalized validation)  x  -DSS_TU_GROUP=0|1|2 (C = 2..4 / 5..6 / 7..8)
-//   x -DSS_TU_SHARED=0|1 (warp_kernel / warp_shared_kernel, the shared-time-sampling variant)
-// so that the 40 kernels build in parallel.
+//   x -DSS_TU_SHARED=0|1|2 (warp_kernel / warp_shared_kernel, the shared-time-sampling variant / warp_opt_kernel,
+//     the listing's options)
+// so that the kernels build in parallel.
 #include "ss_launch.h"
 #include "ss_warp_kernel.cuh"
+#include "ss_warp_opt.cuh"
 #include "ss_warp_shared.cuh"
 
 #ifndef SS_TU_GV
@@ -14,7 +16,7 @@ namespace ss {
 
 #define SS_CAT2(a, b, c, d) a##b##c##d
 #define SS_CAT(a, b, c, d) SS_CAT2(a, b, c, d)
-#if SS_TU_SHARED
+#if SS_TU_SHARED == 1
 #define SS_TU_FN SS_CAT(launch_warp_shared_tu_, SS_TU_GV, _, SS_TU_GROUP)
 #define SS_TU_LAUNCH launch_warp_shared_variant
 #else
@@ -22,6 +24,31 @@ namespace ss {
 #define SS_TU_LAUNCH launch_warp_variant
 #endif
 
+#if SS_TU_SHARED == 2
+// the options variant (ss_warp_opt.cuh): variant = points per lane C; mode 0 = CV, 1 = GV, 2 = fixed span.  This
+// translation unit holds MODE = SS_TU_GV, and the fixed-span kernels ride with SS_TU_GV = 0.
+#undef SS_TU_FN
+#define SS_TU_FN SS_CAT(launch_warp_opt_tu_, SS_TU_GV, _, SS_TU_GROUP)
+ss_status_t SS_TU_FN(const EvalParams& p, int c, int mode, int64_t n_items, cudaStream_t stream)
+{
+#define SS_OPT_CASE(C_)                                                                                   \
+    case C_:                                                                                               \
+        if (mode == SS_TU_GV) return launch_warp_opt_variant<C_, SS_TU_GV>(p, n_items, stream);            \
+        if (SS_TU_GV == 0 && mode == 2) return launch_warp_opt_variant<C_, SS_TU_GV == 0 ? 2 : 1>(p, n_items, stream); \
+        return SS_ERR_UNSUPPORTED;
+    switch (c) {
+#if SS_TU_GROUP == 0
+        SS_OPT_CASE(2) SS_OPT_CASE(3) SS_OPT_CASE(4)
+#elif SS_TU_GROUP == 1
+        SS_OPT_CASE(5) SS_OPT_CASE(6)
+#else
+        SS_OPT_CASE(7) SS_OPT_CASE(8)
+#endif
+        default: return SS_ERR_UNSUPPORTED;
+    }
+#undef SS_OPT_CASE
+}
+#else
 ss_status_t SS_TU_FN(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
 {
     constexpr bool GV = SS_TU_GV != 0;
@@ -43,5 +70,6 @@ ss_status_t SS_TU_FN(const EvalParams& p, int variant, int64_t n_items, cudaStre
         default: return SS_ERR_UNSUPPORTED;
     }
 }
+#endif
 
 }  // namespace ss

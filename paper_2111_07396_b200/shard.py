@@ -12,9 +12,9 @@ from __future__ import annotations
 
 import numpy as np
 
-# Point-evals per second each path class sustains on one B200 (profiles/r1g_crossover.md, CV mode):
-# the relative cost of an object is n / rate(path(n)).  Only the ratios matter.
-_RATE = ((256, 3.3e10), (2055, 1.15e10), (1 << 62, 3.5e9))
+# Point-evals per second each path class sustains on one B200 (profiles/r2_crossover.md, CV mode: warp / group /
+# cluster / global staging): the relative cost of an object is n / rate(path(n)).  Only the ratios matter.
+_RATE = ((256, 3.3e10), (2055, 2.3e10), (40960, 5.0e9), (1 << 62, 1.4e9))
 
 
 def object_cost(n) -> np.ndarray:

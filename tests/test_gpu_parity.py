@@ -955,3 +955,37 @@ def test_async_call_and_caller_workspace(ss):
         ss.ss_periodogram(t, y, e, off, n_obj, 0.5, 24.0, n_freq, CV, pg, None, bi,
                           ss.default_options(workspace=ws.data_ptr(), workspace_bytes=1 << 20))
     assert ei.value.status == ss.SS_ERR_OUT_OF_MEMORY
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("opts", LISTING_OPTIONS, ids=lambda o: ",".join(f"{k}={v}" for k, v in o.items()))
+def test_listing_options_on_the_warp_path(ss, mode, opts):
+    """iper = 2 / span > 0 for n <= 256 are served by warp_opt_kernel (every window by prefix differences through a
+    table of two ranges per point): objects of every points-per-lane class (n = 5 .. 256, incl. n = 32 C exactly), an
+    object with duplicated time stamps (handed over whole) and integer-day times that tie at f = 1 / d, against the
+    definition oracle, best index included; and against the generic CTA kernel (forced) within the parity bar."""
+    rng = np.random.default_rng(818)
+    ns = [5, 6, 9, 31, 64, 65, 96, 100, 128, 150, 160, 192, 200, 224, 255, 256, 120, 48]
+    T, Y, E = [], [], []
+    for i, n in enumerate(ns):
+        t = np.sort(rng.integers(0, 30, size=n) + rng.uniform(0.0, 0.33, size=n))
+        if i == len(ns) - 2:
+            t[11] = t[10]                                   # duplicated time stamp
+        if i == len(ns) - 1:
+            t = np.arange(n, dtype=np.float64) + 0.25 * (np.arange(n) % 3 == 0)      # ties at f = 1
+        e = rng.uniform(0.02, 0.1, size=n)
+        y = 15 + rng.uniform(0.2, 0.8) * np.sin(2 * np.pi * t / np.exp(rng.uniform(np.log(0.3), np.log(2.0))) + i) \
+            + rng.normal(0, 1.0, size=n) * e
+        T.append(t); Y.append(y); E.append(e)
+    off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
+    cat = ss_inputs.Catalog("opts", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
+                            0.25, 4.25, 64, np.full(len(ns), np.nan))
+    assert oracle.freq(cat.f_min, cat.f_max, cat.n_freq, 12) == 1.0
+    ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                                   mode=mode, variant=oracle.DEFINITION, **opts)
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
+    check_parity(cat, res.pgram, ref, mode, label=f"warp-opt {opts}", oracle_opts=opts, max_ambiguous=4)
+    check_best(ref, res.best_index, res.best_freq, cat)
+    blk = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                         force_path=ss.PATH_BLOCK, **opts)
+    check_parity(cat, blk.pgram, ref, mode, label=f"cta-opt {opts}", oracle_opts=opts, max_ambiguous=4)
