@@ -160,7 +160,7 @@ __global__ void __launch_bounds__(WarpOptCfg<C>::WPC * 32, WarpOptCfg<C>::MINB) 
         double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y, Sxy, Syy = 0.0;
         if (GV) { const double2 l2 = E45[wn.lo], h2 = E45[wn.hi]; Sxy = h2.x - l2.x; Syy = h2.y - l2.y; }
         else Sxy = E4[wn.hi] - E4[wn.lo];
-        if (per) {
+        if (per && wn.s != 0.0) {      // only the lanes whose window wraps
             const double2 m0 = E01[wn.blo], n0 = E01[wn.bhi], m1 = E23[wn.blo], n1 = E23[wn.bhi];
             const double bw = n0.x - m0.x, bwx = n0.y - m0.y, bwxx = n1.x - m1.x, by = n1.y - m1.y;
             double bxy, byy = 0.0;
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(WarpOptCfg<C>::WPC * 32, WarpOptCfg<C>::MINB) 
         const WinIdx wn = win_unpack(a, b);
         const double2 l = Ez[wn.lo], h = Ez[wn.hi];
         Sz = h.x - l.x; Sxz = h.y - l.y;
-        if (per) {
+        if (per && wn.s != 0.0) {
             const double2 m = Ez[wn.blo], q = Ez[wn.bhi];
             const double bz = q.x - m.x;
             Sz += bz; Sxz += (q.y - m.y) + wn.s * bz;

@@ -8,6 +8,7 @@ where a path scales and drops where it stops fitting.  The path the library pick
 
     python -m paper_2111_07396_b200.sweep [--ns 50,100,...] [--target-ms 150] [--md out.md]
     python -m paper_2111_07396_b200.sweep --options [--md out.md]     # the listing's options vs the default call
+    python -m paper_2111_07396_b200.sweep --shared | --mixed          # shared time sampling / mixed precision vs the plain call
 
 Needs a CUDA device (no CPU fallback).  Inputs are synthetic: times uniform over 30 nights (8 h per
 night), a sinusoid of random period plus Gaussian noise; the arithmetic under test is all in the library.
@@ -93,6 +94,66 @@ def options_table(torch, dev, md):
     return 0
 
 
+def _best_of(torch, call, reps=3):
+    import time
+    best = float("inf")
+    for _ in range(reps):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        call()
+        torch.cuda.synchronize()
+        best = min(best, time.perf_counter() - t0)
+    return best
+
+
+def shared_table(torch, dev, md):
+    """shared_times = 1 (one fold + sort per frequency for 4 objects) against the ordinary call."""
+    n_obj, nf = 2000, 10000
+    lines = ["| n | mode | plain evals/s | shared_times evals/s | speed-up |", "|---|---|---|---|---|"]
+    for n in (64, 125, 200):
+        rng = np.random.default_rng(n)
+        t1 = np.sort(rng.integers(0, 30, size=n) + rng.uniform(0.0, 0.33, size=n))
+        t = np.tile(t1, n_obj)
+        e = rng.uniform(0.02, 0.1, size=n_obj * n)
+        y = 15 + 0.4 * np.sin(2 * np.pi * t / np.repeat(np.exp(rng.uniform(np.log(0.1), np.log(2.0), size=n_obj)), n)) \
+            + rng.normal(0, 1.0, size=n_obj * n) * e
+        off = np.arange(n_obj + 1, dtype=np.int64) * n
+        a = [torch.as_tensor(v, device=dev) for v in (t, y, e, off)]
+        pg = torch.empty((n_obj, nf), dtype=torch.float64, device=dev)
+        for mode, name in ((CROSS_VALIDATION, "cv"), (GENERALIZED_VALIDATION, "gv")):
+            r = []
+            for sh in (0, 1):
+                o = default_options(shared_times=sh, skip_validation=1)
+                r.append(n_obj * nf / _best_of(torch, lambda: ss_periodogram(*a, n_obj, 0.5, 24.0, nf, mode, pg, None, None, o)))
+            lines.append(f"| {n} | {name} | {r[0]:.4g} | {r[1]:.4g} | {r[1] / r[0]:.3f} |")
+            print(lines[-1], flush=True)
+    if md:
+        with open(md, "w") as f:
+            f.write("\n".join(lines) + "\n")
+    return 0
+
+
+def mixed_table(torch, dev, md):
+    """precision = SS_PRECISION_MIXED (fp32 smoother on the group path) against fp64."""
+    import ss_inputs
+    cat = ss_inputs.config4(n_objects=300, n_freq=4000)
+    a = [torch.as_tensor(v, device=dev) for v in (cat.times, cat.mags, cat.errs, cat.offsets)]
+    pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev)
+    lines = ["| mode | fp64 point-evals/s | mixed point-evals/s | speed-up |", "|---|---|---|---|"]
+    for mode, name in ((CROSS_VALIDATION, "cv"), (GENERALIZED_VALIDATION, "gv")):
+        r = []
+        for pr in (0, 1):
+            o = default_options(precision=pr, skip_validation=1)
+            r.append(cat.n_points * cat.n_freq / _best_of(torch, lambda: ss_periodogram(
+                *a, cat.n_objects, cat.f_min, cat.f_max, cat.n_freq, mode, pg, None, None, o)))
+        lines.append(f"| {name} | {r[0]:.4g} | {r[1]:.4g} | {r[1] / r[0]:.3f} |")
+        print(lines[-1], flush=True)
+    if md:
+        with open(md, "w") as f:
+            f.write("\n".join(lines) + "\n")
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--ns", default=",".join(map(str, DEFAULT_NS)))
@@ -101,6 +162,11 @@ def main(argv=None):
     ap.add_argument("--options", action="store_true",
                     help="instead of the sweep over n: the listing's options (iper = 2, fixed span; PAPER.md:199-210) "
                          "against the default call on 1,000 config-3-shaped objects x 5,000 frequencies")
+    ap.add_argument("--shared", action="store_true",
+                    help="instead: shared_times = 1 against the ordinary call on 2,000 objects with one time vector "
+                         "(PAPER.md:125), n = 64, 125, 200, 10,000 frequencies")
+    ap.add_argument("--mixed", action="store_true",
+                    help="instead: precision = mixed against fp64 on 300 config-4 objects x 4,000 frequencies (PAPER.md:604-616)")
     args = ap.parse_args(argv)
     import torch
     if not torch.cuda.is_available():
@@ -109,6 +175,10 @@ def main(argv=None):
     dev = torch.device("cuda")
     if args.options:
         return options_table(torch, dev, args.md)
+    if args.shared:
+        return shared_table(torch, dev, args.md)
+    if args.mixed:
+        return mixed_table(torch, dev, args.md)
     lines = ["| n | path | auto | objects x frequencies | CV point-evals/s | CV evals/s | GV point-evals/s | GV evals/s |",
              "|---|---|---|---|---|---|---|---|"]
     for n in [int(v) for v in args.ns.split(",")]:
