@@ -78,6 +78,16 @@ struct __align__(16) ClusterMail {
 
 typedef unsigned long long key64;
 
+// One side of a compare-exchange on 64-bit keys: the lower position keeps the smaller key.  Keys are distinct (the index
+// bits; all-ones padding keys are equal but then either choice is the same value), so "take the partner's" is
+// (other < mine) for the lower position and its negation for the upper one: one 64-bit compare and one select instead
+// of a min, a max and a select between them.
+__device__ __forceinline__ key64 cex_side64(key64 mine, key64 other, bool lower)
+{
+    const bool lt = other < mine;
+    return (lt == lower) ? other : mine;
+}
+
 // odd-even transposition network on C keys (C rounds): the lane-local sort for 64-bit keys
 template <int C>
 __device__ __forceinline__ void local_sort64(key64 (&k)[C])
@@ -86,7 +96,8 @@ __device__ __forceinline__ void local_sort64(key64 (&k)[C])
     for (int r = 0; r < C; r++) {
 #pragma unroll
         for (int s = r & 1; s + 1 < C; s += 2) {
-            const key64 lo = min(k[s], k[s + 1]), hi = max(k[s], k[s + 1]);
+            const bool lt = k[s + 1] < k[s];
+            const key64 lo = lt ? k[s + 1] : k[s], hi = lt ? k[s] : k[s + 1];
             k[s] = lo; k[s + 1] = hi;
         }
     }
@@ -109,7 +120,7 @@ __device__ __forceinline__ void cta_step64(key64 (&key)[C], int mask, bool lower
         for (int s = 0; s < C; s++) other[s] = kb[(REV ? C - 1 - s : s) * CL_NT + pt];
     }
 #pragma unroll
-    for (int s = 0; s < C; s++) key[s] = lower ? min(key[s], other[s]) : max(key[s], other[s]);
+    for (int s = 0; s < C; s++) key[s] = cex_side64(key[s], other[s], lower);
 }
 
 // the half-cleaners at thread strides 256 .. 1 inside the CTA, then the lane-local network
@@ -390,7 +401,7 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const EvalParams p, c
 #pragma unroll
                 for (int s = 0; s < C; s++) {
                     const key64 o = ld_cl_u64(ra + (uint32_t)(((C - 1 - s) * NT + (NT - 1 - tid)) * 8));
-                    key[s] = lower ? min(key[s], o) : max(key[s], o);
+                    key[s] = cex_side64(key[s], o, lower);
                 }
                 xflip ^= 1;
             }
@@ -404,7 +415,7 @@ __global__ void __launch_bounds__(CL_NT, 1) cluster_kernel(const EvalParams p, c
 #pragma unroll
                 for (int s = 0; s < C; s++) {
                     const key64 o = ld_cl_u64(ra + (uint32_t)((s * NT + tid) * 8));
-                    key[s] = lower ? min(key[s], o) : max(key[s], o);
+                    key[s] = cex_side64(key[s], o, lower);
                 }
                 xflip ^= 1;
             }
