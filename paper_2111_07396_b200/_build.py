@@ -34,7 +34,7 @@ def units():
         if base == "ss_warp_tu":
             for gv in (0, 1):
                 for grp in (0, 1, 2):
-                    for sh in (0, 1, 2):
+                    for sh in (0, 1, 2, 3):
                         u.append((f"{base}_{gv}_{grp}_{sh}.o", src,
                                   [f"-DSS_TU_GV={gv}", f"-DSS_TU_GROUP={grp}", f"-DSS_TU_SHARED={sh}"]))
         elif base == "ss_group_tu":

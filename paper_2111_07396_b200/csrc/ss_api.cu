@@ -523,7 +523,9 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (path == SS_PATH_CLUSTER && (r.n > SS_CLUSTER_MAX_N || r.n < 2 * 512)) path = SS_PATH_STAGE;
             if (path == SS_PATH_BLOCK && r.n > BLOCK_MAX_N) path = SS_PATH_STAGE;
             int variant = 0;
-            if (path == SS_PATH_WARP) variant = has_listing_options(o) ? WARP_VARIANT_OPT + std::max(2, (r.n + 31) / 32) : warp_variant_for_n(r.n);
+            if (path == SS_PATH_WARP)
+                variant = has_listing_options(o) ? WARP_VARIANT_OPT + std::max(2, (r.n + 31) / 32)
+                                                 : warp_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? WARP_VARIANT_F32 : 0);
             else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? GROUP_VARIANT_F32 : 0);
             else if (path == SS_PATH_CLUSTER) variant = cluster_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
@@ -640,7 +642,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         p.counter = counters + (next_counter % n_counters);
         p.stage = stage; p.stage_stride = stage_stride;
         p.defer_entries = defer_entries; p.defer_count = defer_count; p.defer_capacity = defer_capacity;
-        const bool shared = opt.shared_times && c.path == SS_PATH_WARP && c.variant < WARP_VARIANT_OPT;      // one fold + sort per group of objects
+        const bool shared = opt.shared_times && c.path == SS_PATH_WARP && c.variant < WARP_VARIANT_F32;      // one fold + sort per group of objects
         const int64_t n_items = (shared ? ((int64_t)p.n_list + SHARED_TIMES_M - 1) / SHARED_TIMES_M : (int64_t)p.n_list) * cpo;
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;

@@ -154,9 +154,22 @@ ss_status_t launch_block_debug(const EvalParams& p, bool opt, double f, double* 
 SS_DECL(0, 0) SS_DECL(0, 1) SS_DECL(0, 2) SS_DECL(1, 0) SS_DECL(1, 1) SS_DECL(1, 2)
 #undef SS_DECL
 
+#define SS_DECL(gv, g) ss_status_t launch_warp_f32_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
+SS_DECL(0, 0) SS_DECL(0, 1) SS_DECL(0, 2) SS_DECL(1, 0) SS_DECL(1, 1) SS_DECL(1, 2)
+#undef SS_DECL
+
 ss_status_t launch_warp_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
 {
+    const bool f32 = variant >= WARP_VARIANT_F32;
+    if (f32) variant -= WARP_VARIANT_F32;
     const int c = variant / 8, g = c <= 4 ? 0 : (c <= 6 ? 1 : 2);
+    if (f32) {
+        if (p.mode == 1)
+            return g == 0 ? launch_warp_f32_tu_1_0(p, variant, n_items, stream)
+                 : g == 1 ? launch_warp_f32_tu_1_1(p, variant, n_items, stream) : launch_warp_f32_tu_1_2(p, variant, n_items, stream);
+        return g == 0 ? launch_warp_f32_tu_0_0(p, variant, n_items, stream)
+             : g == 1 ? launch_warp_f32_tu_0_1(p, variant, n_items, stream) : launch_warp_f32_tu_0_2(p, variant, n_items, stream);
+    }
     if (p.mode == 1)
         return g == 0 ? launch_warp_tu_1_0(p, variant, n_items, stream)
              : g == 1 ? launch_warp_tu_1_1(p, variant, n_items, stream) : launch_warp_tu_1_2(p, variant, n_items, stream);

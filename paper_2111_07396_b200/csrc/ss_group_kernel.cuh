@@ -26,85 +26,6 @@
 
 namespace ss {
 
-template <typename T> struct Real;
-template <> struct Real<double> {
-    using vec2 = double2;
-    static constexpr int WORDS = 2;             // 32-bit tensor-memory columns per value
-    static constexpr int TINY = 0x00100000;     // high word of the smallest normal
-    static __device__ __forceinline__ double2 make2(double a, double b) { return make_double2(a, b); }
-    static __device__ __forceinline__ double rcp(double x) { return rcp64(x); }
-    static __device__ __forceinline__ double sqrt0(double x) { return sqrt64(x); }
-    static __device__ __forceinline__ double wpad() { return W_PAD; }
-    static __device__ __forceinline__ int hi_word(double a) { return __double2hiint(a); }
-};
-template <> struct Real<float> {
-    using vec2 = float2;
-    static constexpr int WORDS = 1;
-    static constexpr int TINY = 0x00800000;
-    static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
-    static __device__ __forceinline__ float rcp(float x) { return __frcp_rn(x); }
-    static __device__ __forceinline__ float sqrt0(float x) { return x > 0.0f ? sqrtf(x) : 0.0f; }
-    static __device__ __forceinline__ float wpad() { return 1.0e-30f; }
-    static __device__ __forceinline__ int hi_word(float a) { return __float_as_int(a); }
-};
-
-// parked values in tensor memory: doubles take two columns, floats one (arrays padded to an even number of columns)
-template <typename T, int N> struct TmemArr;
-template <int N> struct TmemArr<double, N> {
-    static constexpr uint32_t COLS = 2 * N;
-    static __device__ __forceinline__ void park(uint32_t a, const double (&v)[N]) { tmem_park<N>(a, v); }
-    static __device__ __forceinline__ void fetch(uint32_t a, double (&v)[N]) { tmem_fetch<N>(a, v); }
-};
-template <int N> struct TmemArr<float, N> {
-    static constexpr int NE = (N + 1) & ~1;
-    static constexpr uint32_t COLS = NE;
-    static __device__ __forceinline__ void park(uint32_t a, const float (&v)[N])
-    {
-        int w[N];
-#pragma unroll
-        for (int i = 0; i < N; i++) w[i] = __float_as_int(v[i]);
-        tmem_park_words<N>(a, w);
-    }
-    static __device__ __forceinline__ void fetch(uint32_t a, float (&v)[N])
-    {
-        int w[NE];
-        tmem_fetch_words<NE>(a, w);
-#pragma unroll
-        for (int i = 0; i < N; i++) v[i] = __int_as_float(w[i]);
-    }
-};
-
-// Listing 1 lines 63-77, loop-invariant tests hoisted (cf. pick_span_w), any scalar
-template <typename T>
-__device__ __forceinline__ T pick_span_t(T v0, T v1, T v2, int bass, double bexp)
-{
-    T resmin = v0, sp = (T)SPAN0;
-    if (v1 < resmin) { resmin = v1; sp = (T)SPAN1; }
-    if (v2 < resmin) { resmin = v2; sp = (T)SPAN2; }
-    if (bass != 0 && resmin < v2 && resmin > (T)0) {
-        T tmp = resmin * Real<T>::rcp(v2);
-        if (tmp < (T)1.e-7) tmp = (T)1.e-7;
-        const T pw = bass == 1 ? tmp : (T)pow((double)tmp, bexp);
-        sp += ((T)SPAN2 - sp) * pw;
-    }
-    return sp;
-}
-// Listing 1 lines 83-95 (R10), any scalar
-template <typename T>
-__device__ __forceinline__ T interp_spans_t(T sps, T A0, T A1, T A2)
-{
-    if (sps <= (T)SPAN0) sps = (T)SPAN0;
-    if (sps >= (T)SPAN2) sps = (T)SPAN2;
-    T f = sps - (T)SPAN1;
-    constexpr double G0 = 1.0 / (SPAN0 - SPAN1), G2 = 1.0 / (SPAN2 - SPAN1);
-    if (f < (T)0) {
-        f *= (T)G0;
-        return ((T)1 - f) * A1 + f * A0;
-    }
-    f *= (T)G2;
-    return ((T)1 - f) * A1 + f * A2;
-}
-
 template <int G, int C, typename T = double> struct GroupCfg {
     static constexpr int NT = 32 * G;               // threads
     static constexpr int NP = NT * C;               // capacity in points

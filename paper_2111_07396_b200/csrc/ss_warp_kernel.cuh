@@ -21,7 +21,7 @@ namespace ss {
 
 // Launch shape per points-per-lane: warps per CTA and resident CTAs per SM (register budget =
 // 65536 / (32 * WPC * MINB), rounded down to a multiple of 8).
-template <int C, bool GV> struct WarpCfg {
+template <int C, bool GV, typename T = double> struct WarpCfg {
     // each shape chosen by measurement on config 3:
     //   GV: C <= 4: 4 warps x 5 CTAs (20 warps/SM,  96 registers);  C >= 5: 4 x 3 (12 warps, 168)
     //   CV: C <= 3: 4 x 5 (20 warps/SM, 96 registers: +2.6 % over 16 warps, round 2);  C = 4..6: 8 warps x 2 CTAs (16 warps/SM,
@@ -29,6 +29,17 @@ template <int C, bool GV> struct WarpCfg {
     //       C = 8: 8 x 1 (255)
     static constexpr int WPC = GV ? 4 : ((C == 7 || C <= 3) ? 4 : 8);
     static constexpr int MINB = GV ? (C <= 4 ? 5 : 3) : (C <= 3 ? 5 : (C <= 6 ? 2 : (C == 7 ? 3 : 1)));
+};
+// MIXED precision (T = float: half the registers, tensor-memory columns and shared memory per eval): 4 warps per CTA,
+//   C <= 4: 8 CTAs (32 warps/SM, 64 registers);  C = 5..6: 6 CTAs (24 warps, 80);  C = 7..8: 4 CTAs (16 warps, 128)
+template <int C, bool GV> struct WarpCfg<C, GV, float> {
+#ifndef SS_F32_MINB_A
+#define SS_F32_MINB_A 4
+#define SS_F32_MINB_B 3
+#define SS_F32_MINB_C 2
+#endif
+    static constexpr int WPC = 8;
+    static constexpr int MINB = C <= 4 ? SS_F32_MINB_A : (C <= 6 ? SS_F32_MINB_B : SS_F32_MINB_C);
 };
 constexpr int WROW = 33;   // row length of the transposed prefix arrays (32 lanes + the total)
 constexpr double W_PAD = 1.0e-300;   // weight of the padded slots j >= n: keeps every window sum > 0
@@ -38,6 +49,10 @@ template <int C> struct Pow2Ceil { static constexpr int value = C <= 2 ? 2 : (C 
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 __device__ __forceinline__ double shfl_up_d(double v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
 __device__ __forceinline__ double shfl_down_d(double v, int d) { return __shfl_down_sync(0xffffffffu, v, d); }
+
+template <typename T> __device__ __forceinline__ T shfl_v(T v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+template <typename T> __device__ __forceinline__ T shfl_up_v(T v, int d) { return __shfl_up_sync(0xffffffffu, v, d); }
+template <typename T> __device__ __forceinline__ T shfl_down_v(T v, int d) { return __shfl_down_sync(0xffffffffu, v, d); }
 
 template <int C>
 __device__ __forceinline__ int wst(int e) { return (e % C) * WROW + e / C; }
@@ -57,42 +72,92 @@ __device__ __forceinline__ void scan_step(double& inc, int i, const ScanMask& mk
     inc = fma(shfl_up_d(inc, 1 << i), mk.m[i], inc);
 }
 
+// sqrt(v) for v >= 0: MUFU.RSQ64H seed and two coupled Newton steps (Goldschmidt), ~1 ulp; 0 for v <= 0.
+__device__ __forceinline__ double sqrt64(double v)
+{
+    double r;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(v));
+    double g = v * r, h = 0.5 * r;
+    double e = fma(-h, g, 0.5);
+    g = fma(g, e, g); h = fma(h, e, h);
+    e = fma(-h, g, 0.5);
+    g = fma(g, e, g);
+    return v > 0.0 ? g : 0.0;
+}
+
+// Scalar traits of the smoother ("toggle between using FP32 or FP64"): T = double is the
+// library's default; T = float is the MIXED mode (ss_options_t::precision), see the note at warp_eval_body.
+template <typename T> struct Real;
+template <> struct Real<double> {
+    using vec2 = double2;
+    static constexpr int WORDS = 2;             // 32-bit tensor-memory columns per value
+    static constexpr int TINY = 0x00100000;     // high word of the smallest normal
+    static __device__ __forceinline__ double2 make2(double a, double b) { return make_double2(a, b); }
+    static __device__ __forceinline__ double rcp(double x) { return rcp64(x); }
+    static __device__ __forceinline__ double sqrt0(double x) { return sqrt64(x); }
+    static __device__ __forceinline__ double wpad() { return W_PAD; }
+    static __device__ __forceinline__ int hi_word(double a) { return __double2hiint(a); }
+};
+template <> struct Real<float> {
+    using vec2 = float2;
+    static constexpr int WORDS = 1;
+    static constexpr int TINY = 0x00800000;
+    static __device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
+    // one MUFU each (1 ulp): the mode's error budget is the fp32 prefix differences, ~1e-5 relative
+    static __device__ __forceinline__ float rcp(float x)
+    {
+        float r;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return r;
+    }
+    static __device__ __forceinline__ float sqrt0(float x)
+    {
+        float r;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+        return x > 0.0f ? r : 0.0f;
+    }
+    static __device__ __forceinline__ float wpad() { return 1.0e-30f; }
+    static __device__ __forceinline__ int hi_word(float a) { return __float_as_int(a); }
+};
+
 // Warp-wide exclusive prefix sums of two arrays at once (C values per lane, blocked), written
-// interleaved as double2 and transposed: E[wst(j)] = (sum_{i<j} a_i, sum_{i<j} b_i), j = 0..32C.
-template <int C>
-__device__ __forceinline__ void pair_prefix_store(const double (&a)[C], const double (&b)[C], double2* E, int lane,
+// interleaved as double2 (float2) and transposed: E[wst(j)] = (sum_{i<j} a_i, sum_{i<j} b_i), j = 0..32C.
+// T = float: the lane's own C values are summed in fp32, the scan across lanes runs in fp64 and its result is rounded
+// once per lane (two conversions per lane and stream).
+template <int C, typename T>
+__device__ __forceinline__ void pair_prefix_store(const T (&a)[C], const T (&b)[C], typename Real<T>::vec2* E, int lane,
                                                   const ScanMask& mk)
 {
-    double ra = a[0], rb = b[0];
+    T ra = a[0], rb = b[0];
 #pragma unroll
     for (int s = 1; s < C; s++) { ra += a[s]; rb += b[s]; }
     double ia = ra, ib = rb;
 #pragma unroll
     for (int i = 0; i < 5; i++) { scan_step(ia, i, mk); scan_step(ib, i, mk); }
     // exclusive prefixes are re-accumulated from the lane's offset (no second register array)
-    double xa = ia - ra, xb = ib - rb;
+    T xa = (T)(ia - ra), xb = (T)(ib - rb);
 #pragma unroll
     for (int s = 0; s < C; s++) {
-        E[s * WROW + lane] = make_double2(xa, xb);
+        E[s * WROW + lane] = Real<T>::make2(xa, xb);
         xa += a[s]; xb += b[s];
     }
-    if (lane == 31) E[32] = make_double2(ia, ib);     // E[32*C] lives at row 0, column 32
+    if (lane == 31) E[32] = Real<T>::make2((T)ia, (T)ib);     // E[32*C] lives at row 0, column 32
 }
 
-// One array: E[wst(j)] = sum_{i<j} a_i as plain doubles (row length WROW doubles).
-template <int C>
-__device__ __forceinline__ void single_prefix_store(const double (&a)[C], double* E, int lane, const ScanMask& mk)
+// One array: E[wst(j)] = sum_{i<j} a_i as plain scalars (row length WROW).
+template <int C, typename T>
+__device__ __forceinline__ void single_prefix_store(const T (&a)[C], T* E, int lane, const ScanMask& mk)
 {
-    double ra = a[0];
+    T ra = a[0];
 #pragma unroll
     for (int s = 1; s < C; s++) ra += a[s];
     double ia = ra;
 #pragma unroll
     for (int i = 0; i < 5; i++) scan_step(ia, i, mk);
-    double xa = ia - ra;
+    T xa = (T)(ia - ra);
 #pragma unroll
     for (int s = 0; s < C; s++) { E[s * WROW + lane] = xa; xa += a[s]; }
-    if (lane == 31) E[32] = ia;
+    if (lane == 31) E[32] = (T)ia;
 }
 
 __device__ __forceinline__ void cex32(unsigned& a, unsigned& b)
@@ -197,15 +262,15 @@ __device__ __forceinline__ void warp_sort_any(unsigned (&key)[C], int lane)
 }
 
 // Halo of one register array: u[t] = element at j = lane*C - IBW0 + t (fill outside 0..32C-1).
-template <int C, int IBW0, bool FILL = true>
-__device__ __forceinline__ void make_halo(const double (&v)[C], double (&u)[C + 2 * IBW0], int lane, double fill)
+template <int C, int IBW0, bool FILL = true, typename T>
+__device__ __forceinline__ void make_halo(const T (&v)[C], T (&u)[C + 2 * IBW0], int lane, T fill)
 {
     static_assert(IBW0 <= C, "halo reaches one lane to either side");
 #pragma unroll
     for (int t = 0; t < IBW0; t++) {
-        double l = shfl_up_d(v[C - IBW0 + t], 1);
+        T l = shfl_up_v(v[C - IBW0 + t], 1);
         u[t] = (FILL && lane == 0) ? fill : l;
-        double r = shfl_down_d(v[t], 1);
+        T r = shfl_down_v(v[t], 1);
         u[IBW0 + C + t] = (FILL && lane == 31) ? fill : r;
     }
 #pragma unroll
@@ -214,10 +279,10 @@ __device__ __forceinline__ void make_halo(const double (&v)[C], double (&u)[C + 
 
 // Sums of e over the 2*IBW0+1 halo elements around each of the lane's C points, by sliding:
 // out[0] = e[0] + .. + e[2*IBW0]; out[s] = out[s-1] + e[s + 2*IBW0] - e[s-1].
-template <int C, int IBW0>
-__device__ __forceinline__ void slide_sums(const double (&e)[C + 2 * IBW0], double (&out)[C])
+template <int C, int IBW0, typename T>
+__device__ __forceinline__ void slide_sums(const T (&e)[C + 2 * IBW0], T (&out)[C])
 {
-    double acc = e[0];
+    T acc = e[0];
 #pragma unroll
     for (int t = 1; t <= 2 * IBW0; t++) acc += e[t];
     out[0] = acc;
@@ -227,27 +292,14 @@ __device__ __forceinline__ void slide_sums(const double (&e)[C + 2 * IBW0], doub
 
 // Value of register slot `slot` (warp-uniform, run time) of lane `src`, without a select chain:
 // the uniform branch picks the one shuffle that runs.
-template <int C>
-__device__ __forceinline__ double bcast_slot(const double (&a)[C], int slot, int src)
+template <int C, typename T>
+__device__ __forceinline__ T bcast_slot(const T (&a)[C], int slot, int src)
 {
-    double v = 0.0;
+    T v = (T)0;
 #pragma unroll
     for (int s = 0; s < C; s++)
-        if (slot == s) v = shfl_d(a[s], src);
+        if (slot == s) v = shfl_v(a[s], src);
     return v;
-}
-
-// sqrt(v) for v >= 0: MUFU.RSQ64H seed and two coupled Newton steps (Goldschmidt), ~1 ulp; 0 for v <= 0.
-__device__ __forceinline__ double sqrt64(double v)
-{
-    double r;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(v));
-    double g = v * r, h = 0.5 * r;
-    double e = fma(-h, g, 0.5);
-    g = fma(g, e, g); h = fma(h, e, h);
-    e = fma(-h, g, 0.5);
-    g = fma(g, e, g);
-    return v > 0.0 ? g : 0.0;
 }
 
 // ---- Tensor memory as a per-thread parking area -------------------------------------------------
@@ -371,13 +423,99 @@ __device__ __forceinline__ void tmem_fetch_words_any(uint32_t taddr, int (&v)[N]
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
+// parked values in tensor memory: doubles take two columns, floats one (arrays padded to an even number of columns)
+template <typename T, int N> struct TmemArr;
+template <int N> struct TmemArr<double, N> {
+    static constexpr uint32_t COLS = 2 * N;
+    static __device__ __forceinline__ void park(uint32_t a, const double (&v)[N]) { tmem_park<N>(a, v); }
+    static __device__ __forceinline__ void fetch(uint32_t a, double (&v)[N]) { tmem_fetch<N>(a, v); }
+};
+template <int N> struct TmemArr<float, N> {
+    static constexpr int NE = (N + 1) & ~1;
+    static constexpr uint32_t COLS = NE;
+    static __device__ __forceinline__ void park(uint32_t a, const float (&v)[N])
+    {
+        int w[N];
+#pragma unroll
+        for (int i = 0; i < N; i++) w[i] = __float_as_int(v[i]);
+        tmem_park_words<N>(a, w);
+    }
+    static __device__ __forceinline__ void fetch(uint32_t a, float (&v)[N])
+    {
+        int w[NE];
+        tmem_fetch_words<NE>(a, w);
+#pragma unroll
+        for (int i = 0; i < N; i++) v[i] = __int_as_float(w[i]);
+    }
+};
+
+// Window ends (lo[C], hi[C] element indices into a transposed prefix array) of one span in tensor memory: 2C words in
+// fp64 (round 1's layout); with T = float the two indices of a point (< 65536) share a word: C words, padded to even.
+template <typename T, int C> struct WinTab;
+template <int C> struct WinTab<double, C> {
+    static constexpr uint32_t COLS = 2 * C;
+    static __device__ __forceinline__ void park(uint32_t a, const int (&w)[2 * C]) { tmem_park_words<2 * C>(a, w); }
+    static __device__ __forceinline__ void fetch(uint32_t a, int (&w)[2 * C]) { tmem_fetch_words<2 * C>(a, w); }
+};
+template <int C> struct WinTab<float, C> {
+    static constexpr int CE = (C + 1) & ~1;
+    static constexpr uint32_t COLS = CE;
+    static __device__ __forceinline__ void park(uint32_t a, const int (&w)[2 * C])
+    {
+        int t[CE];
+#pragma unroll
+        for (int s = 0; s < CE; s++) t[s] = s < C ? (w[s < C ? s : 0] | (w[C + (s < C ? s : 0)] << 16)) : 0;
+        tmem_park_words<CE>(a, t);
+    }
+    static __device__ __forceinline__ void fetch(uint32_t a, int (&w)[2 * C])
+    {
+        int t[CE];
+        tmem_fetch_words<CE>(a, t);
+#pragma unroll
+        for (int s = 0; s < C; s++) { w[s] = t[s] & 0xffff; w[C + s] = (int)((unsigned)t[s] >> 16); }
+    }
+};
+
+// Listing 1 lines 63-77, loop-invariant tests hoisted (cf. pick_span_w), any scalar
+template <typename T>
+__device__ __forceinline__ T pick_span_t(T v0, T v1, T v2, int bass, double bexp)
+{
+    T resmin = v0, sp = (T)SPAN0;
+    if (v1 < resmin) { resmin = v1; sp = (T)SPAN1; }
+    if (v2 < resmin) { resmin = v2; sp = (T)SPAN2; }
+    if (bass != 0 && resmin < v2 && resmin > (T)0) {
+        T tmp = resmin * Real<T>::rcp(v2);
+        if (tmp < (T)1.e-7) tmp = (T)1.e-7;
+        const T pw = bass == 1 ? tmp : (T)pow((double)tmp, bexp);
+        sp += ((T)SPAN2 - sp) * pw;
+    }
+    return sp;
+}
+// Listing 1 lines 83-95 (R10), any scalar
+template <typename T>
+__device__ __forceinline__ T interp_spans_t(T sps, T A0, T A1, T A2)
+{
+    if (sps <= (T)SPAN0) sps = (T)SPAN0;
+    if (sps >= (T)SPAN2) sps = (T)SPAN2;
+    T f = sps - (T)SPAN1;
+    constexpr double G0 = 1.0 / (SPAN0 - SPAN1), G2 = 1.0 / (SPAN2 - SPAN1);
+    if (f < (T)0) {
+        f *= (T)G0;
+        return ((T)1 - f) * A1 + f * A0;
+    }
+    f *= (T)G2;
+    return ((T)1 - f) * A1 + f * A2;
+}
+
 // Per-warp view of the shared memory.
-struct WarpMem {
-    const double* tt; const double* yc; const double* w;   // the object's arrays (CTA-wide)
-    double2* E;              // per-warp: 3 pair-prefix arrays of C*WROW double2
+template <typename T> struct WarpMemT {
+    const double* tt;        // the object's times (CTA-wide), always fp64: the fold needs them
+    const T* yc; const T* w; // centred magnitudes and weights (CTA-wide)
+    typename Real<T>::vec2* E;   // per-warp: 3 pair-prefix arrays of C*WROW pairs
     uint32_t tmem;           // per-warp tensor-memory base (lane quarter + first column), CV only
     ScanMask mk;             // Kogge-Stone masks of this lane
 };
+using WarpMem = WarpMemT<double>;
 
 // Per-object constants of the eval loop (warp-uniform).
 struct EvalConst {
@@ -405,54 +543,72 @@ __device__ __forceinline__ double pick_span_w(double v0, double v1, double v2, c
     return sp;
 }
 
+template <typename T> __device__ __forceinline__ T pick_span_k(T v0, T v1, T v2, const EvalConst& K)
+{
+    if constexpr (sizeof(T) == 8) return pick_span_w(v0, v1, v2, K);
+    else return pick_span_t<T>(v0, v1, v2, K.bass, K.bexp);
+}
+template <typename T> __device__ __forceinline__ T interp_k(T sps, T A0, T A1, T A2)
+{
+    if constexpr (sizeof(T) == 8) return interp_spans(sps, A0, A1, A2);
+    else return interp_spans_t<T>(sps, A0, A1, A2);
+}
+
 // Smoother + statistic on the sorted, gathered eval (x centred by 0.5, y centred by ybar_w).
 // Padded slots (j >= n) carry x = 0, y = 0, w = W_PAD.
-template <int C, int IBW0, bool GV>
-__device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpMem& M, const double (&x)[C],
-                                                 const double (&y)[C], const double (&w)[C], double vsmlsq,
+//
+// T = float (MIXED precision): the caller folds, sorts and centres in fp64 and hands over x, y, w rounded to fp32; the
+// scans across lanes accumulate in fp64 (pair_prefix_store), everything else -- window fits, residuals, span pick,
+// interpolation, the lane's part of chi2 -- is fp32.  The tweeter's direct, centred window sums lose nothing to
+// cancellation; the midrange / woofer prefix differences keep ~5 digits of sxx at n <= 256.
+template <int C, int IBW0, bool GV, typename T>
+__device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpMemT<T>& M, const T (&x)[C],
+                                                 const T (&y)[C], const T (&w)[C], T vsmlsq,
                                                  int lane, bool& defer)
 {
+    using V2 = typename Real<T>::vec2;
+    constexpr uint32_t PC = TmemArr<T, C>::COLS;      // tensor-memory columns of one parked array
     constexpr int ASZ = C * WROW;
     constexpr int H = C + 2 * IBW0;
     constexpr int K0 = 2 * IBW0 + 1;
     const int n = K.n;
-    double2* E01 = M.E;             // (w, wx)
-    double2* E23 = M.E + ASZ;       // (wxx, wy)
-    double2* E45 = M.E + 2 * ASZ;   // (wxy, wyy)
+    V2* E01 = M.E;             // (w, wx)
+    V2* E23 = M.E + ASZ;       // (wxx, wy)
+    V2* E45 = M.E + 2 * ASZ;   // (wxy, wyy)
 
     // ---- prefix sums of the weighted moments (midrange and woofer windows)
     {
-        double a[C], b[C], c[C];
+        T a[C], b[C], c[C];
 #pragma unroll
         for (int s = 0; s < C; s++) { a[s] = w[s]; b[s] = w[s] * x[s]; }
-        pair_prefix_store<C>(a, b, E01, lane, M.mk);
+        pair_prefix_store<C, T>(a, b, E01, lane, M.mk);
 #pragma unroll
         for (int s = 0; s < C; s++) { c[s] = b[s] * x[s]; a[s] = w[s] * y[s]; }
-        pair_prefix_store<C>(c, a, E23, lane, M.mk);
+        pair_prefix_store<C, T>(c, a, E23, lane, M.mk);
 #pragma unroll
         for (int s = 0; s < C; s++) b[s] = b[s] * y[s];
         if (GV) {
 #pragma unroll
             for (int s = 0; s < C; s++) c[s] = a[s] * y[s];
-            pair_prefix_store<C>(b, c, E45, lane, M.mk);
+            pair_prefix_store<C, T>(b, c, E45, lane, M.mk);
         } else {
-            single_prefix_store<C>(b, reinterpret_cast<double*>(E45), lane, M.mk);   // CV: wxy only
+            single_prefix_store<C, T>(b, reinterpret_cast<T*>(E45), lane, M.mk);   // CV: wxy only
         }
     }
     __syncwarp();
 
     // ---- tweeter: window sums about the lane's first point from neighbour-lane halos, sliding
-    double t_isw[C], t_xb[C], t_isxx[C], t_zb[C], t_b[C], t_g[C];
+    T t_isw[C], t_xb[C], t_isxx[C], t_zb[C], t_b[C], t_g[C];
     {
-        double ux[H], uw[H], uy[H];
+        T ux[H], uw[H], uy[H];
         // only the weights need the zero fill outside 0..32C-1: x and y there are finite and multiply w = 0
-        make_halo<C, IBW0, false>(x, ux, lane, 0.0);
-        make_halo<C, IBW0>(w, uw, lane, 0.0);
-        make_halo<C, IBW0, false>(y, uy, lane, 0.0);
-        const double c0 = x[0];
-        double m0[C], m1[C], m2[C], mz[C], m1z[C], mzz[C];
+        make_halo<C, IBW0, false>(x, ux, lane, (T)0);
+        make_halo<C, IBW0>(w, uw, lane, (T)0);
+        make_halo<C, IBW0, false>(y, uy, lane, (T)0);
+        const T c0 = x[0];
+        T m0[C], m1[C], m2[C], mz[C], m1z[C], mzz[C];
         slide_sums<C, IBW0>(uw, m0);
-        double e1[H], e2[H];
+        T e1[H], e2[H];
 #pragma unroll
         for (int t = 0; t < H; t++) { ux[t] -= c0; e1[t] = uw[t] * ux[t]; }
         slide_sums<C, IBW0>(e1, m1);
@@ -472,18 +628,18 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
         }
 #pragma unroll
         for (int s = 0; s < C; s++) {
-            const double isw = rcp64(m0[s]);
-            const double xr = m1[s] * isw;              // xbar relative to c0
-            const double sxx = m2[s] - xr * m1[s];
-            const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-            const double zb = mz[s] * isw;
-            const double sxz = m1z[s] - xr * mz[s];
-            const double b = sxz * isxx;
+            const T isw = Real<T>::rcp(m0[s]);
+            const T xr = m1[s] * isw;              // xbar relative to c0
+            const T sxx = m2[s] - xr * m1[s];
+            const T isxx = sxx > vsmlsq ? Real<T>::rcp(sxx) : (T)0;
+            const T zb = mz[s] * isw;
+            const T sxz = m1z[s] - xr * mz[s];
+            const T b = sxz * isxx;
             t_isw[s] = isw; t_xb[s] = c0 + xr; t_isxx[s] = isxx; t_zb[s] = zb; t_b[s] = b;
             if (GV) {
-                double rss = (mzz[s] - zb * mz[s]) - b * sxz;
-                constexpr double G1 = 1.0 / (1.0 - 1.0 / (double)K0), G2 = 1.0 / (1.0 - 2.0 / (double)K0);
-                t_g[s] = sqrt64(rss * isw) * (isxx != 0.0 ? G2 : G1);
+                T rss = (mzz[s] - zb * mz[s]) - b * sxz;
+                constexpr T G1 = (T)(1.0 / (1.0 - 1.0 / (double)K0)), G2 = (T)(1.0 / (1.0 - 2.0 / (double)K0));
+                t_g[s] = Real<T>::sqrt0(rss * isw) * (isxx != (T)0 ? G2 : G1);
             }
         }
     }
@@ -496,8 +652,8 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
 #define SS_CLAMP(arr)                                                                     \
         {                                                                                 \
             /* IBW0 < C: the left owner is a slot of lane 0 itself, no shuffle */         \
-            const double vl = LL == 0 ? arr[LS] : shfl_d(arr[LS], LL);                    \
-            const double vr = bcast_slot<C>(arr, sr, lr);                                 \
+            const T vl = LL == 0 ? arr[LS] : shfl_v(arr[LS], LL);                    \
+            const T vr = bcast_slot<C>(arr, sr, lr);                                 \
             _Pragma("unroll") for (int s = 0; s < C; s++) {                               \
                 const int j = lane * C + s;                                               \
                 if (s < IBW0 && j < IBW0) arr[s] = vl;                                    \
@@ -510,172 +666,172 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
 
     // window indices (transposed storage) are loop-invariant: computed once per CTA, parked in tensor
     // memory at columns [14C, 16C) (midrange lo, hi) and [16C, 18C) (woofer lo, hi)
-    constexpr uint32_t TW1 = GV ? 0 : 14 * C, TW2 = TW1 + 2 * C;   // GV parks nothing else
-    double chi2 = 0.0;
+    constexpr uint32_t TW1 = GV ? 0 : 7 * PC, TW2 = TW1 + WinTab<T, C>::COLS;   // GV parks nothing else
+    T chi2 = 0.0;
     if (GV) {
         // ---- O6: scores, pick, interpolate
         int w1[2 * C], w2[2 * C];
-        tmem_fetch_words<2 * C>(M.tmem + TW1, w1);
-        tmem_fetch_words<2 * C>(M.tmem + TW2, w2);
+        WinTab<T, C>::fetch(M.tmem + TW1, w1);
+        WinTab<T, C>::fetch(M.tmem + TW2, w2);
 #pragma unroll
         for (int s = 0; s < C; s++) {
-            const double xj = x[s];
-            const double A0 = t_zb[s] + t_b[s] * (xj - t_xb[s]);
-            double A1, A2, G1, G2;
+            const T xj = x[s];
+            const T A0 = t_zb[s] + t_b[s] * (xj - t_xb[s]);
+            T A1, A2, G1, G2;
             {
-                const double2 l0 = E01[w1[s]], h0 = E01[w1[C + s]], l1 = E23[w1[s]], h1 = E23[w1[C + s]];
-                const double2 l2 = E45[w1[s]], h2 = E45[w1[C + s]];
-                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
-                const double isw = rcp64(Sw), xb = Swx * isw;
-                const double sxx = Swxx - xb * Swx;
-                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
+                const V2 l0 = E01[w1[s]], h0 = E01[w1[C + s]], l1 = E23[w1[s]], h1 = E23[w1[C + s]];
+                const V2 l2 = E45[w1[s]], h2 = E45[w1[C + s]];
+                const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                const T isw = Real<T>::rcp(Sw), xb = Swx * isw;
+                const T sxx = Swxx - xb * Swx;
+                const T isxx = sxx > vsmlsq ? Real<T>::rcp(sxx) : (T)0;
+                const T yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
                 A1 = yb + b * (xj - xb);
-                const double rss = (Syy - yb * Sy) - b * sxy;
-                G1 = sqrt64(rss * isw) * (isxx != 0.0 ? K.kc[1] : K.kc[0]);
+                const T rss = (Syy - yb * Sy) - b * sxy;
+                G1 = Real<T>::sqrt0(rss * isw) * (isxx != (T)0 ? (T)K.kc[1] : (T)K.kc[0]);
             }
             {
                 const int a2 = w2[s], b2 = w2[C + s];
-                const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2], l2 = E45[a2], h2 = E45[b2];
-                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                const double Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
-                const double isw = rcp64(Sw), xb = Swx * isw;
-                const double sxx = Swxx - xb * Swx;
-                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                const double yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
+                const V2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2], l2 = E45[a2], h2 = E45[b2];
+                const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                const T isw = Real<T>::rcp(Sw), xb = Swx * isw;
+                const T sxx = Swxx - xb * Swx;
+                const T isxx = sxx > vsmlsq ? Real<T>::rcp(sxx) : (T)0;
+                const T yb = Sy * isw, sxy = Sxy - xb * Sy, b = sxy * isxx;
                 A2 = yb + b * (xj - xb);
-                const double rss = (Syy - yb * Sy) - b * sxy;
-                G2 = sqrt64(rss * isw) * (isxx != 0.0 ? K.kc[3] : K.kc[2]);
+                const T rss = (Syy - yb * Sy) - b * sxy;
+                G2 = Real<T>::sqrt0(rss * isw) * (isxx != (T)0 ? (T)K.kc[3] : (T)K.kc[2]);
             }
-            const double sp = pick_span_w(t_g[s], G1, G2, K);
-            const double smo = interp_spans(sp, A0, A1, A2);
-            const double r = y[s] - smo;
+            const T sp = pick_span_k<T>(t_g[s], G1, G2, K);
+            const T smo = interp_k<T>(sp, A0, A1, A2);
+            const T r = y[s] - smo;
             chi2 += w[s] * r * r;
         }
     } else {
         // ---- CV pass 1, one span at a time; each smooth is parked in tensor memory
         // as soon as it exists (it is needed again only at the interpolation), so are the tweeter
         // x-moments (needed again by the final smooth) and y (needed again by the statistic)
-        double r0[C], r1[C], r2[C];
-        double m_isw[C], m_xb[C], m_g[C];      // midrange x-moments, reused by four more smooths
-        const double* E4 = reinterpret_cast<const double*>(E45);
+        T r0[C], r1[C], r2[C];
+        T m_isw[C], m_xb[C], m_g[C];      // midrange x-moments, reused by four more smooths
+        const T* E4 = reinterpret_cast<const T*>(E45);
         int amin = 0x7fffffff;                 // smallest high word of the three LOO denominators
         {
-            double A0[C];
+            T A0[C];
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double dx = x[s] - t_xb[s];
+                const T dx = x[s] - t_xb[s];
                 A0[s] = t_zb[s] + t_b[s] * dx;
-                const double a = 1.0 - w[s] * (t_isw[s] + dx * dx * t_isxx[s]);
-                r0[s] = fabs(y[s] - A0[s]) * rcp64(a);
-                amin = min(amin, __double2hiint(a));
+                const T a = (T)1 - w[s] * (t_isw[s] + dx * dx * t_isxx[s]);
+                r0[s] = fabs(y[s] - A0[s]) * Real<T>::rcp(a);
+                amin = min(amin, Real<T>::hi_word(a));
             }
-            tmem_park<C>(M.tmem, A0);
-            tmem_park<C>(M.tmem + 6 * C, t_isw); tmem_park<C>(M.tmem + 8 * C, t_xb); tmem_park<C>(M.tmem + 10 * C, t_isxx);
+            TmemArr<T, C>::park(M.tmem, A0);
+            TmemArr<T, C>::park(M.tmem + 3 * PC, t_isw); TmemArr<T, C>::park(M.tmem + 4 * PC, t_xb); TmemArr<T, C>::park(M.tmem + 5 * PC, t_isxx);
         }
         {
-            double A1[C];
+            T A1[C];
             int w1[2 * C];
-            tmem_fetch_words<2 * C>(M.tmem + TW1, w1);
+            WinTab<T, C>::fetch(M.tmem + TW1, w1);
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double2 l0 = E01[w1[s]], h0 = E01[w1[C + s]], l1 = E23[w1[s]], h1 = E23[w1[C + s]];
-                const double lxy = E4[w1[s]], hxy = E4[w1[C + s]];
-                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                const double Sxy = hxy - lxy;
-                const double isw = rcp64(Sw), xb = Swx * isw;
-                const double sxx = Swxx - xb * Swx;
-                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                const double dx = x[s] - xb;
+                const V2 l0 = E01[w1[s]], h0 = E01[w1[C + s]], l1 = E23[w1[s]], h1 = E23[w1[C + s]];
+                const T lxy = E4[w1[s]], hxy = E4[w1[C + s]];
+                const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const T Sxy = hxy - lxy;
+                const T isw = Real<T>::rcp(Sw), xb = Swx * isw;
+                const T sxx = Swxx - xb * Swx;
+                const T isxx = sxx > vsmlsq ? Real<T>::rcp(sxx) : (T)0;
+                const T dx = x[s] - xb;
                 m_isw[s] = isw; m_xb[s] = xb; m_g[s] = isxx * dx;
                 A1[s] = Sy * isw + (Sxy - xb * Sy) * m_g[s];
-                const double a = 1.0 - w[s] * (isw + dx * m_g[s]);
-                r1[s] = fabs(y[s] - A1[s]) * rcp64(a);
-                amin = min(amin, __double2hiint(a));
+                const T a = (T)1 - w[s] * (isw + dx * m_g[s]);
+                r1[s] = fabs(y[s] - A1[s]) * Real<T>::rcp(a);
+                amin = min(amin, Real<T>::hi_word(a));
             }
-            tmem_park<C>(M.tmem + 2 * C, A1);
+            TmemArr<T, C>::park(M.tmem + 1 * PC, A1);
         }
         {
-            double A2[C];
+            T A2[C];
             int w2[2 * C];
-            tmem_fetch_words<2 * C>(M.tmem + TW2, w2);
+            WinTab<T, C>::fetch(M.tmem + TW2, w2);
 #pragma unroll
             for (int s = 0; s < C; s++) {
                 const int a2 = w2[s], b2 = w2[C + s];
-                const double2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2];
-                const double lxy = E4[a2], hxy = E4[b2];
-                const double Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                const double Sxy = hxy - lxy;
-                const double isw = rcp64(Sw), xb = Swx * isw;
-                const double sxx = Swxx - xb * Swx;
-                const double isxx = sxx > vsmlsq ? rcp64(sxx) : 0.0;
-                const double dx = x[s] - xb, g = isxx * dx;
+                const V2 l0 = E01[a2], h0 = E01[b2], l1 = E23[a2], h1 = E23[b2];
+                const T lxy = E4[a2], hxy = E4[b2];
+                const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                const T Sxy = hxy - lxy;
+                const T isw = Real<T>::rcp(Sw), xb = Swx * isw;
+                const T sxx = Swxx - xb * Swx;
+                const T isxx = sxx > vsmlsq ? Real<T>::rcp(sxx) : (T)0;
+                const T dx = x[s] - xb, g = isxx * dx;
                 A2[s] = Sy * isw + (Sxy - xb * Sy) * g;
-                const double a = 1.0 - w[s] * (isw + dx * g);
-                r2[s] = fabs(y[s] - A2[s]) * rcp64(a);
-                amin = min(amin, __double2hiint(a));
+                const T a = (T)1 - w[s] * (isw + dx * g);
+                r2[s] = fabs(y[s] - A2[s]) * Real<T>::rcp(a);
+                amin = min(amin, Real<T>::hi_word(a));
             }
-            tmem_park<C>(M.tmem + 4 * C, A2);
-            tmem_park<C>(M.tmem + 12 * C, y);
+            TmemArr<T, C>::park(M.tmem + 2 * PC, A2);
+            TmemArr<T, C>::park(M.tmem + 6 * PC, y);
         }
         // a <= 0 (or below the smallest normal): the residual carries (R23) -> generic path.  Padded slots have a ~ 1.
-        if (__any_sync(0xffffffffu, amin < 0x00100000)) { defer = true; return 0.0; }
+        if (__any_sync(0xffffffffu, amin < Real<T>::TINY)) { defer = true; return 0.0; }
         __syncwarp();      // every lane is done reading the primary prefix arrays
 
         // midrange smooth of a register array z through one pair-prefix array
-        auto mid_store = [&](const double (&z)[C], double2* Ez) {
-            double a[C], b[C];
+        auto mid_store = [&](const T (&z)[C], V2* Ez) {
+            T a[C], b[C];
 #pragma unroll
             for (int s = 0; s < C; s++) { a[s] = w[s] * z[s]; b[s] = a[s] * x[s]; }
-            pair_prefix_store<C>(a, b, Ez, lane, M.mk);
+            pair_prefix_store<C, T>(a, b, Ez, lane, M.mk);
         };
-        auto mid_load = [&](const double2* Ez, double (&out)[C]) {
+        auto mid_load = [&](const V2* Ez, T (&out)[C]) {
             int w1[2 * C];
-            tmem_fetch_words<2 * C>(M.tmem + TW1, w1);
+            WinTab<T, C>::fetch(M.tmem + TW1, w1);
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double2 l = Ez[w1[s]], h = Ez[w1[C + s]];
-                const double Sz = h.x - l.x, Sxz = h.y - l.y;
+                const V2 l = Ez[w1[s]], h = Ez[w1[C + s]];
+                const T Sz = h.x - l.x, Sxz = h.y - l.y;
                 out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
             }
         };
-        double sp[C];
+        T sp[C];
         {
             mid_store(r0, E01); mid_store(r1, E23); mid_store(r2, E45);
             __syncwarp();
-            double R0[C], R1[C], R2[C];
+            T R0[C], R1[C], R2[C];
             mid_load(E01, R0); mid_load(E23, R1); mid_load(E45, R2);
             // span pick + bass enhancement
 #pragma unroll
-            for (int s = 0; s < C; s++) sp[s] = pick_span_w(R0[s], R1[s], R2[s], K);
+            for (int s = 0; s < C; s++) sp[s] = pick_span_k<T>(R0[s], R1[s], R2[s], K);
         }
         __syncwarp();
         mid_store(sp, E01);
         __syncwarp();
-        double B[C];
+        T B[C];
         mid_load(E01, B);
         tmem_wait_st();
         {
-            double a0[C], a1[C], a2[C];
-            tmem_fetch<C>(M.tmem, a0); tmem_fetch<C>(M.tmem + 2 * C, a1); tmem_fetch<C>(M.tmem + 4 * C, a2);
+            T a0[C], a1[C], a2[C];
+            TmemArr<T, C>::fetch(M.tmem, a0); TmemArr<T, C>::fetch(M.tmem + 1 * PC, a1); TmemArr<T, C>::fetch(M.tmem + 2 * PC, a2);
 #pragma unroll
-            for (int s = 0; s < C; s++) B[s] = interp_spans(B[s], a0[s], a1[s], a2[s]);
+            for (int s = 0; s < C; s++) B[s] = interp_k<T>(B[s], a0[s], a1[s], a2[s]);
         }
         // ---- final tweeter smooth: direct window sums of (wB, wxB), sliding
-        double zb[C], bb[C];
+        T zb[C], bb[C];
         {
-            double p1[C], p2[C], u[H];
+            T p1[C], p2[C], u[H];
 #pragma unroll
             for (int s = 0; s < C; s++) { p1[s] = w[s] * B[s]; p2[s] = p1[s] * x[s]; }
-            make_halo<C, IBW0>(p1, u, lane, 0.0);
+            make_halo<C, IBW0>(p1, u, lane, (T)0);
             slide_sums<C, IBW0>(u, zb);
-            make_halo<C, IBW0>(p2, u, lane, 0.0);
+            make_halo<C, IBW0>(p2, u, lane, (T)0);
             slide_sums<C, IBW0>(u, bb);
-            tmem_fetch<C>(M.tmem + 6 * C, t_isw); tmem_fetch<C>(M.tmem + 8 * C, t_xb); tmem_fetch<C>(M.tmem + 10 * C, t_isxx);
+            TmemArr<T, C>::fetch(M.tmem + 3 * PC, t_isw); TmemArr<T, C>::fetch(M.tmem + 4 * PC, t_xb); TmemArr<T, C>::fetch(M.tmem + 5 * PC, t_isxx);
 #pragma unroll
             for (int s = 0; s < C; s++) {
-                const double mz = zb[s];
+                const T mz = zb[s];
                 zb[s] = mz * t_isw[s];
                 bb[s] = (bb[s] - t_xb[s] * mz) * t_isxx[s];
             }
@@ -687,25 +843,26 @@ __device__ __forceinline__ double warp_eval_body(const EvalConst& K, const WarpM
             const int sr = K.slot_r, lr = K.lane_r;
             SS_CLAMP(zb) SS_CLAMP(bb)
         }
-        double yy[C];
-        tmem_fetch<C>(M.tmem + 12 * C, yy);
+        T yy[C];
+        TmemArr<T, C>::fetch(M.tmem + 6 * PC, yy);
 #pragma unroll
         for (int s = 0; s < C; s++) {
-            const double smo = zb[s] + bb[s] * (x[s] - t_xb[s]);
-            const double r = yy[s] - smo;
+            const T smo = zb[s] + bb[s] * (x[s] - t_xb[s]);
+            const T r = yy[s] - smo;
             chi2 += w[s] * r * r;
         }
     }
 #undef SS_CLAMP
+    double c2 = chi2;      // the lane's C terms were summed in T
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) chi2 += __shfl_xor_sync(0xffffffffu, chi2, d);
-    return (K.kc[4] - chi2) * K.kc[5];
+    for (int d = 16; d > 0; d >>= 1) c2 += __shfl_xor_sync(0xffffffffu, c2, d);
+    return (K.kc[4] - c2) * K.kc[5];
 }
 
 // One eval.  Returns P in every lane; `defer` is set (warp-uniform) when the fast path cannot
 // decide the eval exactly.
-template <int C, int IBW0, bool GV>
-__device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M, double f, int lane, bool& defer)
+template <int C, int IBW0, bool GV, typename T>
+__device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMemT<T>& M, double f, int lane, bool& defer)
 {
     constexpr int S = Pow2Ceil<C>::value;
     const int n = K.n;
@@ -730,7 +887,8 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
 #pragma unroll
     for (int s = 0; s < C; s++) idx[s] = (int)(key[s] & 0xffu);
     // ---- gather and exact-order check on the full 64-bit phases
-    double x[C], y[C], w[C], phi[C];
+    T x[C], y[C], w[C];
+    double phi[C];
 #pragma unroll
     for (int s = 0; s < C; s++) {
         const int j = lane * C + s;
@@ -739,7 +897,7 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
             phi[s] = fold_phase(M.tt[i], f);
             y[s] = M.yc[i];
             w[s] = M.w[i];
-        } else { phi[s] = 4.0; y[s] = 0.0; w[s] = W_PAD; }
+        } else { phi[s] = 4.0; y[s] = (T)0; w[s] = Real<T>::wpad(); }
     }
     bool bad = false;
     double nxt = shfl_down_d(phi[0], 1);
@@ -754,9 +912,9 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
     const double p3 = bcast_slot<C>(phi, K.q3s, K.q3l);
     if (__any_sync(0xffffffffu, bad)) { defer = true; return 0.0; }
 #pragma unroll
-    for (int s = 0; s < C; s++) x[s] = (lane * C + s < n) ? phi[s] - 0.5 : 0.0;
+    for (int s = 0; s < C; s++) x[s] = (lane * C + s < n) ? (T)(phi[s] - 0.5) : (T)0;
     const double scale = p3 - p1;
-    return warp_eval_body<C, IBW0, GV>(K, M, x, y, w, 1.e-6 * scale * scale, lane, defer);
+    return warp_eval_body<C, IBW0, GV, T>(K, M, x, y, w, (T)(1.e-6 * scale * scale), lane, defer);
 }
 
 
@@ -764,29 +922,32 @@ __device__ __forceinline__ double warp_eval(const EvalConst& K, const WarpMem& M
 // Kernel: one CTA = one work item (object, chunk of frequencies); its WARPS_PER_CTA warps split the
 // chunk into contiguous runs.  P values are staged in registers and written 32 at a time.
 // ------------------------------------------------------------------------------------------------
-template <int C, bool GV>
+template <int C, bool GV, typename T = double>
 inline size_t warp_smem_bytes()
 {
-    // object arrays (3 x 32C doubles) + per warp: 3 pair-prefix arrays
-    return (size_t)3 * 32 * C * 8 + (size_t)WarpCfg<C, GV>::WPC * ((size_t)3 * C * WROW * 16);
+    // object arrays (32C doubles of tt, 2 x 32C of T) + per warp: 3 pair-prefix arrays
+    return (size_t)32 * C * (8 + 2 * sizeof(T)) + (size_t)WarpCfg<C, GV, T>::WPC * ((size_t)3 * C * WROW * 2 * sizeof(T));
 }
 
 __device__ __forceinline__ int uni(int v) { return __shfl_sync(0xffffffffu, v, 0); }
 
-template <int C, int IBW0, bool GV>
-__global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB) warp_kernel(const EvalParams p)
+template <int C, int IBW0, bool GV, typename T = double>
+__global__ void __launch_bounds__(WarpCfg<C, GV, T>::WPC * 32, WarpCfg<C, GV, T>::MINB) warp_kernel(const EvalParams p)
 {
-    constexpr int WPC = WarpCfg<C, GV>::WPC;
+    constexpr int WPC = WarpCfg<C, GV, T>::WPC;
     static_assert(WARPS_PER_CTA % WPC == 0, "chunks are multiples of WARPS_PER_CTA");
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double s_best[WPC];
     __shared__ long long s_bestk[WPC];
     __shared__ uint32_t s_tmem;
-    // tensor-memory columns: 18C words per warp (14C of parked doubles, 4C window indices); warps w and w+4 share a lane quarter
-    constexpr uint32_t TCOLS_WARP = GV ? 4 * C : 18 * C;
+    // tensor-memory columns: 18C words per warp in fp64 (7 parked arrays of C doubles, 4C window indices); warps w and w+4
+    // share a lane quarter
+    constexpr uint32_t PC = TmemArr<T, C>::COLS;
+    constexpr uint32_t WC = WinTab<T, C>::COLS;
+    constexpr uint32_t TCOLS_WARP = GV ? 2 * WC : 7 * PC + 2 * WC;
     constexpr uint32_t TCOLS_NEED = TCOLS_WARP * ((WPC + 3) / 4);
     constexpr uint32_t TCOLS = TCOLS_NEED <= 32 ? 32 : (TCOLS_NEED <= 64 ? 64 : (TCOLS_NEED <= 128 ? 128 : (TCOLS_NEED <= 256 ? 256 : 512)));
-    static_assert(TCOLS * WarpCfg<C, GV>::MINB <= 512, "tensor memory over-subscribed");
+    static_assert(TCOLS * WarpCfg<C, GV, T>::MINB <= 512, "tensor memory over-subscribed");
     const int tid = threadIdx.x, lane = tid & 31;
     // warp index through a lane-0 broadcast: the compiler then knows it (and the eval loop's bounds) to be
     // warp-uniform, so the shuffles inside the loop need no WARPSYNC / ENDCOLLECTIVE wrappers
@@ -829,13 +990,13 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     K.bass = (p.alpha > 0.0 && p.alpha <= 10.0) ? (K.bexp == 1.0 ? 1 : 2) : 0;
 
     double* o_tt = reinterpret_cast<double*>(smem_raw);
-    double* o_y = o_tt + 32 * C;
-    double* o_w = o_y + 32 * C;
-    constexpr size_t WARP_BYTES = (size_t)3 * C * WROW * 16;
-    unsigned char* wbase = smem_raw + (size_t)3 * 32 * C * 8 + (size_t)warp * WARP_BYTES;
-    WarpMem M;
+    T* o_y = reinterpret_cast<T*>(o_tt + 32 * C);
+    T* o_w = o_y + 32 * C;
+    constexpr size_t WARP_BYTES = (size_t)3 * C * WROW * 2 * sizeof(T);
+    unsigned char* wbase = smem_raw + (size_t)32 * C * (8 + 2 * sizeof(T)) + (size_t)warp * WARP_BYTES;
+    WarpMemT<T> M;
     M.tt = o_tt; M.yc = o_y; M.w = o_w;
-    M.E = reinterpret_cast<double2*>(wbase);
+    M.E = reinterpret_cast<typename Real<T>::vec2*>(wbase);
     M.tmem = 0;
     M.mk = make_scan_mask(lane);
     {
@@ -848,8 +1009,8 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     }
     for (int j = tid; j < n; j += WPC * 32) {
         o_tt[j] = p.tt[rec.off + j];
-        o_y[j] = p.yc[rec.off + j];
-        o_w[j] = p.w[rec.off + j];
+        o_y[j] = (T)p.yc[rec.off + j];
+        o_w[j] = (T)p.w[rec.off + j];
     }
     __syncthreads();
     {
@@ -862,8 +1023,8 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
             w1[s] = wst<C>(lo1); w1[C + s] = wst<C>(lo1 + K.K1);
             w2[s] = wst<C>(lo2); w2[C + s] = wst<C>(lo2 + K.K2);
         }
-        tmem_park_words<2 * C>(M.tmem + (GV ? 0 : 14 * C), w1);
-        tmem_park_words<2 * C>(M.tmem + (GV ? 2 * C : 16 * C), w2);
+        WinTab<T, C>::park(M.tmem + (GV ? 0 : 7 * PC), w1);
+        WinTab<T, C>::park(M.tmem + (GV ? WC : 7 * PC + WC), w2);
         tmem_wait_st();
     }
 
@@ -877,10 +1038,18 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     double* prow = p.pgram ? p.pgram + (rec.obj - p.pgram_row0) * p.pgram_row_stride - p.pgram_k0 : nullptr;
     double stash = 0.0;
     int64_t kb = k0;                                       // first k of the current batch of 32
-    for (int64_t k = k0; k < k1; k++) {
+    constexpr bool LOCKSTEP = sizeof(T) == 4;
+    for (int64_t k = k0; k < (LOCKSTEP ? k0 + per_warp : k1); k++) {
+        // T = float runs 24-32 warps per SM and is bound by instruction fetch (ncu: no_instruction the top stall, the
+        // unrolled eval is 50-100 KB of SASS against a 32 KB L1.5 instruction cache): one barrier per eval keeps the
+        // CTA's warps on the same stretch of code (+15 %); the fp64 kernels (16 warps per SM) lose 1 % to it
+        if constexpr (LOCKSTEP) {
+            __syncthreads();
+            if (k >= k1) continue;
+        }
         const double f = freq_of(p.f_min, p.df, k);
         bool defer;
-        double P = warp_eval<C, IBW0, GV>(K, M, f, lane, defer);
+        double P = warp_eval<C, IBW0, GV, T>(K, M, f, lane, defer);
         if (defer) {
             if (lane == 0) {
                 unsigned pos = atomicAdd(p.defer_count, 1u);
@@ -913,13 +1082,13 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
     }
 }
 
-template <int C, int IBW0, bool GV>
+template <int C, int IBW0, bool GV, typename T = double>
 inline ss_status_t launch_warp_variant(const EvalParams& p, int64_t n_items, cudaStream_t stream)
 {
-    const size_t smem = warp_smem_bytes<C, GV>();
-    if (cudaFuncSetAttribute(warp_kernel<C, IBW0, GV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    const size_t smem = warp_smem_bytes<C, GV, T>();
+    if (cudaFuncSetAttribute(warp_kernel<C, IBW0, GV, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return SS_ERR_CUDA;
-    warp_kernel<C, IBW0, GV><<<(unsigned)n_items, WarpCfg<C, GV>::WPC * 32, smem, stream>>>(p);
+    warp_kernel<C, IBW0, GV, T><<<(unsigned)n_items, WarpCfg<C, GV, T>::WPC * 32, smem, stream>>>(p);
     return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
 }
 

@@ -188,7 +188,7 @@ __global__ void __launch_bounds__(WarpCfg<C, GV>::WPC * 32, WarpCfg<C, GV>::MINB
                     w[s] = real ? o_w[m * 32 * C + idx[s]] : W_PAD;
                 }
                 K.kc = s_kc[m];
-                P = warp_eval_body<C, IBW0, GV>(K, M, x, y, w, vsmlsq, lane, defer);
+                P = warp_eval_body<C, IBW0, GV, double>(K, M, x, y, w, vsmlsq, lane, defer);
                 __syncwarp();      // every lane is done with the prefix arrays before the next object overwrites them
             }
             if (defer) { hand_over(m, k); P = 0.0; }

@@ -1,7 +1,7 @@
 // ss_warp_tu.cu -- instantiations of the warp-per-eval kernel.  Compiled twelve times by _build.py:
 //   -DSS_TU_GV=0|1 (cross-validation / generalized validation)  x  -DSS_TU_GROUP=0|1|2 (C = 2..4 / 5..6 / 7..8)
-//   x -DSS_TU_SHARED=0|1|2 (warp_kernel / warp_shared_kernel, the shared-time-sampling variant / warp_opt_kernel,
-//     the listing's options)
+//   x -DSS_TU_SHARED=0|1|2|3 (warp_kernel / warp_shared_kernel, the shared-time-sampling variant / warp_opt_kernel,
+//     the listing's options / warp_kernel with the smoother in fp32, the MIXED precision)
 // so that the kernels build in parallel.
 #include "ss_launch.h"
 #include "ss_warp_kernel.cuh"
@@ -9,7 +9,7 @@
 #include "ss_warp_shared.cuh"
 
 #ifndef SS_TU_GV
-#error "compile with -DSS_TU_GV=0|1 -DSS_TU_GROUP=0|1|2 -DSS_TU_SHARED=0|1"
+#error "compile with -DSS_TU_GV=0|1 -DSS_TU_GROUP=0|1|2 -DSS_TU_SHARED=0|1|2|3"
 #endif
 
 namespace ss {
@@ -18,10 +18,14 @@ namespace ss {
 #define SS_CAT(a, b, c, d) SS_CAT2(a, b, c, d)
 #if SS_TU_SHARED == 1
 #define SS_TU_FN SS_CAT(launch_warp_shared_tu_, SS_TU_GV, _, SS_TU_GROUP)
-#define SS_TU_LAUNCH launch_warp_shared_variant
+#define SS_TU_LAUNCH(C_, I_) launch_warp_shared_variant<C_, I_, GV>
+#elif SS_TU_SHARED == 3
+// MIXED precision: the same kernel with the smoother in fp32
+#define SS_TU_FN SS_CAT(launch_warp_f32_tu_, SS_TU_GV, _, SS_TU_GROUP)
+#define SS_TU_LAUNCH(C_, I_) launch_warp_variant<C_, I_, GV, float>
 #else
 #define SS_TU_FN SS_CAT(launch_warp_tu_, SS_TU_GV, _, SS_TU_GROUP)
-#define SS_TU_LAUNCH launch_warp_variant
+#define SS_TU_LAUNCH(C_, I_) launch_warp_variant<C_, I_, GV, double>
 #endif
 
 #if SS_TU_SHARED == 2
@@ -54,18 +58,18 @@ ss_status_t SS_TU_FN(const EvalParams& p, int variant, int64_t n_items, cudaStre
     constexpr bool GV = SS_TU_GV != 0;
     switch (variant) {
 #if SS_TU_GROUP == 0
-        case 2 * 8 + 2: return SS_TU_LAUNCH<2, 2, GV>(p, n_items, stream);
-        case 3 * 8 + 2: return SS_TU_LAUNCH<3, 2, GV>(p, n_items, stream);
-        case 4 * 8 + 2: return SS_TU_LAUNCH<4, 2, GV>(p, n_items, stream);
-        case 4 * 8 + 3: return SS_TU_LAUNCH<4, 3, GV>(p, n_items, stream);
+        case 2 * 8 + 2: return SS_TU_LAUNCH(2, 2)(p, n_items, stream);
+        case 3 * 8 + 2: return SS_TU_LAUNCH(3, 2)(p, n_items, stream);
+        case 4 * 8 + 2: return SS_TU_LAUNCH(4, 2)(p, n_items, stream);
+        case 4 * 8 + 3: return SS_TU_LAUNCH(4, 3)(p, n_items, stream);
 #elif SS_TU_GROUP == 1
-        case 5 * 8 + 3: return SS_TU_LAUNCH<5, 3, GV>(p, n_items, stream);
-        case 5 * 8 + 4: return SS_TU_LAUNCH<5, 4, GV>(p, n_items, stream);
-        case 6 * 8 + 4: return SS_TU_LAUNCH<6, 4, GV>(p, n_items, stream);
-        case 6 * 8 + 5: return SS_TU_LAUNCH<6, 5, GV>(p, n_items, stream);
+        case 5 * 8 + 3: return SS_TU_LAUNCH(5, 3)(p, n_items, stream);
+        case 5 * 8 + 4: return SS_TU_LAUNCH(5, 4)(p, n_items, stream);
+        case 6 * 8 + 4: return SS_TU_LAUNCH(6, 4)(p, n_items, stream);
+        case 6 * 8 + 5: return SS_TU_LAUNCH(6, 5)(p, n_items, stream);
 #else
-        case 7 * 8 + 5: return SS_TU_LAUNCH<7, 5, GV>(p, n_items, stream);
-        case 8 * 8 + 6: return SS_TU_LAUNCH<8, 6, GV>(p, n_items, stream);
+        case 7 * 8 + 5: return SS_TU_LAUNCH(7, 5)(p, n_items, stream);
+        case 8 * 8 + 6: return SS_TU_LAUNCH(8, 6)(p, n_items, stream);
 #endif
         default: return SS_ERR_UNSUPPORTED;
     }
