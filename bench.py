@@ -357,7 +357,7 @@ def run_ours(args):
            "vs_baseline": None, "dtype": "f64" if args.precision == "f64" else "f32", "data": "synthetic",
            "config": {"workload": f"config{args.config}: {n_obj} objects ({cat.n_points} points) x {n_freq} "
                       f"frequencies on [{cat.f_min},{cat.f_max}), mode={args.mode}, periodogram materialised"
-                      + (", precision=mixed (fp32 smoother on the group path; fp64 fold, sort and prefix accumulation)" if args.precision == "mixed" else ""),
+                      + (", precision=mixed (fp32 smoother on the warp and group paths; fp64 fold, sort and prefix accumulation across threads)" if args.precision == "mixed" else ""),
                       "objects_per_second": world * n_obj * args.steps / (elapsed_ms * 1e-3),
                       "l2": (f"inputs ({24 * cat.n_points / 1e6:.0f} MB catalog) are re-read per frequency by design; the "
                              f"{8 * evals_per_step / 1e9:.2f} GB periodogram written every step "
