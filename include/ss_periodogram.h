@@ -167,6 +167,37 @@ ss_status_t ss_periodogram_host(const double *times, const double *mags, const d
  * final status.  SS_OK when nothing is pending. */
 ss_status_t ss_synchronize(void);
 
+/* ------------------------------------------------------------------ the entry point that allocates nothing */
+
+/* Size of the library's built-in device scratch: a file-scope `static __device__` array, so EVERY GPU that loads the
+ * library holds these bytes until the process exits. */
+#define SS_STATIC_SCRATCH_BYTES (32u << 20)
+
+/*
+ * The operation of ss_periodogram (Algorithm 1; 125), for callers that cannot tolerate a device
+ * allocation: code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  Same DEVICE-pointer
+ * arguments, same kernels, default options; the workspace those kernels need (the centred copy of the catalog, object
+ * records, partial-argmax rows, the hand-over list, counters) is carved from the built-in scratch array of
+ * SS_STATIC_SCRATCH_BYTES instead of the pooled cudaMalloc buffer.  The call makes no cudaMalloc / cudaFree / stream or
+ * event creation and calls no allocating library routine (it does use host memory of the C++ runtime).
+ *
+ *   offsets_host   HOST copy of offsets (n_objects + 1 values), required: the call reads no device memory from the host
+ *                  except one 4-byte status flag.
+ *   stream         cudaStream_t of the caller (0 = the legacy default stream); the call returns once it is complete.
+ *
+ * Limit: the catalog must fit the scratch -- about 24 B per point + 100 B per object + 1 MB (hand-over list of 65,536
+ * entries) + the partial-argmax rows of one frequency tile (the planner tiles frequencies to fit); light curves of more
+ * than SS_GROUP_MAX_N points need per-CTA staging space far beyond it.  A catalog that does not fit is rejected with
+ * SS_ERR_UNSUPPORTED and a message that states the bytes needed, before anything is launched or written.
+ * Sharing: every call on a device uses the SAME array; it keeps the previous call's contents (the call clears what it
+ * needs zeroed), and two calls that overlap on one GPU -- from two host threads, or on two streams -- race.  Serialise them.
+ * Results equal those of ss_periodogram bit for bit (same kernels, same tiling rules).
+ */
+ss_status_t ss_periodogram_static(const double *times, const double *mags, const double *errs,
+                                  const int64_t *offsets, const int64_t *offsets_host, int64_t n_objects,
+                                  double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
+                                  double *pgram_out, double *best_freq_out, int64_t *best_index_out, void *stream);
+
 /* ------------------------------------------------------------------ top-k peaks */
 
 #define SS_MAX_PEAKS 32

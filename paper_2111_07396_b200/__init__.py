@@ -25,7 +25,8 @@ LIB_PATH = os.path.join(_HERE, "libss_b200.so")
 EXPORTS = ["ss_default_options", "ss_periodogram", "ss_periodogram_ex", "ss_periodogram_host",
            "ss_plan", "ss_workspace_bytes", "ss_paper_footprint_bytes", "ss_paper_batches",
            "ss_path_for_n", "ss_debug_eval", "ss_microbench", "ss_last_launch_count", "ss_last_kernel_ms", "ss_last_kernel_count",
-           "ss_last_error", "ss_version", "ss_release_workspace", "ss_periodogram_peaks", "ss_periodogram_peaks_host", "ss_synchronize"]
+           "ss_last_error", "ss_version", "ss_release_workspace", "ss_periodogram_peaks", "ss_periodogram_peaks_host", "ss_synchronize",
+           "ss_periodogram_static"]
 
 
 class SSError(RuntimeError):
@@ -72,6 +73,7 @@ def load():
     L.ss_periodogram.argtypes = common
     L.ss_periodogram_ex.argtypes = common + [C.POINTER(Options)]
     L.ss_periodogram_host.argtypes = common + [C.POINTER(Options)]
+    L.ss_periodogram_static.argtypes = [vp, vp, vp, vp, vp, i64, d, d, i64, C.c_int, vp, vp, vp, vp]
     L.ss_plan.argtypes = [i64, i64, i64, i64, C.c_int, C.c_size_t, C.c_int, C.c_int, C.POINTER(Plan)]
     L.ss_workspace_bytes.argtypes = [i64, i64, i64, i64, C.c_int]
     L.ss_workspace_bytes.restype = C.c_size_t
@@ -189,6 +191,30 @@ def ss_periodogram(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, 
                              _dev_ptr(pgram_out, torch.float64, "pgram_out"),
                              _dev_ptr(best_freq_out, torch.float64, "best_freq_out"),
                              _dev_ptr(best_index_out, torch.int64, "best_index_out"), C.byref(o))
+    _check(st)
+
+
+STATIC_SCRATCH_BYTES = 32 << 20      # SS_STATIC_SCRATCH_BYTES
+
+
+def ss_periodogram_static(times, mags, errs, offsets, offsets_host, n_objects, f_min, f_max, n_freq,
+                          mode=CROSS_VALIDATION, pgram_out=None, best_freq_out=None, best_index_out=None, stream=None):
+    """Device-tensor call that allocates nothing on the device (include/ss_periodogram.h: ss_periodogram_static):
+    the workspace is the library's built-in scratch array of STATIC_SCRATCH_BYTES.  offsets_host is a C-contiguous
+    int64 numpy copy of offsets.  Calls that overlap on one GPU race on that array."""
+    torch = _torch()
+    L = load()
+    if not (isinstance(offsets_host, np.ndarray) and offsets_host.dtype == np.int64 and offsets_host.flags["C_CONTIGUOUS"]
+            and offsets_host.size == int(n_objects) + 1):
+        raise TypeError("offsets_host must be a C-contiguous int64 numpy array of n_objects + 1 values")
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    st = L.ss_periodogram_static(_dev_ptr(times, torch.float64, "times"), _dev_ptr(mags, torch.float64, "mags"),
+                                 _dev_ptr(errs, torch.float64, "errs"), _dev_ptr(offsets, torch.int64, "offsets"),
+                                 C.c_void_p(offsets_host.ctypes.data), int(n_objects), float(f_min), float(f_max),
+                                 int(n_freq), int(mode), _dev_ptr(pgram_out, torch.float64, "pgram_out"),
+                                 _dev_ptr(best_freq_out, torch.float64, "best_freq_out"),
+                                 _dev_ptr(best_index_out, torch.int64, "best_index_out"), C.c_void_p(stream))
     _check(st)
 
 

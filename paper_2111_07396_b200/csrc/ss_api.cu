@@ -7,6 +7,7 @@
 #include <cstring>
 #include <memory>
 #include <string>
+#include <mutex>
 #include <vector>
 
 #include "../../include/ss_periodogram.h"
@@ -1087,6 +1088,74 @@ ss_status_t ss_microbench(double* fp64_flops_out, double* smem_bytes_per_s_out, 
     cudaEventDestroy(e1);
     cudaFree(d);
     return SS_OK;
+}
+
+// ---- the entry point that allocates nothing (include/ss_periodogram.h: ss_periodogram_static) ---------------------
+// The workspace of the ordinary call, carved from a built-in array instead of the pooled cudaMalloc buffer.  In HOST
+// code the array's name is only a handle for the runtime, not a device address: the address every kernel is given
+// comes from cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[SS_STATIC_SCRATCH_BYTES];
+
+constexpr int STATIC_MAX_DEVICES = 64;
+constexpr unsigned int STATIC_DEFER_CAPACITY = 1u << 16;      // hand-over list of the static call: 1 MB instead of 16 MB
+static std::mutex g_static_mutex;
+static void* g_static_addr[STATIC_MAX_DEVICES] = {};
+
+static ss_status_t static_scratch_address(void** out)
+{
+    int dev = 0;
+    SS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= STATIC_MAX_DEVICES) return fail(SS_ERR_UNSUPPORTED, "device ordinal %d (limit %d)", dev, STATIC_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+        if (e != cudaSuccess || !ptr)
+            return fail(SS_ERR_CUDA, "cudaGetSymbolAddress of the built-in scratch failed on device %d: %s", dev, cudaGetErrorString(e));
+        g_static_addr[dev] = ptr;
+    }
+    *out = g_static_addr[dev];
+    return SS_OK;
+}
+
+ss_status_t ss_periodogram_static(const double* times, const double* mags, const double* errs,
+                                  const int64_t* offsets, const int64_t* offsets_host, int64_t n_objects,
+                                  double f_min, double f_max, int64_t n_freq, ss_mode_t mode,
+                                  double* pgram_out, double* best_freq_out, int64_t* best_index_out, void* stream)
+{
+    if (!offsets_host) return fail(SS_ERR_INVALID_ARG, "ss_periodogram_static needs offsets_host");
+    if (n_objects < 0 || n_freq < 1) return fail(SS_ERR_INVALID_ARG, "negative size");
+    // what the call needs, from the host copy of the offsets alone: reject before anything is launched or written
+    int64_t total = 0, max_n = 0;
+    for (int64_t i = 0; i < n_objects; i++) {
+        const int64_t n = offsets_host[i + 1] - offsets_host[i];
+        if (n < 0) return fail(SS_ERR_INVALID_ARG, "offsets not non-decreasing at %lld", (long long)i);
+        total += n;
+        max_n = std::max(max_n, n);
+    }
+    ss_plan_t need{}, fit{};
+    PlanInput pin{total, max_n, n_objects, n_freq, (int)mode, (size_t)-1, 0, pgram_out ? 1 : 0, 0, device_sm_count(), STATIC_DEFER_CAPACITY};
+    make_plan(pin, &need);
+    pin.cap_bytes = SS_STATIC_SCRATCH_BYTES;
+    if (make_plan(pin, &fit) != SS_OK || fit.total_bytes > SS_STATIC_SCRATCH_BYTES)
+        return fail(SS_ERR_UNSUPPORTED,
+                    "ss_periodogram_static: this catalog (%lld points, longest light curve %lld) needs at least %zu B of "
+                    "workspace (%zu B untiled); the built-in scratch holds %u B -- use ss_periodogram_ex",
+                    (long long)total, (long long)max_n, (size_t)(need.fixed_bytes + need.stage_bytes), (size_t)need.total_bytes,
+                    (unsigned)SS_STATIC_SCRATCH_BYTES);
+    void* scratch = nullptr;
+    ss_status_t st = static_scratch_address(&scratch);
+    if (st != SS_OK) return st;
+    ss_options_t o;
+    ss_default_options(&o);
+    o.stream = stream;
+    o.workspace = scratch;
+    o.workspace_bytes = SS_STATIC_SCRATCH_BYTES;
+    o.workspace_cap = SS_STATIC_SCRATCH_BYTES;
+    o.offsets_host = offsets_host;
+    o.defer_capacity = STATIC_DEFER_CAPACITY;
+    return ss_periodogram_ex(times, mags, errs, offsets, n_objects, f_min, f_max, n_freq, mode, pgram_out, best_freq_out,
+                             best_index_out, &o);
 }
 
 }  // extern "C"
