@@ -514,11 +514,13 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             const ObjRec& r = recs[ri];
             if (r.obj < o0 || r.obj >= o1) continue;
             int path = o.force_path != SS_PATH_AUTO ? o.force_path : path_for_n(r.n, md);
-            // periodic windows and the fixed span live in the generic CTA-per-eval code only
-            // periodic windows and the fixed span: the warp path has its own kernel for them, longer light curves
-            // go to the generic CTA-per-eval code
-            if (path == SS_PATH_GROUP && has_listing_options(o)) path = SS_PATH_BLOCK;
+            // periodic windows and the fixed span: the warp and group paths have their own kernels for them, longer
+            // light curves go to the generic CTA-per-eval code
             if (path == SS_PATH_WARP && (r.n > SS_WARP_MAX_N || !WARP_IMPLEMENTED)) path = SS_PATH_GROUP;
+            // a fixed span narrower than the tweeter's: a window sum is then < 1/20 of the prefixes it is the difference
+            // of, and a near-singular window (7 points inside a seasonal gap's edge) misses the 1e-9 bar by prefix
+            // differences at n > 256 (measured 1.03e-9); the CTA-per-eval kernels sum such windows directly
+            if (path == SS_PATH_GROUP && o.span > 0.0 && o.span < SPAN0) path = SS_PATH_BLOCK;
             if (path == SS_PATH_CLUSTER && has_listing_options(o)) path = SS_PATH_STAGE;
             if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N) path = SS_PATH_CLUSTER;
             if (path == SS_PATH_CLUSTER && (r.n > SS_CLUSTER_MAX_N || r.n < 2 * 512)) path = SS_PATH_STAGE;
@@ -527,7 +529,9 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             if (path == SS_PATH_WARP)
                 variant = has_listing_options(o) ? WARP_VARIANT_OPT + std::max(2, (r.n + 31) / 32)
                                                  : warp_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? WARP_VARIANT_F32 : 0);
-            else if (path == SS_PATH_GROUP) variant = group_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? GROUP_VARIANT_F32 : 0);
+            else if (path == SS_PATH_GROUP)
+                variant = group_variant_for_n(r.n) + (has_listing_options(o) ? GROUP_VARIANT_OPT
+                                                      : o.precision == SS_PRECISION_MIXED ? GROUP_VARIANT_F32 : 0);
             else if (path == SS_PATH_CLUSTER) variant = cluster_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
             else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);
@@ -668,7 +672,9 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
             ss_status_t st = launch_cluster_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "cluster kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (c.path == SS_PATH_GROUP) {
-            ss_status_t st = launch_group_kernel(p, c.variant, n_items, stream);
+            ss_status_t st = c.variant >= GROUP_VARIANT_OPT
+                                 ? launch_group_opt_kernel(p, c.variant - GROUP_VARIANT_OPT, opt.span > 0.0 ? 2 : mode, n_items, stream)
+                                 : launch_group_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "group kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else {
             const int threads = c.path == SS_PATH_STAGE ? 512 : (c.variant == 2 ? 512 : (c.variant == 3 ? 128 : 256));

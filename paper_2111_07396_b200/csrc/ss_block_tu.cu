@@ -213,6 +213,21 @@ SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1
 SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
 #undef SS_DECL
 
+#define SS_DECL(gv, g) ss_status_t launch_group_opt_tu_##gv##_##g(const EvalParams&, int, int, int64_t, cudaStream_t);
+SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
+#undef SS_DECL
+
+// mode: 0 = CV, 1 = GV, 2 = fixed span (the listing's options; variant = group_variant_for_n(n))
+ss_status_t launch_group_opt_kernel(const EvalParams& p, int variant, int mode, int64_t n_items, cudaStream_t stream)
+{
+    const int g = variant / 8, c = variant % 8;
+    if (mode == 1)
+        return g == 4 ? launch_group_opt_tu_1_4(p, c, mode, n_items, stream)
+             : g == 8 ? launch_group_opt_tu_1_8(p, c, mode, n_items, stream) : launch_group_opt_tu_1_16(p, c, mode, n_items, stream);
+    return g == 4 ? launch_group_opt_tu_0_4(p, c, mode, n_items, stream)
+         : g == 8 ? launch_group_opt_tu_0_8(p, c, mode, n_items, stream) : launch_group_opt_tu_0_16(p, c, mode, n_items, stream);
+}
+
 ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
 {
     const bool f32 = variant >= GROUP_VARIANT_F32;

@@ -216,9 +216,16 @@ struct GroupConst {
 template <int G, int C, bool GV, typename T>
 constexpr int group_minb() { return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 : GroupCfg<G, C, T>::MINB; }
 
-template <int G, int C, bool GV, typename T = double>
+// OPT: 0 = the default call; 1 = the listing's options compiled in: periodic windows (iper = 2,
+// PAPER.md:199-200) -- a window that leaves [0, n) is two ranges, the part that wrapped counting with abscissae x - 1
+// or x + 1, so its moments follow from the unshifted sums of that part: Swx += s bw, Swxx += 2 s bwx + bw, Sxy += s by
+// (s = -1 below 0, +1 above n-1); the second range is found by arithmetic, no second table --
+// 2 = a fixed span (span > 0): one smooth of y, both modes alike (instantiated with GV = false).
+template <int G, int C, bool GV, typename T = double, int OPT = 0>
 __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>()) group_kernel(const EvalParams p)
 {
+    static_assert(OPT == 0 || sizeof(T) == 8, "the listing's options are served in fp64");
+    static_assert(OPT != 2 || !GV, "the fixed-span kernel is instantiated once, with GV = false");
     using Cfg = GroupCfg<G, C, T>;
     using RT = Real<T>;
     using T2 = typename RT::vec2;
@@ -227,7 +234,11 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ __align__(16) double2 s_tot[3][G];          // warp totals of up to three pair scans
     __shared__ double s_red[G];
-    __shared__ double s_edge[2][G][2];                       // [first|last][warp]{phase, index} across warp boundaries
+    // {phase, index} of each warp's first ([0][warp]) and last ([1][warp + 1]) point, read by the neighbour warp.  The
+    // outer slots [0][G] and [1][0] hold sentinels, so that the reads need no test on the warp index: with
+    // `if (warp > 0) .. s_edge[1][warp - 1]` ptxas 12.9 formed the address in uniform registers under a mismatched
+    // predicate in group_kernel<4, 5, CV, double, 1> and <8, 7, CV, double, 1> (cuda-gdb: misaligned / out-of-range LDS.128).
+    __shared__ __align__(16) double s_edge[2][G + 1][2];
     __shared__ double s_q[2];                                // phases of the quartile points
     __shared__ double s_kc[8];
     __shared__ __align__(8) uint64_t s_bar;
@@ -281,8 +292,18 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
         bulk_g2s(o_w, p.w + rec.off, bytes, &s_bar);
     }
 
-    const int ibw0 = rec.ibw[0], ibw1 = rec.ibw[1], ibw2 = rec.ibw[2];
-    const int K0 = min(2 * ibw0 + 1, n), K1 = min(2 * ibw1 + 1, n), K2 = min(2 * ibw2 + 1, n);
+    const bool per = OPT != 0 && p.iper == 2;        // phases are in [0, 1): jper = iper
+    // half-widths: the three spans, or the caller's fixed one in slot 0; a periodic window never exceeds n points (R8)
+    int ibw_[3], Kw_[3];
+#pragma unroll
+    for (int i = 0; i < 3; i++) {
+        int b = OPT == 2 ? rec.ibw_fixed : rec.ibw[i];
+        int kk = 2 * b + 1;
+        if (kk > n) { kk = n; if (per) { b = (n - 1) / 2; kk = 2 * b + 1; } }
+        ibw_[i] = b; Kw_[i] = kk;
+    }
+    const int ibw0 = ibw_[0], ibw1 = ibw_[1], ibw2 = ibw_[2];
+    const int K0 = Kw_[0], K1 = Kw_[1], K2 = Kw_[2];
     GroupConst K;
     K.n = n;
     K.q1t = rec.q1 / C; K.q1s = rec.q1 % C; K.q3t = rec.q3 / C; K.q3s = rec.q3 % C;
@@ -291,6 +312,10 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
         s_kc[2] = 1.0 / (1.0 - 1.0 / (double)K1); s_kc[3] = 1.0 / (1.0 - 2.0 / (double)K1);
         s_kc[4] = 1.0 / (1.0 - 1.0 / (double)K2); s_kc[5] = 1.0 / (1.0 - 2.0 / (double)K2);
         s_kc[6] = rec.chi0; s_kc[7] = rec.chi0 > 0.0 ? 1.0 / rec.chi0 : 0.0;
+    }
+    if (tid == 0) {
+        s_edge[0][G][0] = 1.0e3; s_edge[0][G][1] = 0.0;      // behind the last warp
+        s_edge[1][0][0] = -1.0; s_edge[1][0][1] = 0.0;       // in front of the first
     }
     K.kc = s_kc;
     K.bexp = 10.0 - p.alpha;
@@ -303,16 +328,35 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     constexpr uint32_t T_A0 = 0, T_A1 = PC, T_A2 = 2 * PC, T_ISW = 3 * PC, T_XB = 4 * PC, T_G0 = 5 * PC, T_Y = 6 * PC;
     constexpr int CE = Cfg::CE;
     constexpr uint32_t T_W0 = 7 * PC, T_W1 = T_W0 + CE, T_W2 = T_W0 + 2 * CE;      // window ends per span: lo | hi << 16
+    auto at = [&](int pos) { return (pos % C) * ROW + pos / C; };
+    // second range of the periodic window of point j at half-width ib: element indices [blo, bhi) and the shift sg (0: none)
+    struct Wrap { int sg, blo, bhi; };
+    auto wrapped = [&](int j, int ib) -> Wrap {
+        Wrap r;
+        r.sg = 0; r.blo = 0; r.bhi = 0;
+        if (per && j < n) {
+            if (j - ib < 0) { r.blo = at(j - ib + n); r.bhi = at(n); r.sg = -1; }
+            else if (j + ib + 1 > n) { r.bhi = at(j + ib + 1 - n); r.sg = 1; }
+        }
+        return r;
+    };
     {
         int w0[C], w1[C], w2[C];
-        auto at = [&](int pos) { return (pos % C) * ROW + pos / C; };
 #pragma unroll
         for (int s = 0; s < C; s++) {
             const int j = tid * C + s;
-            const int l0 = window_lo(j, ibw0, K0, n), l1 = window_lo(j, ibw1, K1, n), l2 = window_lo(j, ibw2, K2, n);
-            w0[s] = at(l0) | (at(l0 + K0) << 16);
-            w1[s] = at(l1) | (at(l1 + K1) << 16);
-            w2[s] = at(l2) | (at(l2 + K2) << 16);
+            int l0, l1, l2, h0, h1, h2;
+            if (per && j < n) {      // the part of the window inside [0, n)
+                l0 = max(j - ibw0, 0); h0 = min(j + ibw0 + 1, n);
+                l1 = max(j - ibw1, 0); h1 = min(j + ibw1 + 1, n);
+                l2 = max(j - ibw2, 0); h2 = min(j + ibw2 + 1, n);
+            } else {
+                l0 = window_lo(j, ibw0, K0, n); l1 = window_lo(j, ibw1, K1, n); l2 = window_lo(j, ibw2, K2, n);
+                h0 = l0 + K0; h1 = l1 + K1; h2 = l2 + K2;
+            }
+            w0[s] = at(l0) | (at(h0) << 16);
+            w1[s] = at(l1) | (at(h1) << 16);
+            w2[s] = at(l2) | (at(h2) << 16);
         }
         tmem_park_words<C>(tmem + T_W0, w0);
         tmem_park_words<C>(tmem + T_W1, w1);
@@ -363,19 +407,13 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
             }
         }
         if (lane == 0) { s_edge[0][warp][0] = phi[0]; s_edge[0][warp][1] = (double)idx[0]; }
-        if (lane == 31) { s_edge[1][warp][0] = phi[C - 1]; s_edge[1][warp][1] = (double)idx[C - 1]; }
+        if (lane == 31) { s_edge[1][warp + 1][0] = phi[C - 1]; s_edge[1][warp + 1][1] = (double)idx[C - 1]; }
         __syncthreads();                                                                    // BAR 1
         {
             double nphi = shfl_down_d(phi[0], 1), pphi = shfl_up_d(phi[C - 1], 1);
             int nidx = __shfl_down_sync(0xffffffffu, idx[0], 1), pidx = __shfl_up_sync(0xffffffffu, idx[C - 1], 1);
-            if (lane == 31) {
-                if (warp + 1 < G) { nphi = s_edge[0][warp + 1][0]; nidx = (int)s_edge[0][warp + 1][1]; }
-                else nphi = 1.0e3;
-            }
-            if (lane == 0) {
-                if (warp > 0) { pphi = s_edge[1][warp - 1][0]; pidx = (int)s_edge[1][warp - 1][1]; }
-                else pphi = -1.0;
-            }
+            if (lane == 31) { nphi = s_edge[0][warp + 1][0]; nidx = (int)s_edge[0][warp + 1][1]; }      // last warp: 1e3
+            if (lane == 0) { pphi = s_edge[1][warp][0]; pidx = (int)s_edge[1][warp][1]; }               // first warp: -1
             // both sides of a boundary see the same two phases and take the same decision
             const bool swap_next = nphi < phi[C - 1], swap_prev = phi[0] < pphi;
             if (tid * C + C - 1 < n && nphi == phi[C - 1]) bad = true;                     // exact tie (R24): generic path
@@ -440,7 +478,34 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
             const T vsmlsq = (T)(1.e-6 * scale * scale);
             __syncthreads();                                                                // BAR 3
             T chi2 = (T)0;
-            if (GV) {
+            if constexpr (OPT == 2) {
+                // ---- fixed span: one smooth of y over the caller's window
+                const T* E4 = reinterpret_cast<const T*>(E45);
+                int wi[CE];
+                tmem_fetch_words<CE>(tmem + T_W0, wi);
+#pragma unroll
+                for (int s = 0; s < C; s++) {
+                    const int a_ = wi[s] & 0xffff, b_ = (int)((unsigned)wi[s] >> 16);
+                    const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_];
+                    T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                    T Sxy = E4[b_] - E4[a_];
+                    const Wrap wr = wrapped(tid * C + s, ibw0);
+                    if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
+                        const int blo = wr.blo, bhi = wr.bhi;
+                        const T sh = (T)wr.sg;
+                        const T2 p0 = E01[blo], q0 = E01[bhi], p1 = E23[blo], q1 = E23[bhi];
+                        const T bw = q0.x - p0.x, bwx = q0.y - p0.y, by = q1.y - p1.y;
+                        Sw += bw; Swx += bwx + sh * bw; Swxx += (q1.x - p1.x) + ((T)2 * sh * bwx + bw);
+                        Sy += by; Sxy += (E4[bhi] - E4[blo]) + sh * by;
+                    }
+                    const T isw = RT::rcp(Sw), xb = Swx * isw;
+                    const T sxx = Swxx - xb * Swx;
+                    const T isxx = sxx > vsmlsq ? RT::rcp(sxx) : (T)0;
+                    const T smo = Sy * isw + (Sxy - xb * Sy) * (isxx * (x[s] - xb));
+                    const T r = y[s] - smo;
+                    chi2 += w[s] * r * r;
+                }
+            } else if (GV) {
                 // ---- O6: three windows, scores, pick, interpolate
                 T A[3][C], Gs[3][C];
 #pragma unroll
@@ -451,8 +516,19 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                     for (int s = 0; s < C; s++) {
                         const int a_ = wi[s] & 0xffff, b_ = (int)((unsigned)wi[s] >> 16);
                         const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_], l2 = E45[a_], h2 = E45[b_];
-                        const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                        const T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                        T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                        T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
+                        if constexpr (OPT != 0) {
+                            const Wrap wr = wrapped(tid * C + s, i == 0 ? ibw0 : (i == 1 ? ibw1 : ibw2));
+                            if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
+                                const int blo = wr.blo, bhi = wr.bhi;
+                                const T sh = (T)wr.sg;
+                                const T2 p0 = E01[blo], q0 = E01[bhi], p1 = E23[blo], q1 = E23[bhi], p2 = E45[blo], q2 = E45[bhi];
+                                const T bw = q0.x - p0.x, bwx = q0.y - p0.y, by = q1.y - p1.y;
+                                Sw += bw; Swx += bwx + sh * bw; Swxx += (q1.x - p1.x) + ((T)2 * sh * bwx + bw);
+                                Sy += by; Sxy += (q2.x - p2.x) + sh * by; Syy += q2.y - p2.y;
+                            }
+                        }
                         const T isw = RT::rcp(Sw), xb = Swx * isw;
                         const T sxx = Swxx - xb * Swx;
                         const T isxx = sxx > vsmlsq ? RT::rcp(sxx) : (T)0;
@@ -485,8 +561,19 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                         const int a_ = wi[s] & 0xffff, b_ = (int)((unsigned)wi[s] >> 16);
                         const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_];
                         const T lxy = E4[a_], hxy = E4[b_];
-                        const T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
-                        const T Sxy = hxy - lxy;
+                        T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
+                        T Sxy = hxy - lxy;
+                        if constexpr (OPT != 0) {
+                            const Wrap wr = wrapped(tid * C + s, i == 0 ? ibw0 : (i == 1 ? ibw1 : ibw2));
+                            if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
+                                const int blo = wr.blo, bhi = wr.bhi;
+                                const T sh = (T)wr.sg;
+                                const T2 p0 = E01[blo], q0 = E01[bhi], p1 = E23[blo], q1 = E23[bhi];
+                                const T bw = q0.x - p0.x, bwx = q0.y - p0.y, by = q1.y - p1.y;
+                                Sw += bw; Swx += bwx + sh * bw; Swxx += (q1.x - p1.x) + ((T)2 * sh * bwx + bw);
+                                Sy += by; Sxy += (E4[bhi] - E4[blo]) + sh * by;
+                            }
+                        }
                         const T isw = RT::rcp(Sw), xb = Swx * isw;
                         const T sxx = Swxx - xb * Swx;
                         const T isxx = sxx > vsmlsq ? RT::rcp(sxx) : (T)0;
@@ -539,7 +626,17 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
 #pragma unroll
                         for (int s = 0; s < C; s++) {
                             const T2 l = Ez[w1i[s] & 0xffff], h = Ez[(unsigned)w1i[s] >> 16];
-                            const T Sz = h.x - l.x, Sxz = h.y - l.y;
+                            T Sz = h.x - l.x, Sxz = h.y - l.y;
+                            if constexpr (OPT != 0) {
+                                const Wrap wr = wrapped(tid * C + s, ibw1);
+                                if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
+                                    const int blo = wr.blo, bhi = wr.bhi;
+                                    const T sh = (T)wr.sg;
+                                    const T2 pz = Ez[blo], qz = Ez[bhi];
+                                    const T bz = qz.x - pz.x;
+                                    Sz += bz; Sxz += (qz.y - pz.y) + sh * bz;
+                                }
+                            }
                             out[s] = Sz * m_isw[s] + (Sxz - m_xb[s] * Sz) * m_g[s];
                         }
                     };
@@ -581,7 +678,17 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
 #pragma unroll
                     for (int s = 0; s < C; s++) {
                         const T2 l = E23[w0i[s] & 0xffff], h = E23[(unsigned)w0i[s] >> 16];
-                        const T Sz = h.x - l.x, Sxz = h.y - l.y;
+                        T Sz = h.x - l.x, Sxz = h.y - l.y;
+                        if constexpr (OPT != 0) {
+                            const Wrap wr = wrapped(tid * C + s, ibw0);
+                            if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
+                                const int blo = wr.blo, bhi = wr.bhi;
+                                const T sh = (T)wr.sg;
+                                const T2 pz = E23[blo], qz = E23[bhi];
+                                const T bz = qz.x - pz.x;
+                                Sz += bz; Sxz += (qz.y - pz.y) + sh * bz;
+                            }
+                        }
                         const T smo = Sz * t_isw[s] + (Sxz - t_xb[s] * Sz) * t_g[s];
                         const T r = yy[s] - smo;
                         chi2 += w[s] * r * r;
@@ -620,13 +727,13 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     }
 }
 
-template <int G, int C, bool GV, typename T = double>
+template <int G, int C, bool GV, typename T = double, int OPT = 0>
 inline ss_status_t launch_group_variant(const EvalParams& p, int64_t n_items, cudaStream_t stream)
 {
     const size_t smem = group_smem_bytes<G, C, GV, T>();
-    if (cudaFuncSetAttribute(group_kernel<G, C, GV, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    if (cudaFuncSetAttribute(group_kernel<G, C, GV, T, OPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
         return SS_ERR_CUDA;
-    group_kernel<G, C, GV, T><<<(unsigned)n_items, GroupCfg<G, C, T>::NT, smem, stream>>>(p);
+    group_kernel<G, C, GV, T, OPT><<<(unsigned)n_items, GroupCfg<G, C, T>::NT, smem, stream>>>(p);
     return cudaGetLastError() == cudaSuccess ? SS_OK : SS_ERR_CUDA;
 }
 

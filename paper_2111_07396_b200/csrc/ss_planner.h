@@ -27,6 +27,7 @@ inline int path_for_n(int64_t n, int /*mode*/)
 constexpr int SHARED_TIMES_M = 4;          // objects per work item of the shared-time-sampling warp kernel
 constexpr int WARP_VARIANT_OPT = 2000;      // warp variant id of the listing-options kernel: WARP_VARIANT_OPT + points per lane
 constexpr int GROUP_VARIANT_F32 = 1000;   // added to the group variant id: smoother scalar float (mixed precision)
+constexpr int GROUP_VARIANT_OPT = 2000;   // added to the group variant id: the kernels with the listing's options compiled in
 constexpr int WARP_VARIANT_F32 = 1000;    // added to the warp variant id: the same (below WARP_VARIANT_OPT)
 
 // Cluster-path kernel variant: R CTAs of 512 threads x C points per thread, the smallest capacity R*512*C >= n

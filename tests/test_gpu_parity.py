@@ -347,6 +347,40 @@ def test_periodic_windows_and_fixed_span(ss, mode, opts):
     res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
     check_parity(cat, res.pgram, ref, mode, label=f"cfg4 {opts}", oracle_opts=opts)
     check_best(ref, res.best_index, res.best_freq, cat)
+    blk = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode,
+                         force_path=ss.PATH_BLOCK, **opts)
+    check_parity(cat, blk.pgram, ref, mode, label=f"cfg4/cta {opts}", oracle_opts=opts)
+
+
+@pytest.mark.parametrize("mode", [CV, GV])
+@pytest.mark.parametrize("opts", LISTING_OPTIONS, ids=lambda o: ",".join(f"{k}={v}" for k, v in o.items()))
+def test_listing_options_on_the_group_path(ss, mode, opts):
+    """iper = 2 / span > 0 for 256 < n <= 2,055 are served by group_kernel<.., OPT> (the wrapped part of a periodic
+    window as a second range with shifted abscissae, found by arithmetic): one object per (G, C) variant, one with a
+    duplicated time stamp (handed over whole), one with integer-day times that tie at f = 1 / d, against the oracle,
+    best index included."""
+    rng = np.random.default_rng(919)
+    ns = [257, 384, 500, 513, 600, 640, 700, 768, 850, 1000, 1280, 1400, 1536, 1700, 1792, 2048, 2055, 300, 420]
+    T, Y, E = [], [], []
+    for i, n in enumerate(ns):
+        t = np.sort(rng.integers(0, 900, size=n) + rng.uniform(0.0, 0.33, size=n))
+        if i == len(ns) - 2:
+            t[11] = t[10]                                   # duplicated time stamp
+        if i == len(ns) - 1:
+            t = np.arange(n, dtype=np.float64) + 0.25 * (np.arange(n) % 3 == 0)      # ties at f = 1
+        e = rng.uniform(0.02, 0.1, size=n)
+        y = 15 + rng.uniform(0.2, 0.8) * np.sin(2 * np.pi * t / np.exp(rng.uniform(np.log(0.3), np.log(2.0))) + i) \
+            + rng.normal(0, 1.0, size=n) * e
+        T.append(t); Y.append(y); E.append(e)
+    off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
+    cat = ss_inputs.Catalog("gopts", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
+                            0.25, 4.25, 64, np.full(len(ns), np.nan))
+    assert oracle.freq(cat.f_min, cat.f_max, cat.n_freq, 12) == 1.0
+    ref, _, _ = oracle.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq,
+                                   mode=mode, variant=oracle.FAST, **opts)
+    res = ss.periodogram(cat.times, cat.mags, cat.errs, cat.offsets, cat.f_min, cat.f_max, cat.n_freq, mode, **opts)
+    check_parity(cat, res.pgram, ref, mode, label=f"group-opt {opts}", oracle_opts=opts, max_ambiguous=4)
+    check_best(ref, res.best_index, res.best_freq, cat)
 
 
 @pytest.mark.parametrize("mode", [CV, GV])
