@@ -73,10 +73,13 @@ typedef struct {
     double alpha;           /* bass enhancement.  Default 9.0.                 */
     double span;            /* 0 = variable span (default).  In (0, 1]: Listing 1's fixed-span branch
                                (PAPER.md:202-210): one running-line smooth at this span, in both modes.
-                               Served by the CTA-per-eval kernels for every n.                           */
+                               Served by the warp kernels for n <= SS_WARP_MAX_N, by the group kernels for
+                               n <= SS_GROUP_MAX_N when span >= 0.05, by the CTA-per-eval kernels otherwise;
+                               always in fp64.                                                           */
     int iper;               /* 1 = windows pinned at the ends (default, R8).  2 = periodic windows
                                (PAPER.md:199-200): the window of point j is j-ibw..j+ibw modulo n, phases
-                               that wrapped count as x-1 / x+1.  Served by the CTA-per-eval kernels.     */
+                               that wrapped count as x-1 / x+1.  Served like the fixed span (warp, group or
+                               CTA-per-eval kernels by n), in fp64.                                      */
     int force_path;         /* ss_path_t; SS_PATH_AUTO = choose by n.  For tests and sweeps.            */
     void *stream;           /* cudaStream_t the work is enqueued on (NULL = legacy default stream)      */
     size_t workspace_cap;   /* bytes of device workspace the library may allocate; 0 = 75 % of free
