@@ -106,8 +106,9 @@ typedef struct {
                                fp64 throughput for n <= SS_WARP_MAX_N.                                             */
     int shared_times;       /* 1 = every object of the catalog has the SAME time stamps in the same order (one field
                                observed together).  The fold and the sort are then done once per
-                               frequency for 4 objects at a time (objects of n <= SS_WARP_MAX_N; longer ones are
-                               served as usual).  Checked on the device unless skip_validation is set: a catalog
+                               frequency for 4 objects at a time (objects of n <= SS_GROUP_MAX_N, fp64 precision,
+                               default listing options; otherwise the objects are served one by one as usual).
+                               Checked on the device unless skip_validation is set: a catalog
                                whose time arrays differ is SS_ERR_INVALID_ARG.  Results equal those of
                                shared_times = 0 to rounding (same arithmetic, same order).                   */
     void *workspace;        /* device entry points: a DEVICE buffer of workspace_bytes bytes (256-byte aligned) the library

@@ -40,7 +40,7 @@ def units():
         elif base == "ss_group_tu":
             for gv in (0, 1):
                 for g in (4, 8, 16):
-                    for f32 in (0, 1, 2):
+                    for f32 in (0, 1, 2, 3):
                         u.append((f"{base}_{gv}_{g}_{f32}.o", src, [f"-DSS_TU_GV={gv}", f"-DSS_TU_G={g}", f"-DSS_TU_F32={f32}"]))
         elif base == "ss_cluster_tu":
             for gv in (0, 1):

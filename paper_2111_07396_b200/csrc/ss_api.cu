@@ -647,7 +647,9 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         p.counter = counters + (next_counter % n_counters);
         p.stage = stage; p.stage_stride = stage_stride;
         p.defer_entries = defer_entries; p.defer_count = defer_count; p.defer_capacity = defer_capacity;
-        const bool shared = opt.shared_times && c.path == SS_PATH_WARP && c.variant < WARP_VARIANT_F32;      // one fold + sort per group of objects
+        // one fold + sort per group of objects (fp64 kernels with default options)
+        const bool shared = opt.shared_times && ((c.path == SS_PATH_WARP && c.variant < WARP_VARIANT_F32) ||
+                                                 (c.path == SS_PATH_GROUP && c.variant < GROUP_VARIANT_F32));
         const int64_t n_items = (shared ? ((int64_t)p.n_list + SHARED_TIMES_M - 1) / SHARED_TIMES_M : (int64_t)p.n_list) * cpo;
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -674,7 +676,8 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         } else if (c.path == SS_PATH_GROUP) {
             ss_status_t st = c.variant >= GROUP_VARIANT_OPT
                                  ? launch_group_opt_kernel(p, c.variant - GROUP_VARIANT_OPT, opt.span > 0.0 ? 2 : mode, n_items, stream)
-                                 : launch_group_kernel(p, c.variant, n_items, stream);
+                                 : shared ? launch_group_shared_kernel(p, c.variant, n_items, stream)
+                                          : launch_group_kernel(p, c.variant, n_items, stream);
             if (st != SS_OK) return fail(st, "group kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else {
             const int threads = c.path == SS_PATH_STAGE ? 512 : (c.variant == 2 ? 512 : (c.variant == 3 ? 128 : 256));

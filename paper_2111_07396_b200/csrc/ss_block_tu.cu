@@ -217,6 +217,21 @@ SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1
 SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
 #undef SS_DECL
 
+#define SS_DECL(gv, g) ss_status_t launch_group_shared_tu_##gv##_##g(const EvalParams&, int, int64_t, cudaStream_t);
+SS_DECL(0, 4) SS_DECL(0, 8) SS_DECL(0, 16) SS_DECL(1, 4) SS_DECL(1, 8) SS_DECL(1, 16)
+#undef SS_DECL
+
+// one shared time sampling: n_items = groups of SHARED_TIMES_M objects x chunks; variant = group_variant_for_n(n)
+ss_status_t launch_group_shared_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream)
+{
+    const int g = variant / 8, c = variant % 8;
+    if (p.mode == 1)
+        return g == 4 ? launch_group_shared_tu_1_4(p, c, n_items, stream)
+             : g == 8 ? launch_group_shared_tu_1_8(p, c, n_items, stream) : launch_group_shared_tu_1_16(p, c, n_items, stream);
+    return g == 4 ? launch_group_shared_tu_0_4(p, c, n_items, stream)
+         : g == 8 ? launch_group_shared_tu_0_8(p, c, n_items, stream) : launch_group_shared_tu_0_16(p, c, n_items, stream);
+}
+
 // mode: 0 = CV, 1 = GV, 2 = fixed span (the listing's options; variant = group_variant_for_n(n))
 ss_status_t launch_group_opt_kernel(const EvalParams& p, int variant, int mode, int64_t n_items, cudaStream_t stream)
 {

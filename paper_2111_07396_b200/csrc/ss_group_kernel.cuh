@@ -220,18 +220,28 @@ constexpr int group_minb() { return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 
 // PAPER.md:199-200) -- a window that leaves [0, n) is two ranges, the part that wrapped counting with abscissae x - 1
 // or x + 1, so its moments follow from the unshifted sums of that part: Swx += s bw, Swxx += 2 s bwx + bw, Sxy += s by
 // (s = -1 below 0, +1 above n-1); the second range is found by arithmetic, no second table --
-// 2 = a fixed span (span > 0): one smooth of y, both modes alike (instantiated with GV = false).
+// 2 = a fixed span (span > 0): one smooth of y, both modes alike (instantiated with GV = false);
+// 3 = shared time sampling (ss_options_t::shared_times): the work item is a group of SHARED_TIMES_M objects
+// with one time vector; fold, sort, order repair and the abscissae are done once per frequency, the smoother once per
+// object on that permutation (y and w gathered from the catalog copy in global memory).
 template <int G, int C, bool GV, typename T = double, int OPT = 0>
 __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>()) group_kernel(const EvalParams p)
 {
-    static_assert(OPT == 0 || sizeof(T) == 8, "the listing's options are served in fp64");
+    static_assert(OPT == 0 || sizeof(T) == 8, "the listing's options and shared sampling are served in fp64");
     static_assert(OPT != 2 || !GV, "the fixed-span kernel is instantiated once, with GV = false");
     using Cfg = GroupCfg<G, C, T>;
     using RT = Real<T>;
     using T2 = typename RT::vec2;
     using TA = TmemArr<T, C>;
     constexpr int NT = Cfg::NT, NP = Cfg::NP, ROW = Cfg::ROW, ASZ = C * ROW;
+    constexpr bool LOPT = OPT == 1 || OPT == 2;            // the listing's options
+    constexpr bool SH = OPT == 3;
+    constexpr int M_ = SH ? SHARED_TIMES_M : 1;            // objects per work item
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int s_ri[M_];                               // per object of the group: record index, offset into the
+    __shared__ long long s_off[M_];                        // catalog copy, chi0 and 1 / chi0, periodogram row
+    __shared__ double s_chi[M_][2];
+    __shared__ double* s_prow[M_];
     __shared__ __align__(16) double2 s_tot[3][G];          // warp totals of up to three pair scans
     __shared__ double s_red[G];
     // {phase, index} of each warp's first ([0][warp]) and last ([1][warp + 1]) point, read by the neighbour warp.  The
@@ -247,21 +257,30 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);     // provably warp-uniform (see warp_kernel)
     const int item = blockIdx.x;
-    const int li = item / p.chunks_per_obj, ch = item - li * p.chunks_per_obj;
+    const int grp = item / p.chunks_per_obj, ch = item - grp * p.chunks_per_obj;
+    const int li = grp * M_;
+    const int mcnt = SH ? min(M_, p.n_list - li) : 1;        // objects in this group
     const int ri = p.list[li];
-    const ObjRec rec = p.recs[ri];
+    const ObjRec rec = p.recs[ri];                           // shared sampling: n, windows and times of the first object
     if (rec.dup) {
-        // duplicated time stamps: every eval ties; the generic kernel takes the whole work item
-        if (tid == 0) {
+        // duplicated time stamps: every eval ties; the generic kernel takes the whole work item(s)
+        if (tid < mcnt) {
             const unsigned pos = atomicAdd(p.defer_count, 1u);
             if (pos < p.defer_capacity)
-                p.defer_entries[pos] = DEFER_ITEM | ((unsigned long long)ri << 32) | (unsigned long long)ch;
+                p.defer_entries[pos] = DEFER_ITEM | ((unsigned long long)(SH ? p.list[li + tid] : ri) << 32) | (unsigned long long)ch;
             else
                 p.defer_count[1] = 1u;
         }
         return;
     }
     const int n = rec.n;
+    if (SH && tid < mcnt) {
+        const int rm = p.list[li + tid];
+        const ObjRec r = p.recs[rm];
+        s_ri[tid] = rm; s_off[tid] = r.off;
+        s_chi[tid][0] = r.chi0; s_chi[tid][1] = r.chi0 > 0.0 ? 1.0 / r.chi0 : 0.0;
+        s_prow[tid] = p.pgram ? p.pgram + (r.obj - p.pgram_row0) * p.pgram_row_stride - p.pgram_k0 : nullptr;
+    }
 
     double* o_tt = reinterpret_cast<double*>(smem_raw);
     double* o_y = o_tt + NP;
@@ -286,13 +305,15 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     if (tid == 0) {
         const unsigned bytes = (unsigned)(((n + 1) & ~1) * 8);      // the workspace pads every object to an even length
-        mbar_expect_tx(&s_bar, 3 * bytes);
+        mbar_expect_tx(&s_bar, (SH ? 1 : 3) * bytes);
         bulk_g2s(o_tt, p.tt + rec.off, bytes, &s_bar);
-        bulk_g2s(o_y, p.yc + rec.off, bytes, &s_bar);
-        bulk_g2s(o_w, p.w + rec.off, bytes, &s_bar);
+        if (!SH) {      // shared sampling: y and w differ per object and are gathered from the catalog copy
+            bulk_g2s(o_y, p.yc + rec.off, bytes, &s_bar);
+            bulk_g2s(o_w, p.w + rec.off, bytes, &s_bar);
+        }
     }
 
-    const bool per = OPT != 0 && p.iper == 2;        // phases are in [0, 1): jper = iper
+    const bool per = LOPT && p.iper == 2;            // phases are in [0, 1): jper = iper
     // half-widths: the three spans, or the caller's fixed one in slot 0; a periodic window never exceeds n points (R8)
     int ibw_[3], Kw_[3];
 #pragma unroll
@@ -376,7 +397,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
 
     for (int64_t k = k0; k < k1; k++) {
         const double f = freq_of(p.f_min, p.df, k);
-        bool bad = false;
+        bool bad_sort = false;     // per thread: a tie or an order this path cannot settle
 
         // ---- P1 fold + 32-bit keys; P2 sort
         unsigned key[C];
@@ -416,22 +437,24 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
             if (lane == 0) { pphi = s_edge[1][warp][0]; pidx = (int)s_edge[1][warp][1]; }               // first warp: -1
             // both sides of a boundary see the same two phases and take the same decision
             const bool swap_next = nphi < phi[C - 1], swap_prev = phi[0] < pphi;
-            if (tid * C + C - 1 < n && nphi == phi[C - 1]) bad = true;                     // exact tie (R24): generic path
+            if (tid * C + C - 1 < n && nphi == phi[C - 1]) bad_sort = true;                     // exact tie (R24): generic path
             if (swap_next) { phi[C - 1] = nphi; idx[C - 1] = nidx; }
             if (swap_prev) { phi[0] = pphi; idx[0] = pidx; }
         }
 #pragma unroll
         for (int s = 0; s + 1 < C; s++)
-            if (tid * C + s + 1 < n && phi[s + 1] <= phi[s]) bad = true;                   // tie, or a bucket of three
+            if (tid * C + s + 1 < n && phi[s + 1] <= phi[s]) bad_sort = true;                   // tie, or a bucket of three
 
-        // ---- gather; x centred by 0.5, padded slots carry x = 0, y = 0, w = W_PAD
+        // ---- gather; x centred by 0.5, padded slots carry x = 0, y = 0, w = W_PAD; quartile phases for
+        // vsmlsq
         T x[C], y[C], w[C];
 #pragma unroll
         for (int s = 0; s < C; s++) {
-            if (tid * C + s < n) { x[s] = (T)(phi[s] - 0.5); y[s] = (T)o_y[idx[s]]; w[s] = (T)o_w[idx[s]]; }
-            else { x[s] = (T)0; y[s] = (T)0; w[s] = RT::wpad(); }
+            if (tid * C + s < n) {
+                x[s] = (T)(phi[s] - 0.5);
+                if constexpr (!SH) { y[s] = (T)o_y[idx[s]]; w[s] = (T)o_w[idx[s]]; }
+            } else { x[s] = (T)0; y[s] = (T)0; w[s] = RT::wpad(); }
         }
-        // quartile phases for vsmlsq
         if (tid == K.q1t) {
 #pragma unroll
             for (int s = 0; s < C; s++) if (s == K.q1s) s_q[0] = phi[s];
@@ -439,6 +462,16 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
         if (tid == K.q3t) {
 #pragma unroll
             for (int s = 0; s < C; s++) if (s == K.q3s) s_q[1] = phi[s];
+        }
+
+        // ---- the smoother, once per object of the work item (one object unless the time sampling is shared)
+        for (int m = 0; m < (SH ? mcnt : 1); m++) {
+        bool bad = bad_sort;
+        const int rim = SH ? s_ri[m] : ri;
+        if constexpr (SH) {      // gather of this object's y and w from the catalog copy
+#pragma unroll
+            for (int s = 0; s < C; s++)
+                if (tid * C + s < n) { y[s] = (T)__ldg(p.yc + s_off[m] + idx[s]); w[s] = (T)__ldg(p.w + s_off[m] + idx[s]); }
         }
 
         // ---- prefix sums of the weighted moments
@@ -463,7 +496,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
             if (tid == 0) {
                 const unsigned pos = atomicAdd(p.defer_count, 1u);
                 if (pos < p.defer_capacity)
-                    p.defer_entries[pos] = ((unsigned long long)ri << 32) | (unsigned long long)(k - p.k_begin);
+                    p.defer_entries[pos] = ((unsigned long long)rim << 32) | (unsigned long long)(k - p.k_begin);
                 else
                     p.defer_count[1] = 1u;
             }
@@ -518,7 +551,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                         const T2 l0 = E01[a_], h0 = E01[b_], l1 = E23[a_], h1 = E23[b_], l2 = E45[a_], h2 = E45[b_];
                         T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                         T Sxy = h2.x - l2.x, Syy = h2.y - l2.y;
-                        if constexpr (OPT != 0) {
+                        if constexpr (LOPT) {
                             const Wrap wr = wrapped(tid * C + s, i == 0 ? ibw0 : (i == 1 ? ibw1 : ibw2));
                             if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
                                 const int blo = wr.blo, bhi = wr.bhi;
@@ -563,7 +596,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                         const T lxy = E4[a_], hxy = E4[b_];
                         T Sw = h0.x - l0.x, Swx = h0.y - l0.y, Swxx = h1.x - l1.x, Sy = h1.y - l1.y;
                         T Sxy = hxy - lxy;
-                        if constexpr (OPT != 0) {
+                        if constexpr (LOPT) {
                             const Wrap wr = wrapped(tid * C + s, i == 0 ? ibw0 : (i == 1 ? ibw1 : ibw2));
                             if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
                                 const int blo = wr.blo, bhi = wr.bhi;
@@ -610,7 +643,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                     if (tid == 0) {
                         const unsigned pos = atomicAdd(p.defer_count, 1u);
                         if (pos < p.defer_capacity)
-                            p.defer_entries[pos] = ((unsigned long long)ri << 32) | (unsigned long long)(k - p.k_begin);
+                            p.defer_entries[pos] = ((unsigned long long)rim << 32) | (unsigned long long)(k - p.k_begin);
                         else
                             p.defer_count[1] = 1u;
                     }
@@ -627,7 +660,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                         for (int s = 0; s < C; s++) {
                             const T2 l = Ez[w1i[s] & 0xffff], h = Ez[(unsigned)w1i[s] >> 16];
                             T Sz = h.x - l.x, Sxz = h.y - l.y;
-                            if constexpr (OPT != 0) {
+                            if constexpr (LOPT) {
                                 const Wrap wr = wrapped(tid * C + s, ibw1);
                                 if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
                                     const int blo = wr.blo, bhi = wr.bhi;
@@ -679,7 +712,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                     for (int s = 0; s < C; s++) {
                         const T2 l = E23[w0i[s] & 0xffff], h = E23[(unsigned)w0i[s] >> 16];
                         T Sz = h.x - l.x, Sxz = h.y - l.y;
-                        if constexpr (OPT != 0) {
+                        if constexpr (LOPT) {
                             const Wrap wr = wrapped(tid * C + s, ibw0);
                             if (__any_sync(0xffffffffu, wr.sg != 0)) {      // warp-uniform; lanes that do not wrap read element 0 twice: + 0
                                 const int blo = wr.blo, bhi = wr.bhi;
@@ -704,13 +737,22 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
                 double c2 = 0.0;
 #pragma unroll
                 for (int q = 0; q < G; q++) c2 += s_red[q];
-                P = (K.kc[6] - c2) * K.kc[7];
+                P = SH ? (s_chi[m][0] - c2) * s_chi[m][1] : (K.kc[6] - c2) * K.kc[7];
             }
         }
-        if (!bad && P > best) { best = P; best_k = k; }
-        if (tid == (int)(k - kb)) stash = bad ? 0.0 : P;      // a handed-over eval is patched by the generic kernel
+        // thread m keeps object m's best; thread 32 m + i stashes its i-th value of the current batch of 32
+        if ((!SH || tid == m) && !bad && P > best) { best = P; best_k = k; }
+        if (tid == 32 * m + (int)(k - kb)) stash = bad ? 0.0 : P;      // a handed-over eval is patched by the generic kernel
+        }      // objects of the work item
         if (k - kb == 31 || k == k1 - 1) {
-            if (prow && tid < 32 && kb + tid <= k) prow[kb + tid] = stash;
+            if constexpr (SH) {
+                if (tid < 32 * mcnt) {
+                    double* pr = s_prow[tid >> 5];
+                    if (pr && kb + lane <= k) pr[kb + lane] = stash;
+                }
+            } else {
+                if (prow && tid < 32 && kb + tid <= k) prow[kb + tid] = stash;
+            }
             kb = k + 1;
         }
     }
@@ -720,8 +762,8 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" :: "r"(s_tmem), "n"(Cfg::TCOLS) : "memory");
     }
-    if (tid == 0) {
-        const int64_t slot = (int64_t)ri * p.chunks_total + p.chunk_base + ch;
+    if (SH ? tid < mcnt : tid == 0) {
+        const int64_t slot = (int64_t)(SH ? s_ri[tid] : ri) * p.chunks_total + p.chunk_base + ch;
         p.part_val[slot] = best;
         p.part_idx[slot] = best_k == INT64_MAX ? k0 : best_k;
     }

@@ -21,6 +21,9 @@ ss_status_t launch_warp_opt_kernel(const EvalParams& p, int c, int mode, int64_t
 // G-warps-per-eval kernels (ss_group_kernel.cuh); variant = group_variant_for_n(n)
 ss_status_t launch_group_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
 
+// the group kernels for a catalog with one shared time sampling (fp64, default options)
+ss_status_t launch_group_shared_kernel(const EvalParams& p, int variant, int64_t n_items, cudaStream_t stream);
+
 // the listing's options on the group path: variant = group_variant_for_n(n), mode 0 = CV, 1 = GV, 2 = fixed span
 ss_status_t launch_group_opt_kernel(const EvalParams& p, int variant, int mode, int64_t n_items, cudaStream_t stream);
 

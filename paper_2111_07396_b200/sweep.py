@@ -110,11 +110,12 @@ def _best_of(torch, call, reps=3):
 
 def shared_table(torch, dev, md):
     """shared_times = 1 (one fold + sort per frequency for 4 objects) against the ordinary call."""
-    n_obj, nf = 2000, 10000
-    lines = ["| n | mode | plain evals/s | shared_times evals/s | speed-up |", "|---|---|---|---|---|"]
-    for n in (64, 125, 200):
+    lines = ["| n | objects x frequencies | mode | plain evals/s | shared_times evals/s | speed-up |", "|---|---|---|---|---|---|"]
+    # n <= 256: warp path, 2,000 objects x 10,000 frequencies; beyond: group path, 400 x 3,000
+    for n, n_obj, nf in ((64, 2000, 10000), (125, 2000, 10000), (200, 2000, 10000), (500, 400, 3000), (1000, 400, 3000),
+                         (2000, 400, 3000)):
         rng = np.random.default_rng(n)
-        t1 = np.sort(rng.integers(0, 30, size=n) + rng.uniform(0.0, 0.33, size=n))
+        t1 = np.sort(rng.integers(0, 30 if n <= 256 else 900, size=n) + rng.uniform(0.0, 0.33, size=n))
         t = np.tile(t1, n_obj)
         e = rng.uniform(0.02, 0.1, size=n_obj * n)
         y = 15 + 0.4 * np.sin(2 * np.pi * t / np.repeat(np.exp(rng.uniform(np.log(0.1), np.log(2.0), size=n_obj)), n)) \
@@ -127,7 +128,7 @@ def shared_table(torch, dev, md):
             for sh in (0, 1):
                 o = default_options(shared_times=sh, skip_validation=1)
                 r.append(n_obj * nf / _best_of(torch, lambda: ss_periodogram(*a, n_obj, 0.5, 24.0, nf, mode, pg, None, None, o)))
-            lines.append(f"| {n} | {name} | {r[0]:.4g} | {r[1]:.4g} | {r[1] / r[0]:.3f} |")
+            lines.append(f"| {n} | {n_obj} x {nf} | {name} | {r[0]:.4g} | {r[1]:.4g} | {r[1] / r[0]:.3f} |")
             print(lines[-1], flush=True)
     if md:
         with open(md, "w") as f:
@@ -166,8 +167,8 @@ def main(argv=None):
                     help="instead of the sweep over n: the listing's options (iper = 2, fixed span; PAPER.md:199-210) "
                          "against the default call on config-3- and config-4-shaped catalogs")
     ap.add_argument("--shared", action="store_true",
-                    help="instead: shared_times = 1 against the ordinary call on 2,000 objects with one time vector "
-                         "(PAPER.md:125), n = 64, 125, 200, 10,000 frequencies")
+                    help="instead: shared_times = 1 against the ordinary call on catalogs with one time vector "
+                         "(PAPER.md:125), n = 64 ... 2,000")
     ap.add_argument("--mixed", action="store_true",
                     help="instead: precision = mixed against fp64 on config-3- and config-4-shaped catalogs (PAPER.md:604-616)")
     args = ap.parse_args(argv)

@@ -911,7 +911,9 @@ def test_shared_time_sampling_reuses_the_sort(ss, mode):
     parity with the oracle, for group sizes that do not divide the catalog, every points-per-lane variant, a shared
     sampling with a duplicated time stamp (every eval handed over) and tied phases at f = 1 / d on integer times;
     a catalog whose time stamps differ is refused."""
-    for n_objects, n, dup in ((37, 150, False), (9, 64, False), (6, 200, False), (5, 256, False), (7, 90, True)):
+    # n <= 256: warp_shared_kernel; beyond: group_kernel<.., 3> (one (G, C) variant per warp count, and the largest)
+    for n_objects, n, dup in ((37, 150, False), (9, 64, False), (6, 200, False), (5, 256, False), (7, 90, True),
+                              (9, 700, False), (6, 1100, False), (5, 2055, False), (7, 400, True), (3, 257, False)):
         t, y, e, off = _shared_times_catalog(n_objects, n, seed=n, dup=dup)
         plain = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode)
         shared = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode, shared_times=1)
@@ -921,18 +923,19 @@ def test_shared_time_sampling_reuses_the_sort(ss, mode):
         assert np.array_equal(shared.best_index, plain.best_index) and np.array_equal(shared.best_freq, plain.best_freq)
         if n_objects == 9:
             cat = ss_inputs.Catalog("shared", t, y, e, off, 0.5, 24.0, 131, np.full(n_objects, np.nan))
-            ref, _, _ = oracle.periodogram(t, y, e, off, 0.5, 24.0, 131, mode=mode, variant=oracle.DEFINITION)
+            ref, _, _ = oracle.periodogram(t, y, e, off, 0.5, 24.0, 131, mode=mode,
+                                           variant=oracle.DEFINITION if n <= 256 else oracle.FAST)
             check_parity(cat, shared.pgram, ref, mode, label="shared times")
             check_best(ref, shared.best_index, shared.best_freq, cat)
-    # integer-day times: at f = 1 every phase ties (handed over for the whole group)
-    n = 40
-    t1 = np.arange(n, dtype=np.float64) + 0.25 * (np.arange(n) % 3 == 0)
-    rng = np.random.default_rng(3)
-    T = np.tile(t1, 5); Y = 15 + rng.normal(0, 0.1, size=5 * n); E = np.full(5 * n, 0.05)
-    off = np.arange(6, dtype=np.int64) * n
-    plain = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode)
-    shared = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode, shared_times=1)
-    assert np.allclose(shared.pgram, plain.pgram, rtol=1e-13, atol=1e-14) and np.array_equal(shared.best_index, plain.best_index)
+    # integer-day times: at f = 1 every phase ties (handed over for the whole group); warp and group path
+    for n in (300, 40):
+        t1 = np.arange(n, dtype=np.float64) + 0.25 * (np.arange(n) % 3 == 0)
+        rng = np.random.default_rng(3)
+        T = np.tile(t1, 5); Y = 15 + rng.normal(0, 0.1, size=5 * n); E = np.full(5 * n, 0.05)
+        off = np.arange(6, dtype=np.int64) * n
+        plain = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode)
+        shared = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode, shared_times=1)
+        assert np.allclose(shared.pgram, plain.pgram, rtol=1e-13, atol=1e-14) and np.array_equal(shared.best_index, plain.best_index)
     # not actually shared
     T2 = T.copy(); T2[3 * n + 5] += 1e-9
     with pytest.raises(ss.SSError) as ei:
