@@ -59,14 +59,16 @@ typedef enum {
     SS_PATH_WARP = 1,  /* one warp per (object, frequency); n <= SS_WARP_MAX_N; registers + shuffles   */
     SS_PATH_BLOCK = 2, /* one CTA per (object, frequency); per-eval arrays in shared memory            */
     SS_PATH_STAGE = 3, /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
-    SS_PATH_GROUP = 4, /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_MAX_N;
-                          points in registers, prefix sums in shared memory, smooths in tensor memory     */
-    SS_PATH_CLUSTER = 5 /* a thread-block cluster of 2..16 CTAs per (object, frequency); SS_GROUP_MAX_N < n <=
-                          SS_CLUSTER_MAX_N; prefix sums in distributed shared memory                      */
+    SS_PATH_GROUP = 4, /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_LONG_MAX_N;
+                          points in registers, prefix sums in shared memory, smooths in tensor memory.
+                          Up to SS_GROUP_MAX_N with every option; beyond it the fp64 default call only     */
+    SS_PATH_CLUSTER = 5 /* a thread-block cluster of 2..16 CTAs per (object, frequency); SS_GROUP_LONG_MAX_N <
+                          n <= SS_CLUSTER_MAX_N; prefix sums in distributed shared memory                  */
 } ss_path_t;
 
 #define SS_WARP_MAX_N 256
 #define SS_GROUP_MAX_N 2055
+#define SS_GROUP_LONG_MAX_N 3584
 #define SS_CLUSTER_MAX_N 40960
 
 typedef struct {

@@ -75,13 +75,17 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                     "r"((uint32_t)__cvta_generic_to_shared(bar)) : "memory");
 }
 
+// The object's y and w are staged in shared memory beside its times up to 2,560 points; beyond (G = 16, C = 6, 7:
+// 3,072 / 3,584 points -- the three pair-prefix arrays then take 148 / 172 KB) they are gathered from the catalog copy
+// in global memory once per eval, as the shared-sampling kernels do.
+constexpr int GROUP_STAGE_YW_MAX = 2560;
 template <int G, int C, bool GV, typename T = double>
 inline size_t group_smem_bytes()
 {
     using Cfg = GroupCfg<G, C, T>;
-    // object arrays (3 x NP doubles) + 3 pair-prefix arrays of C*ROW vec2 (the sort's exchange buffers, 2 x NT*C words,
-    // overlay the first of them: C*ROW*sizeof(vec2) >= 8*NT*C also for float2)
-    return (size_t)3 * Cfg::NP * 8 + (size_t)3 * C * Cfg::ROW * sizeof(typename Real<T>::vec2);
+    // object arrays (3 x NP doubles, or the times alone) + 3 pair-prefix arrays of C*ROW vec2 (the sort's exchange
+    // buffers, 2 x NT*C words, overlay the first of them: C*ROW*sizeof(vec2) >= 8*NT*C also for float2)
+    return (size_t)(Cfg::NP > GROUP_STAGE_YW_MAX ? 1 : 3) * Cfg::NP * 8 + (size_t)3 * C * Cfg::ROW * sizeof(typename Real<T>::vec2);
 }
 
 // Exclusive prefix sums of two streams over the whole CTA (C values per thread, blocked), stored interleaved and
@@ -236,6 +240,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     constexpr int NT = Cfg::NT, NP = Cfg::NP, ROW = Cfg::ROW, ASZ = C * ROW;
     constexpr bool LOPT = OPT == 1 || OPT == 2;            // the listing's options
     constexpr bool SH = OPT == 3;
+    constexpr bool YW_GLOBAL = SH || Cfg::NP > GROUP_STAGE_YW_MAX;      // y, w gathered from the catalog copy per eval
     constexpr int M_ = SH ? SHARED_TIMES_M : 1;            // objects per work item
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_ri[M_];                               // per object of the group: record index, offset into the
@@ -285,7 +290,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     double* o_tt = reinterpret_cast<double*>(smem_raw);
     double* o_y = o_tt + NP;
     double* o_w = o_y + NP;
-    T2* E01 = reinterpret_cast<T2*>(smem_raw + (size_t)3 * NP * 8);                // (w, wx)      | residual 0 | spans
+    T2* E01 = reinterpret_cast<T2*>(smem_raw + (size_t)(NP > GROUP_STAGE_YW_MAX ? 1 : 3) * NP * 8);   // (w, wx) | residual 0 | spans
     T2* E23 = E01 + ASZ;                                                           // (wxx, wy)    | residual 1 | final
     T2* E45 = E23 + ASZ;                                                           // (wxy[, wyy]) | residual 2
     unsigned* kbuf = reinterpret_cast<unsigned*>(E01);                             // sort exchange (2 x NT*C words)
@@ -305,9 +310,9 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     if (tid == 0) {
         const unsigned bytes = (unsigned)(((n + 1) & ~1) * 8);      // the workspace pads every object to an even length
-        mbar_expect_tx(&s_bar, (SH ? 1 : 3) * bytes);
+        mbar_expect_tx(&s_bar, (YW_GLOBAL ? 1 : 3) * bytes);
         bulk_g2s(o_tt, p.tt + rec.off, bytes, &s_bar);
-        if (!SH) {      // shared sampling: y and w differ per object and are gathered from the catalog copy
+        if (!YW_GLOBAL) {      // shared sampling: y and w differ per object and are gathered from the catalog copy
             bulk_g2s(o_y, p.yc + rec.off, bytes, &s_bar);
             bulk_g2s(o_w, p.w + rec.off, bytes, &s_bar);
         }
@@ -452,7 +457,7 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
         for (int s = 0; s < C; s++) {
             if (tid * C + s < n) {
                 x[s] = (T)(phi[s] - 0.5);
-                if constexpr (!SH) { y[s] = (T)o_y[idx[s]]; w[s] = (T)o_w[idx[s]]; }
+                if constexpr (!YW_GLOBAL) { y[s] = (T)o_y[idx[s]]; w[s] = (T)o_w[idx[s]]; }
             } else { x[s] = (T)0; y[s] = (T)0; w[s] = RT::wpad(); }
         }
         if (tid == K.q1t) {
@@ -468,10 +473,11 @@ __global__ void __launch_bounds__(GroupCfg<G, C, T>::NT, group_minb<G, C, GV, T>
         for (int m = 0; m < (SH ? mcnt : 1); m++) {
         bool bad = bad_sort;
         const int rim = SH ? s_ri[m] : ri;
-        if constexpr (SH) {      // gather of this object's y and w from the catalog copy
+        if constexpr (YW_GLOBAL) {      // gather of this object's y and w from the catalog copy
+            const long long om = SH ? s_off[m] : (long long)rec.off;
 #pragma unroll
             for (int s = 0; s < C; s++)
-                if (tid * C + s < n) { y[s] = (T)__ldg(p.yc + s_off[m] + idx[s]); w[s] = (T)__ldg(p.w + s_off[m] + idx[s]); }
+                if (tid * C + s < n) { y[s] = (T)__ldg(p.yc + om + idx[s]); w[s] = (T)__ldg(p.w + om + idx[s]); }
         }
 
         // ---- prefix sums of the weighted moments

@@ -19,7 +19,7 @@ static_assert(SS_GROUP_MAX_N <= BLOCK_MAX_N, "what the group path hands over mus
 inline int path_for_n(int64_t n, int /*mode*/)
 {
     if (n <= SS_WARP_MAX_N) return SS_PATH_WARP;
-    if (n <= SS_GROUP_MAX_N) return SS_PATH_GROUP;
+    if (n <= SS_GROUP_LONG_MAX_N) return SS_PATH_GROUP;
     if (n <= SS_CLUSTER_MAX_N) return SS_PATH_CLUSTER;
     return SS_PATH_STAGE;
 }
@@ -41,7 +41,8 @@ inline int cluster_variant_for_n(int n)
 }
 
 // Group-path kernel variant of an object: G warps x C points per thread, the smallest capacity 32*G*C >= n among
-// (4,3) 384, (4,4) 512, (4,5) 640, (4,6) 768, (8,4) 1,024, (8,5) 1,280, (8,6) 1,536, (16,4) 2,048, (16,5) 2,560.  More
+// (4,3) 384, (4,4) 512, (4,5) 640, (4,6) 768, (8,4) 1,024, (8,5) 1,280, (8,6) 1,536, (16,4) 2,048, (16,5) 2,560, and for
+// the fp64 default call alone (SS_GROUP_MAX_N < n <= SS_GROUP_LONG_MAX_N) (16,6) 3,072, (16,7) 3,584.  More
 // points per thread beat more warps per eval (measured: (8,6) 2.37e10 point-evals/s at n = 1,400 where (16,3) gave
 // 1.85e10; (4,6) 2.49e10 at n = 700 where (8,3) gave 2.23e10); C = 6 is what tensor memory allows at 16 warps per SM
 // (20C columns per warp <= 128).  id = G*8 + C.
@@ -49,9 +50,9 @@ inline int group_variant_for_n(int n)
 {
     const int gs[3] = {4, 8, 16};
     for (int gi = 0; gi < 3; gi++)
-        for (int c = 3; c <= (gs[gi] == 16 ? 5 : 7); c++)
+        for (int c = 3; c <= 7; c++)
             if (32 * gs[gi] * c >= n && !(gs[gi] > 4 && c == 3)) return gs[gi] * 8 + c;
-    return 16 * 8 + 5;
+    return 16 * 8 + 7;
 }
 
 // Window half-width of Friedman's smoother (O4/R21): max(2, floor(0.5*span*n + 0.5)),

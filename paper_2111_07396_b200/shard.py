@@ -14,7 +14,7 @@ import numpy as np
 
 # Point-evals per second each path class sustains on one B200 (profiles/r2_crossover.md, CV mode: warp / group /
 # cluster / global staging): the relative cost of an object is n / rate(path(n)).  Only the ratios matter.
-_RATE = ((256, 3.3e10), (2055, 2.3e10), (40960, 5.0e9), (1 << 62, 1.4e9))
+_RATE = ((256, 3.3e10), (3584, 2.2e10), (40960, 5.5e9), (1 << 62, 1.4e9))
 
 
 def object_cost(n) -> np.ndarray:

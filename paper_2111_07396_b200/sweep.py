@@ -2,7 +2,7 @@
 kernel-cascade study).
 
 For each n a catalog of equal-length light curves is timed through the device entry point on every path
-class that can serve it (SS_PATH_WARP for n <= 256, SS_PATH_GROUP and SS_PATH_BLOCK for n <= 2,055,
+class that can serve it (SS_PATH_WARP for n <= 256, SS_PATH_GROUP for n <= 3,584, SS_PATH_BLOCK for n <= 2,055,
 SS_PATH_CLUSTER for 2,055 < n <= 40,960, SS_PATH_STAGE for any n), in both modes; the table reports point-evals/s (n x frequencies x objects / second), which is flat
 where a path scales and drops where it stops fitting.  The path the library picks by itself is marked.
 
@@ -26,7 +26,7 @@ from . import (CROSS_VALIDATION, GENERALIZED_VALIDATION, PATH_BLOCK, PATH_CLUSTE
 
 DEFAULT_NS = [50, 64, 96, 128, 160, 200, 256, 257, 320, 400, 512, 700, 1000, 1400, 2055, 2056, 3000, 5000, 10000, 20000, 40000]
 PATH_NAME = {PATH_WARP: "warp", PATH_GROUP: "group", PATH_CLUSTER: "cluster", PATH_BLOCK: "cta-smem", PATH_STAGE: "cta-staged"}
-WARP_MAX_N, BLOCK_MAX_N, CLUSTER_MAX_N = 256, 2055, 40960
+WARP_MAX_N, BLOCK_MAX_N, GROUP_LONG_MAX_N, CLUSTER_MAX_N = 256, 2055, 3584, 40960
 
 
 def catalog(n: int, n_objects: int, seed: int):
@@ -187,7 +187,8 @@ def main(argv=None):
              "|---|---|---|---|---|---|---|---|"]
     for n in [int(v) for v in args.ns.split(",")]:
         paths = [p for p in (PATH_WARP, PATH_GROUP, PATH_CLUSTER, PATH_BLOCK, PATH_STAGE)
-                 if (p != PATH_WARP or n <= WARP_MAX_N) and (p not in (PATH_BLOCK, PATH_GROUP) or n <= BLOCK_MAX_N)
+                 if (p != PATH_WARP or n <= WARP_MAX_N) and (p != PATH_BLOCK or n <= BLOCK_MAX_N)
+                 and (p != PATH_GROUP or n <= GROUP_LONG_MAX_N)
                  and (p != PATH_CLUSTER or BLOCK_MAX_N < n <= CLUSTER_MAX_N)]
         auto = path_for_n(n)
         for path in paths:

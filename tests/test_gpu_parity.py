@@ -718,10 +718,12 @@ def test_config4_full_size_sampled(ss, mode):
 @pytest.mark.parametrize("mode", [CV, GV])
 def test_group_kernel_every_variant(ss, mode):
     """The G-warps-per-eval kernels, one object per (G, C) variant at both ends of its range of n (capacities 384,
-    512, 640, 768 = 4 warps x 6 points, 1,024, 1,280, 1,536 = 8 x 6, 2,048, 2,560 points; the path ends at n = 2,055), heteroscedastic errors,
+    512, 640, 768 = 4 warps x 6 points, 1,024, 1,280, 1,536 = 8 x 6, 2,048, 2,560, and the long variants 3,072 and
+    3,584 = 16 x 7 that gather y and w from global memory; the path ends at n = 3,584), heteroscedastic errors,
     config-4 time sampling; against the definition oracle, best index included."""
     rng = np.random.default_rng(515)
-    ns = [257, 384, 385, 512, 513, 640, 641, 700, 768, 769, 1024, 1025, 1280, 1281, 1400, 1536, 1537, 2048, 2049, 2055]
+    ns = [257, 384, 385, 512, 513, 640, 641, 700, 768, 769, 1024, 1025, 1280, 1281, 1400, 1536, 1537, 2048, 2049, 2055,
+          2056, 2560, 2561, 3072, 3073, 3554, 3584]
     T, Y, E = [], [], []
     for i, n in enumerate(ns):
         assert ss.path_for_n(n) == ss.PATH_GROUP
@@ -760,7 +762,7 @@ def test_cluster_kernel_every_cluster_size(ss, mode):
     ns = [2056, 3072, 3073, 5120, 6000, 10240, 12288, 16385, 20480, 24577, 40960]
     T, Y, E = [], [], []
     for i, n in enumerate(ns):
-        assert ss.path_for_n(n) == ss.PATH_CLUSTER
+        assert ss.path_for_n(n) == (ss.PATH_CLUSTER if n > 3584 else ss.PATH_GROUP)      # forced below: every (R, C)
         t = np.sort(rng.integers(0, 3652, size=n) + rng.uniform(0.0, 0.3, size=n))
         if n == 6000:
             t[100] = t[99]; t[4000] = t[3999]
@@ -771,7 +773,7 @@ def test_cluster_kernel_every_cluster_size(ss, mode):
     off = np.zeros(len(ns) + 1, dtype=np.int64); off[1:] = np.cumsum(ns)
     cat = ss_inputs.Catalog("cluster", np.concatenate(T), np.concatenate(Y), np.concatenate(E), off,
                             0.01, 20.0, 9, np.full(len(ns), np.nan))
-    res, ref = run_both(ss, cat, mode, oracle.FAST)
+    res, ref = run_both(ss, cat, mode, oracle.FAST, force_path=ss.PATH_CLUSTER)
     check_parity(cat, res.pgram, ref, mode, label="cluster variants")
     check_best(ref, res.best_index, res.best_freq, cat)
     t, y, e = cat.obj(0)
