@@ -24,7 +24,7 @@ from . import (CROSS_VALIDATION, GENERALIZED_VALIDATION, PATH_BLOCK, PATH_CLUSTE
                load,
                path_for_n, ss_periodogram)
 
-DEFAULT_NS = [50, 64, 96, 128, 160, 200, 256, 257, 320, 400, 512, 700, 1000, 1400, 2055, 2056, 3000, 5000, 10000, 20000, 40000]
+DEFAULT_NS = [50, 64, 96, 128, 160, 200, 256, 257, 320, 400, 512, 700, 1000, 1400, 2055, 2056, 3000, 3584, 3585, 5000, 10000, 20000, 40000]
 PATH_NAME = {PATH_WARP: "warp", PATH_GROUP: "group", PATH_CLUSTER: "cluster", PATH_BLOCK: "cta-smem", PATH_STAGE: "cta-staged"}
 WARP_MAX_N, BLOCK_MAX_N, GROUP_LONG_MAX_N, CLUSTER_MAX_N = 256, 2055, 3584, 40960
 
