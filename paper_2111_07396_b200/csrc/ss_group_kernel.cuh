@@ -218,7 +218,13 @@ struct GroupConst {
 // Resident CTAs per SM: 16 warps at 128 registers, except 4-warp CTAs with 6 or 7 points per thread, which spill less and
 // run faster at 12 warps / 168 registers (measured, CV: +11..13 % at C = 7, +2..3 % at C = 6; GV: C = 7 only)
 template <int G, int C, bool GV, typename T>
-constexpr int group_minb() { return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 : GroupCfg<G, C, T>::MINB; }
+constexpr int group_minb()
+{
+    // (8, 7) in fp64 CV spills 390 bytes at 128 registers; one CTA per SM at 255 registers and no spills is 13 % faster
+    // (1.94e10 -> 2.19e10 point-evals/s at n = 1,792; the same trade loses at (8, 6) and does not compile for GV)
+    if (G == 8 && C == 7 && sizeof(T) == 8 && !GV) return 1;
+    return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 : GroupCfg<G, C, T>::MINB;
+}
 
 // OPT: 0 = the default call; 1 = the listing's options compiled in: periodic windows (iper = 2,
 // PAPER.md:199-200) -- a window that leaves [0, n) is two ranges, the part that wrapped counting with abscissae x - 1
