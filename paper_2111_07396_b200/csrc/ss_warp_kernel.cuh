@@ -331,83 +331,78 @@ __device__ __forceinline__ void tmem_park(uint32_t taddr, const double (&v)[N])
     }
 }
 #undef SS_LOHI
-#define SS_O(i) "=r"(lo[i]), "=r"(hi[i])
-template <int N, int S0 = 0>
-__device__ __forceinline__ void tmem_issue_ld(uint32_t taddr, int (&lo)[N], int (&hi)[N])
+// Loads from tensor memory are asynchronous: the destination registers are valid only after tcgen05.wait::ld.  The
+// loads and the wait therefore form ONE asm statement -- were they separate, the compiler would regard the destinations
+// as defined after the load and would be free to copy or spill them before the data has landed.  (Early-clobber
+// outputs: a destination must not share a register with the address of a later load of the same statement.)
+// 32-bit words (the loop-invariant window indices, parked floats)
+template <int N>
+__device__ __forceinline__ void tmem_fetch_words(uint32_t taddr, int (&v)[N])
 {
-    if constexpr (N - S0 >= 4) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                     : SS_O(S0), SS_O(S0 + 1), SS_O(S0 + 2), SS_O(S0 + 3) : "r"(taddr + 2 * S0) : "memory");
-        tmem_issue_ld<N, S0 + 4>(taddr, lo, hi);
-    } else if constexpr (N - S0 >= 2) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
-                     : SS_O(S0), SS_O(S0 + 1) : "r"(taddr + 2 * S0) : "memory");
-        tmem_issue_ld<N, S0 + 2>(taddr, lo, hi);
-    } else if constexpr (N - S0 == 1) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : SS_O(S0) : "r"(taddr + 2 * S0) : "memory");
-    }
+    static_assert(N >= 2 && N <= 16 && N % 2 == 0, "tmem_fetch_words: 2..16 words, even");
+    if constexpr (N == 2)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1])
+                     : "r"(taddr + 0) : "memory");
+    else if constexpr (N == 4)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3])
+                     : "r"(taddr + 0) : "memory");
+    else if constexpr (N == 6)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%6];\n\t"
+                     "tcgen05.ld.sync.aligned.32x32b.x2.b32 {%4, %5}, [%7];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3]), "=&r"(v[4]), "=&r"(v[5])
+                     : "r"(taddr + 0), "r"(taddr + 4) : "memory");
+    else if constexpr (N == 8)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3]), "=&r"(v[4]), "=&r"(v[5]), "=&r"(v[6]), "=&r"(v[7])
+                     : "r"(taddr + 0) : "memory");
+    else if constexpr (N == 10)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%10];\n\t"
+                     "tcgen05.ld.sync.aligned.32x32b.x2.b32 {%8, %9}, [%11];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3]), "=&r"(v[4]), "=&r"(v[5]), "=&r"(v[6]), "=&r"(v[7]), "=&r"(v[8]), "=&r"(v[9])
+                     : "r"(taddr + 0), "r"(taddr + 8) : "memory");
+    else if constexpr (N == 12)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%12];\n\t"
+                     "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%8, %9, %10, %11}, [%13];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3]), "=&r"(v[4]), "=&r"(v[5]), "=&r"(v[6]), "=&r"(v[7]), "=&r"(v[8]), "=&r"(v[9]), "=&r"(v[10]), "=&r"(v[11])
+                     : "r"(taddr + 0), "r"(taddr + 8) : "memory");
+    else if constexpr (N == 14)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%14];\n\t"
+                     "tcgen05.ld.sync.aligned.32x32b.x4.b32 {%8, %9, %10, %11}, [%15];\n\t"
+                     "tcgen05.ld.sync.aligned.32x32b.x2.b32 {%12, %13}, [%16];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3]), "=&r"(v[4]), "=&r"(v[5]), "=&r"(v[6]), "=&r"(v[7]), "=&r"(v[8]), "=&r"(v[9]), "=&r"(v[10]), "=&r"(v[11]), "=&r"(v[12]), "=&r"(v[13])
+                     : "r"(taddr + 0), "r"(taddr + 8), "r"(taddr + 12) : "memory");
+    else if constexpr (N == 16)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%16];\n\t"
+                     "tcgen05.ld.sync.aligned.32x32b.x8.b32 {%8, %9, %10, %11, %12, %13, %14, %15}, [%17];\n\t"
+                     "tcgen05.wait::ld.sync.aligned;"
+                     : "=&r"(v[0]), "=&r"(v[1]), "=&r"(v[2]), "=&r"(v[3]), "=&r"(v[4]), "=&r"(v[5]), "=&r"(v[6]), "=&r"(v[7]), "=&r"(v[8]), "=&r"(v[9]), "=&r"(v[10]), "=&r"(v[11]), "=&r"(v[12]), "=&r"(v[13]), "=&r"(v[14]), "=&r"(v[15])
+                     : "r"(taddr + 0), "r"(taddr + 8) : "memory");
 }
-#undef SS_O
+// doubles: two words each, low word first
 template <int N>
 __device__ __forceinline__ void tmem_fetch(uint32_t taddr, double (&v)[N])
 {
-    int lo[N], hi[N];
-    tmem_issue_ld<N>(taddr, lo, hi);
-    // the loaded registers are valid only after the wait: tie them to it (one wait per fetch)
-    static_assert(N >= 2 && N <= 8, "tmem_fetch: 2..8 doubles");
-#define SS_T(i) "+r"(lo[i < N ? i : 0]), "+r"(hi[i < N ? i : 0])
-    if (N == 2) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1) :: "memory");
-    else if (N == 3) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2) :: "memory");
-    else if (N == 4) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3) :: "memory");
-    else if (N == 5) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4) :: "memory");
-    else if (N == 6) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5) :: "memory");
-    else if (N == 7) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6) :: "memory");
-    else asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6), SS_T(7) :: "memory");
-#undef SS_T
+    static_assert(N >= 1 && N <= 8, "tmem_fetch: 1..8 doubles");
+    int w[2 * N];
+    tmem_fetch_words<2 * N>(taddr, w);
 #pragma unroll
-    for (int s = 0; s < N; s++) v[s] = __hiloint2double(hi[s], lo[s]);
+    for (int s = 0; s < N; s++) v[s] = __hiloint2double(w[2 * s + 1], w[2 * s]);
 }
-// 32-bit words (the loop-invariant window indices)
 template <int N>
 __device__ __forceinline__ void tmem_park_words(uint32_t taddr, const int (&v)[N])
 {
 #pragma unroll
     for (int s = 0; s < N; s++)
         asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" :: "r"(taddr + s), "r"(v[s]) : "memory");
-}
-template <int N, int S0 = 0>
-__device__ __forceinline__ void tmem_issue_ld_words(uint32_t taddr, int (&v)[N])
-{
-    if constexpr (N - S0 >= 8) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
-                     : "=r"(v[S0]), "=r"(v[S0 + 1]), "=r"(v[S0 + 2]), "=r"(v[S0 + 3]), "=r"(v[S0 + 4]), "=r"(v[S0 + 5]),
-                       "=r"(v[S0 + 6]), "=r"(v[S0 + 7]) : "r"(taddr + S0) : "memory");
-        tmem_issue_ld_words<N, S0 + 8>(taddr, v);
-    } else if constexpr (N - S0 >= 4) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
-                     : "=r"(v[S0]), "=r"(v[S0 + 1]), "=r"(v[S0 + 2]), "=r"(v[S0 + 3]) : "r"(taddr + S0) : "memory");
-        tmem_issue_ld_words<N, S0 + 4>(taddr, v);
-    } else if constexpr (N - S0 >= 2) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];"
-                     : "=r"(v[S0]), "=r"(v[S0 + 1]) : "r"(taddr + S0) : "memory");
-        tmem_issue_ld_words<N, S0 + 2>(taddr, v);
-    }
-}
-template <int N>
-__device__ __forceinline__ void tmem_fetch_words(uint32_t taddr, int (&v)[N])
-{
-    static_assert(N >= 2 && N <= 16 && N % 2 == 0, "tmem_fetch_words: 2..16 words, even");
-    tmem_issue_ld_words<N>(taddr, v);
-#define SS_T(i) "+r"(v[2 * (i) < N ? 2 * (i) : 0]), "+r"(v[2 * (i) + 1 < N ? 2 * (i) + 1 : 1])
-    if (N == 2) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0) :: "memory");
-    else if (N == 4) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1) :: "memory");
-    else if (N == 6) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2) :: "memory");
-    else if (N == 8) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3) :: "memory");
-    else if (N == 10) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4) :: "memory");
-    else if (N == 12) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5) :: "memory");
-    else if (N == 14) asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6) :: "memory");
-    else asm volatile("tcgen05.wait::ld.sync.aligned;" : SS_T(0), SS_T(1), SS_T(2), SS_T(3), SS_T(4), SS_T(5), SS_T(6), SS_T(7) :: "memory");
-#undef SS_T
 }
 // N words, N odd or even: an odd count reads one column more (the caller's tables leave it allocated)
 template <int N>
