@@ -58,7 +58,7 @@ def parse():
     ap.add_argument("--objects", type=int, default=None, help="(debug) fewer objects than the config has (configs 3, 4)")
     ap.add_argument("--freqs", type=int, default=None, help="(debug) fewer frequencies than the config has")
     ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
-                    help="mixed = the paper's FP32 switch as built here (fp32 smoother for n <= 2,055; never the headline)")
+                    help="mixed = the paper's FP32 switch as built here (fp32 smoother for n <= 3,584; never the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     return ap.parse_args()

@@ -61,7 +61,7 @@ typedef enum {
     SS_PATH_STAGE = 3, /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
     SS_PATH_GROUP = 4, /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_LONG_MAX_N;
                           points in registers, prefix sums in shared memory, smooths in tensor memory.
-                          Up to SS_GROUP_MAX_N with every option; beyond it the fp64 default call only     */
+                          Up to SS_GROUP_MAX_N with every option; beyond it the default call only (fp64 / mixed) */
     SS_PATH_CLUSTER = 5 /* a thread-block cluster of 2..16 CTAs per (object, frequency); SS_GROUP_LONG_MAX_N <
                           n <= SS_CLUSTER_MAX_N; prefix sums in distributed shared memory                  */
 } ss_path_t;
@@ -97,7 +97,7 @@ typedef struct {
                                grid.  k_count = 0: up to the end of the grid.  For splitting one object's
                                frequency range across GPUs.                           */
     int precision;          /* ss_precision_t.  SS_PRECISION_F64 (default): everything in fp64.  SS_PRECISION_MIXED
-                               (the paper's FP32 switch): for objects of n <= SS_GROUP_MAX_N
+                               (the paper's FP32 switch): for objects of n <= SS_GROUP_LONG_MAX_N
                                points (warp and group paths, default listing options) the smoother runs in fp32 --
                                prefix arrays stored and window fits, residuals, span selection and interpolation
                                computed in float -- while the fold, the sort, the centring and the accumulation of

@@ -521,7 +521,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             // of, and a near-singular window (7 points inside a seasonal gap's edge) misses the 1e-9 bar by prefix
             // differences at n > 256 (measured 1.03e-9); the CTA-per-eval kernels sum such windows directly
             if (path == SS_PATH_GROUP && o.span > 0.0 && o.span < SPAN0) path = SS_PATH_BLOCK;
-            // beyond SS_GROUP_MAX_N the group path has the fp64 default kernels only
+            // beyond SS_GROUP_MAX_N the group path serves the default call only (fp64 or mixed precision)
             if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N && has_listing_options(o)) path = SS_PATH_STAGE;
             if (path == SS_PATH_GROUP && r.n > SS_GROUP_LONG_MAX_N) path = SS_PATH_CLUSTER;
             if (path == SS_PATH_CLUSTER && has_listing_options(o)) path = SS_PATH_STAGE;
@@ -533,7 +533,7 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
                                                  : warp_variant_for_n(r.n) + (o.precision == SS_PRECISION_MIXED ? WARP_VARIANT_F32 : 0);
             else if (path == SS_PATH_GROUP)
                 variant = group_variant_for_n(r.n) + (has_listing_options(o) ? GROUP_VARIANT_OPT
-                                                      : o.precision == SS_PRECISION_MIXED && r.n <= SS_GROUP_MAX_N ? GROUP_VARIANT_F32 : 0);
+                                                      : o.precision == SS_PRECISION_MIXED ? GROUP_VARIANT_F32 : 0);
             else if (path == SS_PATH_CLUSTER) variant = cluster_variant_for_n(r.n);
             // CTA size by n (profiles/r1g_crossover.md): 128 threads up to 512 points, 256 up to 1,020, 512 beyond
             else if (path == SS_PATH_BLOCK) variant = r.n <= 512 ? 3 : (r.n <= 1020 ? 1 : 2);

@@ -844,14 +844,14 @@ MIXED_MEDIAN = 2e-6    # the typical value (measured 2e-7)
 @pytest.mark.parametrize("mode", [CV, GV])
 def test_mixed_precision_mode(ss, mode):
     """precision = SS_PRECISION_MIXED: fp64 fold / sort / prefix accumulation, fp32 smoother,
-    for n <= 2,055 (warp and group paths).  (a) every periodogram value within MIXED_ATOL of the fp64 ORACLE; (b) the
+    for n <= 3,584 (warp and group paths).  (a) every periodogram value within MIXED_ATOL of the fp64 ORACLE; (b) the
     paper's criterion: the best period within 3 % of the fp64 one for at least 93 % of the objects (the
     paper reports 93.0-95.4 %); (c) longer objects are served in fp64 and keep the fp64 bits."""
     cat = ss_inputs.config4(n_objects=40, n_freq=3000)
     small = ss_inputs.config3(n_objects=60, n_freq=3000)
     rng = np.random.default_rng(99)
-    nl = 2100
-    tl = np.sort(rng.integers(0, 1500, size=nl) + rng.uniform(0.0, 0.3, size=nl))
+    nl = 3700
+    tl = np.sort(rng.integers(0, 2500, size=nl) + rng.uniform(0.0, 0.3, size=nl))
     el = rng.uniform(0.01, 0.2, size=nl)
     yl = 15 + 0.3 * np.sin(2 * np.pi * tl / 1.37) + rng.normal(0, 1.0, size=nl) * el
     times = np.concatenate([cat.times, small.times, tl]); mags = np.concatenate([cat.mags, small.mags, yl])
@@ -871,11 +871,11 @@ def test_mixed_precision_mode(ss, mode):
         assert not np.array_equal(mix.pgram[lo:hi], f64.pgram[lo:hi])           # the fp32 smoother really ran
         match = np.abs(1.0 / mix.best_freq[lo:hi] - 1.0 / bf_ref[lo:hi]) <= 0.03 / bf_ref[lo:hi]
         assert match.mean() >= 0.93, match.mean()
-    assert np.array_equal(mix.pgram[n_f32:], f64.pgram[n_f32:])                  # n > 2,055: fp64, same bits
+    assert np.array_equal(mix.pgram[n_f32:], f64.pgram[n_f32:])                  # n > 3,584: fp64, same bits
     # every (G, C) variant of the float kernel
     rng = np.random.default_rng(717)
     ns = [40, 64, 65, 96, 100, 128, 150, 160, 170, 192, 200, 224, 250, 256,      # every warp variant (C, IBW0)
-          257, 384, 500, 640, 700, 768, 1000, 1280, 1400, 1536, 2048, 2055]
+          257, 384, 500, 640, 700, 768, 1000, 1280, 1400, 1536, 2048, 2055, 2560, 3072, 3584]
     T, Y, E = [], [], []
     for i, n in enumerate(ns):
         t = np.sort(rng.integers(0, 1200, size=n) + rng.uniform(0.0, 0.3, size=n))
