@@ -18,6 +18,8 @@ from __future__ import annotations
 import argparse
 import sys
 
+import time
+
 import numpy as np
 
 from . import (CROSS_VALIDATION, GENERALIZED_VALIDATION, PATH_BLOCK, PATH_CLUSTER, PATH_GROUP, PATH_STAGE, PATH_WARP, default_options,
@@ -96,8 +98,9 @@ def options_table(torch, dev, md):
     return 0
 
 
-def _best_of(torch, call, reps=3):
-    import time
+def _best_of(torch, call, reps=4):
+    """Best wall time of `reps` calls after one untimed call (module load, clocks)."""
+    call()
     best = float("inf")
     for _ in range(reps):
         torch.cuda.synchronize()
@@ -140,8 +143,12 @@ def mixed_table(torch, dev, md):
     """precision = SS_PRECISION_MIXED (fp32 smoother on the warp and group paths) against fp64."""
     import ss_inputs
     lines = ["| catalog | mode | fp64 evals/s | mixed evals/s | speed-up |", "|---|---|---|---|---|"]
+    # the third catalog: eight light curves of the paper's ObjLarge length (N_t = 3,554, PAPER.md:504-516)
+    t3, y3, e3, o3 = catalog(3554, 8, seed=3554)
+    long = ss_inputs.Catalog("long", t3, y3, e3, o3, 0.5, 24.0, 20000, np.full(8, np.nan))
     for cat, label in ((ss_inputs.config3(n_objects=1000, n_freq=5000), "config 3 shape, 1,000 x 5,000 (warp path)"),
-                       (ss_inputs.config4(n_objects=300, n_freq=4000), "config 4 shape, 300 x 4,000 (group path)")):
+                       (ss_inputs.config4(n_objects=300, n_freq=4000), "config 4 shape, 300 x 4,000 (group path)"),
+                       (long, "n = 3,554, 8 x 20,000 (group path, 16 warps x 7 points)")):
         a = [torch.as_tensor(v, device=dev) for v in (cat.times, cat.mags, cat.errs, cat.offsets)]
         pg = torch.empty((cat.n_objects, cat.n_freq), dtype=torch.float64, device=dev)
         for mode, name in ((CROSS_VALIDATION, "cv"), (GENERALIZED_VALIDATION, "gv")):
