@@ -61,7 +61,7 @@ typedef enum {
     SS_PATH_STAGE = 3, /* one CTA per (object, frequency); per-eval arrays staged in global memory/L2  */
     SS_PATH_GROUP = 4, /* 4, 8 or 16 warps per (object, frequency); SS_WARP_MAX_N < n <= SS_GROUP_LONG_MAX_N;
                           points in registers, prefix sums in shared memory, smooths in tensor memory.
-                          Up to SS_GROUP_MAX_N with every option; beyond it the default call only (fp64 / mixed) */
+                          Beyond 2,560 points the object's y and w are read from global memory per eval    */
     SS_PATH_CLUSTER = 5 /* a thread-block cluster of 2..16 CTAs per (object, frequency); SS_GROUP_LONG_MAX_N <
                           n <= SS_CLUSTER_MAX_N; prefix sums in distributed shared memory                  */
 } ss_path_t;
@@ -76,7 +76,7 @@ typedef struct {
     double span;            /* 0 = variable span (default).  In (0, 1]: Listing 1's fixed-span branch
                                (PAPER.md:202-210): one running-line smooth at this span, in both modes.
                                Served by the warp kernels for n <= SS_WARP_MAX_N, by the group kernels for
-                               n <= SS_GROUP_MAX_N when span >= 0.05, by the CTA-per-eval kernels otherwise;
+                               n <= SS_GROUP_LONG_MAX_N when span >= 0.05, by the CTA-per-eval kernels otherwise;
                                always in fp64.                                                           */
     int iper;               /* 1 = windows pinned at the ends (default, R8).  2 = periodic windows
                                (PAPER.md:199-200): the window of point j is j-ibw..j+ibw modulo n, phases
@@ -108,7 +108,7 @@ typedef struct {
                                fp64 throughput for n <= SS_WARP_MAX_N.                                             */
     int shared_times;       /* 1 = every object of the catalog has the SAME time stamps in the same order (one field
                                observed together).  The fold and the sort are then done once per
-                               frequency for 4 objects at a time (objects of n <= SS_GROUP_MAX_N, fp64 precision,
+                               frequency for 4 objects at a time (objects of n <= SS_GROUP_LONG_MAX_N, fp64 precision,
                                default listing options; otherwise the objects are served one by one as usual).
                                Checked on the device unless skip_validation is set: a catalog
                                whose time arrays differ is SS_ERR_INVALID_ARG.  Results equal those of

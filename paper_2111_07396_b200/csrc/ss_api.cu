@@ -521,8 +521,6 @@ ss_status_t Engine::setup(const double* times, const double* mags, const double*
             // of, and a near-singular window (7 points inside a seasonal gap's edge) misses the 1e-9 bar by prefix
             // differences at n > 256 (measured 1.03e-9); the CTA-per-eval kernels sum such windows directly
             if (path == SS_PATH_GROUP && o.span > 0.0 && o.span < SPAN0) path = SS_PATH_BLOCK;
-            // beyond SS_GROUP_MAX_N the group path serves the default call only (fp64 or mixed precision)
-            if (path == SS_PATH_GROUP && r.n > SS_GROUP_MAX_N && has_listing_options(o)) path = SS_PATH_STAGE;
             if (path == SS_PATH_GROUP && r.n > SS_GROUP_LONG_MAX_N) path = SS_PATH_CLUSTER;
             if (path == SS_PATH_CLUSTER && has_listing_options(o)) path = SS_PATH_STAGE;
             if (path == SS_PATH_CLUSTER && (r.n > SS_CLUSTER_MAX_N || r.n < 2 * 512)) path = SS_PATH_STAGE;
@@ -651,7 +649,7 @@ ss_status_t Engine::run_tile(int obj_tile, int64_t k_begin, int64_t k_end, int f
         p.defer_entries = defer_entries; p.defer_count = defer_count; p.defer_capacity = defer_capacity;
         // one fold + sort per group of objects (fp64 kernels with default options)
         const bool shared = opt.shared_times && ((c.path == SS_PATH_WARP && c.variant < WARP_VARIANT_F32) ||
-                                                 (c.path == SS_PATH_GROUP && c.variant < GROUP_VARIANT_F32 && c.max_n <= SS_GROUP_MAX_N));
+                                                 (c.path == SS_PATH_GROUP && c.variant < GROUP_VARIANT_F32));
         const int64_t n_items = (shared ? ((int64_t)p.n_list + SHARED_TIMES_M - 1) / SHARED_TIMES_M : (int64_t)p.n_list) * cpo;
         if (n_items > 0x7fffffffLL) return fail(SS_ERR_UNSUPPORTED, "too many work items in one tile");
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;

@@ -44,10 +44,7 @@ ss_status_t SS_TU_FN(const EvalParams& p, int c, int mode, int64_t n_items, cuda
 #endif
     (void)mode;
     switch (c) {
-        SS_OPT_CASE(3) SS_OPT_CASE(4) SS_OPT_CASE(5)
-#if SS_TU_G != 16
-        SS_OPT_CASE(6) SS_OPT_CASE(7)
-#endif
+        SS_OPT_CASE(3) SS_OPT_CASE(4) SS_OPT_CASE(5) SS_OPT_CASE(6) SS_OPT_CASE(7)
         default: return SS_ERR_UNSUPPORTED;
     }
 #undef SS_OPT_CASE
@@ -63,11 +60,8 @@ ss_status_t SS_TU_FN(const EvalParams& p, int c, int64_t n_items, cudaStream_t s
         case 3: return launch_group_variant<SS_TU_G, 3, GV, tu_real, SS_TU_OPT>(p, n_items, stream);
         case 4: return launch_group_variant<SS_TU_G, 4, GV, tu_real, SS_TU_OPT>(p, n_items, stream);
         case 5: return launch_group_variant<SS_TU_G, 5, GV, tu_real, SS_TU_OPT>(p, n_items, stream);
-        // 16 warps x 6 or 7 points (3,072 / 3,584): the default call only, fp64 or mixed (SS_GROUP_LONG_MAX_N)
-#if SS_TU_G != 16 || SS_TU_F32 <= 1
         case 6: return launch_group_variant<SS_TU_G, 6, GV, tu_real, SS_TU_OPT>(p, n_items, stream);
         case 7: return launch_group_variant<SS_TU_G, 7, GV, tu_real, SS_TU_OPT>(p, n_items, stream);
-#endif
         default: return SS_ERR_UNSUPPORTED;
     }
 }

@@ -14,7 +14,7 @@ constexpr int64_t BLOCK_SMEM_MAX = 232448 - 2048;   // dynamic part; 2 KB left f
 constexpr int64_t BLOCK_BYTES_PER_POINT = 14 * 8;
 constexpr int64_t BLOCK_MAX_N = BLOCK_SMEM_MAX / BLOCK_BYTES_PER_POINT - 2;   // 2055
 
-static_assert(SS_GROUP_MAX_N <= BLOCK_MAX_N, "what the group path hands over must fit the generic shared-memory kernel");
+static_assert(SS_GROUP_MAX_N == BLOCK_MAX_N, "SS_GROUP_MAX_N: up to here the group path's hand-over fits the generic shared-memory kernel; beyond it uses the staging scratch");
 
 inline int path_for_n(int64_t n, int /*mode*/)
 {
@@ -42,7 +42,7 @@ inline int cluster_variant_for_n(int n)
 
 // Group-path kernel variant of an object: G warps x C points per thread, the smallest capacity 32*G*C >= n among
 // (4,3) 384, (4,4) 512, (4,5) 640, (4,6) 768, (8,4) 1,024, (8,5) 1,280, (8,6) 1,536, (16,4) 2,048, (16,5) 2,560, and for
-// the fp64 default call alone (SS_GROUP_MAX_N < n <= SS_GROUP_LONG_MAX_N) (16,6) 3,072, (16,7) 3,584.  More
+// SS_GROUP_MAX_N < n <= SS_GROUP_LONG_MAX_N (y, w gathered from global memory) (16,6) 3,072, (16,7) 3,584.  More
 // points per thread beat more warps per eval (measured: (8,6) 2.37e10 point-evals/s at n = 1,400 where (16,3) gave
 // 1.85e10; (4,6) 2.49e10 at n = 700 where (8,3) gave 2.23e10); C = 6 is what tensor memory allows at 16 warps per SM
 // (20C columns per warp <= 128).  id = G*8 + C.

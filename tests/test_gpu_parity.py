@@ -355,12 +355,13 @@ def test_periodic_windows_and_fixed_span(ss, mode, opts):
 @pytest.mark.parametrize("mode", [CV, GV])
 @pytest.mark.parametrize("opts", LISTING_OPTIONS, ids=lambda o: ",".join(f"{k}={v}" for k, v in o.items()))
 def test_listing_options_on_the_group_path(ss, mode, opts):
-    """iper = 2 / span > 0 for 256 < n <= 2,055 are served by group_kernel<.., OPT> (the wrapped part of a periodic
+    """iper = 2 / span > 0 for 256 < n <= 3,584 are served by group_kernel<.., OPT> (the wrapped part of a periodic
     window as a second range with shifted abscissae, found by arithmetic): one object per (G, C) variant, one with a
     duplicated time stamp (handed over whole), one with integer-day times that tie at f = 1 / d, against the oracle,
     best index included."""
     rng = np.random.default_rng(919)
-    ns = [257, 384, 500, 513, 600, 640, 700, 768, 850, 1000, 1280, 1400, 1536, 1700, 1792, 2048, 2055, 300, 420]
+    ns = [257, 384, 500, 513, 600, 640, 700, 768, 850, 1000, 1280, 1400, 1536, 1700, 1792, 2048, 2055, 2560, 3072, 3584,
+          300, 420]
     T, Y, E = [], [], []
     for i, n in enumerate(ns):
         t = np.sort(rng.integers(0, 900, size=n) + rng.uniform(0.0, 0.33, size=n))
@@ -915,7 +916,8 @@ def test_shared_time_sampling_reuses_the_sort(ss, mode):
     a catalog whose time stamps differ is refused."""
     # n <= 256: warp_shared_kernel; beyond: group_kernel<.., 3> (one (G, C) variant per warp count, and the largest)
     for n_objects, n, dup in ((37, 150, False), (9, 64, False), (6, 200, False), (5, 256, False), (7, 90, True),
-                              (9, 700, False), (6, 1100, False), (5, 2055, False), (7, 400, True), (3, 257, False)):
+                              (9, 700, False), (6, 1100, False), (5, 2055, False), (7, 400, True), (3, 257, False),
+                              (5, 3000, False), (3, 3584, False)):
         t, y, e, off = _shared_times_catalog(n_objects, n, seed=n, dup=dup)
         plain = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode)
         shared = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode, shared_times=1)

@@ -57,7 +57,7 @@ def test_path_classes():
     assert ss.path_for_n(257) == ss.PATH_GROUP
     assert ss.path_for_n(2000) == ss.PATH_GROUP
     assert ss.path_for_n(2055) == ss.PATH_GROUP
-    assert ss.path_for_n(2056) == ss.PATH_GROUP          # fp64 default call; options go to the CTA kernels
+    assert ss.path_for_n(2056) == ss.PATH_GROUP          # the long group variants (y, w read from global memory)
     assert ss.path_for_n(3584) == ss.PATH_GROUP
     assert ss.path_for_n(3585) == ss.PATH_CLUSTER
     assert ss.path_for_n(20000) == ss.PATH_CLUSTER
