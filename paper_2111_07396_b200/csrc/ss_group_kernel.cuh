@@ -223,6 +223,8 @@ constexpr int group_minb()
     // (8, 7) in fp64 CV spills 390 bytes at 128 registers; one CTA per SM at 255 registers and no spills is 13 % faster
     // (1.94e10 -> 2.19e10 point-evals/s at n = 1,792; the same trade loses at (8, 6) and does not compile for GV)
     if (G == 8 && C == 7 && sizeof(T) == 8 && !GV) return 1;
+    // (4, 3) fits 96 registers: 20 warps per SM, +6 % CV / +4 % GV at n = 257..384 (24 warps at 80 registers lose again)
+    if (G == 4 && C == 3 && sizeof(T) == 8) return 5;
     return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 : GroupCfg<G, C, T>::MINB;
 }
 

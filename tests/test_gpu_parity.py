@@ -922,8 +922,10 @@ def test_shared_time_sampling_reuses_the_sort(ss, mode):
         plain = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode)
         shared = ss.periodogram(t, y, e, off, 0.5, 24.0, 131, mode, shared_times=1)
         # the same arithmetic in the same order; the compiler is free to contract a*b+c differently in the two kernels
-        # (seen: 4e-16 on P for the 8-points-per-lane variant), so equality is to rounding, not to the bit
-        assert np.allclose(shared.pgram, plain.pgram, rtol=1e-13, atol=1e-14), (n_objects, n)
+        # (seen: 4e-16 on P for the 8-points-per-lane variant, 2.6e-14 on P = 0.06 -- one ulp of chi2 -- for the 4-warp x
+        # 3-point group kernel, whose two instantiations differ in register budget), so equality is to rounding, not to
+        # the bit: three orders inside the parity bar
+        assert np.allclose(shared.pgram, plain.pgram, rtol=1e-12, atol=1e-13), (n_objects, n)
         assert np.array_equal(shared.best_index, plain.best_index) and np.array_equal(shared.best_freq, plain.best_freq)
         if n_objects == 9:
             cat = ss_inputs.Catalog("shared", t, y, e, off, 0.5, 24.0, 131, np.full(n_objects, np.nan))
@@ -939,7 +941,7 @@ def test_shared_time_sampling_reuses_the_sort(ss, mode):
         off = np.arange(6, dtype=np.int64) * n
         plain = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode)
         shared = ss.periodogram(T, Y, E, off, 0.25, 1.25, 4, mode, shared_times=1)
-        assert np.allclose(shared.pgram, plain.pgram, rtol=1e-13, atol=1e-14) and np.array_equal(shared.best_index, plain.best_index)
+        assert np.allclose(shared.pgram, plain.pgram, rtol=1e-12, atol=1e-13) and np.array_equal(shared.best_index, plain.best_index)
     # not actually shared
     T2 = T.copy(); T2[3 * n + 5] += 1e-9
     with pytest.raises(ss.SSError) as ei:
