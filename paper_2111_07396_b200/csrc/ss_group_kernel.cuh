@@ -223,6 +223,14 @@ constexpr int group_minb()
     // (8, 7) in fp64 CV spills 390 bytes at 128 registers; one CTA per SM at 255 registers and no spills is 13 % faster
     // (1.94e10 -> 2.19e10 point-evals/s at n = 1,792; the same trade loses at (8, 6) and does not compile for GV)
     if (G == 8 && C == 7 && sizeof(T) == 8 && !GV) return 1;
+    // T = float needs half the registers, tensor-memory columns and prefix-array bytes: 32 warps per SM at 64 registers
+    // for C <= 4, 24 at 80 for C = 5, 6, 16 at 128 for C = 7 (measured per variant: CV +2..16 %, GV +2..30 % over the
+    // fp64 shapes; the one loser, (4, 5) GV, keeps 16 warps)
+    if (sizeof(T) == 4) {
+        if (G == 4) return C <= 4 ? 8 : (C <= 6 ? ((C == 5 && GV) ? 4 : 6) : 4);
+        if (G == 8) return C <= 4 ? 4 : (C <= 6 ? 3 : 2);
+        return C <= 4 ? 2 : 1;
+    }
     // (4, 3) fits 96 registers: 20 warps per SM, +6 % CV / +4 % GV at n = 257..384 (24 warps at 80 registers lose again)
     if (G == 4 && C == 3 && sizeof(T) == 8) return 5;
     return (G == 4 && (C >= 7 || (C >= 6 && !GV))) ? 3 : GroupCfg<G, C, T>::MINB;
