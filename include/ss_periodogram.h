@@ -160,7 +160,10 @@ ss_status_t ss_periodogram_ex(const double *times, const double *mags, const dou
  * pinned).  The library copies the catalog to the device, tiles objects x frequencies with the batch
  * planner so the device-side periodogram tile plus workspace stays under opt->workspace_cap
  * (the batching scheme), overlaps the device->host copy of finished tiles with the
- * next tile's kernels, and returns when every output has landed in host memory.
+ * next tile's kernels, and returns when every output has landed in host memory.  The overlap needs
+ * PAGE-LOCKED output arrays (cudaHostAlloc / cudaHostRegister): a copy into pageable memory blocks the
+ * host until it is done, so the next tile's kernels are launched only afterwards -- same results, the
+ * copies and the kernels then alternate instead of overlapping (bench.py's e2e leg uses pinned buffers).
  */
 ss_status_t ss_periodogram_host(const double *times, const double *mags, const double *errs,
                                 const int64_t *offsets, int64_t n_objects,
